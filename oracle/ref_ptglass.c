@@ -1,0 +1,475 @@
+/*
+ * ref_ptglass.c -- CPU ORACLE (TEST INFRASTRUCTURE ONLY; see ref_ptglass.h).
+ *
+ * Plain single-threaded C, int8 spins and couplings, one site at a time, in the paper's order and
+ * notation.  No blocking, no bit tricks, no shared code with the CUDA path.  Each function cites the
+ * passage of /root/reference/PAPER.md ("P:n") or the DESIGN.md reading ("Rk") it follows.
+ *
+ * Pins (tests/test_oracle_*.py): Philox known answers; gauge / ferromagnet / brute-force energy; beta=0 and
+ * beta=50 sweeps; incremental == recomputed energy; PT cyclic shift and Eq. (5) decision grid; Houdayer
+ * E1+E2, Q, QL conservation, involution, union-find component; exact enumeration of <E>, <q^2> at 2D L=4
+ * and <E> at 3D L=2; sharding invariance; the survey's worked examples W1-W3.  The 10^4-MCS trajectories of
+ * configs C2-C5 themselves are "parity unpinned" beyond oracle == GPU.
+ */
+#include "ref_ptglass.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+struct ref_ctx {
+    int L, d, S, T, N;
+    uint64_t seed;
+    uint32_t sample_offset;
+    double *betas;        /* [T] */
+    int8_t *J;            /* [S][d][N]       J[mu][i] = bond i -> i+e_mu */
+    int8_t *spin;         /* [S][2][T][N]    slot order */
+    int32_t *E;           /* [S][2][T]       slot order */
+    int32_t *temp_of_slot;/* [S][2][T] */
+    int32_t *slot_of_temp;/* [S][2][T] */
+    uint32_t *thrM;       /* [T][d] */
+    int *sgn;             /* [T-1] */
+    uint64_t *attempts, *accepts; /* [S][2][T-1] */
+    uint32_t *last_size;  /* [S][T] */
+    uint64_t *cum_size;   /* [S][T] */
+    uint32_t n_sweep, n_exchange, n_houdayer;
+    int *nbr;             /* [N][2d]: nbr[i][2mu] = i+e_mu, nbr[i][2mu+1] = i-e_mu */
+    int *queue;           /* [N] BFS queue */
+    uint8_t *mark;        /* [N] */
+};
+
+/* ---------------------------------------------------------------- Philox4x32-10, ref. [70] */
+
+void ref_philox4x32_10(const uint32_t key[2], const uint32_t ctr[4], uint32_t out[4])
+{
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)M0 * c0;
+        uint64_t p1 = (uint64_t)M1 * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        uint32_t n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        uint32_t n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += W0; k1 += W1;          /* key bumped after each round; round r uses key + r*W */
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* Counter convention 8(c).1 (R11): key = seed, ctr = (index, step, global sample, TAG). */
+static uint32_t draw(const ref_ctx *c, uint32_t index, uint32_t step, uint32_t g, int domain, int aux,
+                     int chain, int idx16, int word)
+{
+    uint32_t key[2] = { (uint32_t)(c->seed & 0xFFFFFFFFu), (uint32_t)(c->seed >> 32) };
+    uint32_t ctr[4] = { index, step, g,
+                        ((uint32_t)domain << 28) | ((uint32_t)aux << 24) | ((uint32_t)chain << 16) |
+                            (uint32_t)idx16 };
+    uint32_t out[4];
+    ref_philox4x32_10(key, ctr, out);
+    return out[word];
+}
+
+static int8_t sign_of(uint32_t w) { return (w >> 31) == 0 ? (int8_t)1 : (int8_t)-1; }
+
+/* ---------------------------------------------------------------- thresholds (R5, R6) */
+
+uint32_t ref_threshold(double x)
+{
+    double v = floor(ldexp(exp(x), 32));
+    if (v >= 4294967295.0) return 4294967295u;
+    if (v <= 0.0) return 0u;
+    return (uint32_t)v;
+}
+
+static uint32_t thrX_of(const ref_ctx *c, int t, long m)
+{
+    return ref_threshold(-(fabs(c->betas[t + 1] - c->betas[t]) * (double)(4 * m)));
+}
+
+/* ---------------------------------------------------------------- lattice */
+
+static void build_neighbours(ref_ctx *c)
+{
+    int L = c->L, d = c->d;
+    for (int i = 0; i < c->N; ++i) {
+        int x[3] = { i % L, (i / L) % L, d == 3 ? i / (L * L) : 0 };
+        int stride = 1;
+        for (int mu = 0; mu < d; ++mu) {
+            int up = (x[mu] + 1) % L, dn = (x[mu] + L - 1) % L;
+            c->nbr[i * 2 * d + 2 * mu]     = i + (up - x[mu]) * stride;
+            c->nbr[i * 2 * d + 2 * mu + 1] = i + (dn - x[mu]) * stride;
+            stride *= L;
+        }
+    }
+}
+
+static int colour_of(const ref_ctx *c, int i)
+{
+    int L = c->L;
+    return ((i % L) + (i / L) % L + (c->d == 3 ? i / (L * L) : 0)) & 1;
+}
+
+/* E = -sum_{mu<d} sum_i J[mu][i] s_i s_{i+e_mu}   (Eq. (1) with H = 0; R3: both bonds counted at L=2) */
+static int32_t energy_of(const ref_ctx *c, const int8_t *J, const int8_t *s)
+{
+    int32_t e = 0;
+    for (int mu = 0; mu < c->d; ++mu)
+        for (int i = 0; i < c->N; ++i)
+            e -= J[mu * c->N + i] * s[i] * s[c->nbr[i * 2 * c->d + 2 * mu]];
+    return e;
+}
+
+static int8_t *spins_of(const ref_ctx *c, int s, int ch, int r)
+{
+    return c->spin + (((size_t)s * 2 + ch) * c->T + r) * c->N;
+}
+static size_t rep(const ref_ctx *c, int s, int ch, int r) { return ((size_t)s * 2 + ch) * c->T + r; }
+
+static void recompute_all(ref_ctx *c)
+{
+    for (int s = 0; s < c->S; ++s)
+        for (int ch = 0; ch < 2; ++ch)
+            for (int r = 0; r < c->T; ++r)
+                c->E[rep(c, s, ch, r)] = energy_of(c, c->J + (size_t)s * c->d * c->N, spins_of(c, s, ch, r));
+}
+
+/* ---------------------------------------------------------------- init (8(c).2) */
+
+ref_ctx *ref_create(int L, int d, int S, int T, const double *betas, uint64_t seed, uint32_t sample_offset)
+{
+    if (d != 2 && d != 3) return NULL;
+    if (L < 2 || (L & 1)) return NULL;
+    if (S < 1 || T < 1 || T > 65535 || betas == NULL) return NULL;
+    for (int t = 0; t < T; ++t)
+        if (!isfinite(betas[t]) || betas[t] < 0.0) return NULL;
+    double Nd = pow((double)L, d) * d;
+    if (Nd > 2147483647.0) return NULL;
+    if ((uint64_t)sample_offset + (uint64_t)S > 4294967296ull) return NULL;
+
+    ref_ctx *c = (ref_ctx *)calloc(1, sizeof(ref_ctx));
+    c->L = L; c->d = d; c->S = S; c->T = T; c->seed = seed; c->sample_offset = sample_offset;
+    c->N = (d == 2) ? L * L : L * L * L;
+    size_t R = (size_t)S * 2 * T, N = (size_t)c->N;
+    c->betas = (double *)malloc(sizeof(double) * T);
+    memcpy(c->betas, betas, sizeof(double) * T);
+    c->J = (int8_t *)malloc((size_t)S * d * N);
+    c->spin = (int8_t *)malloc(R * N);
+    c->E = (int32_t *)malloc(R * sizeof(int32_t));
+    c->temp_of_slot = (int32_t *)malloc(R * sizeof(int32_t));
+    c->slot_of_temp = (int32_t *)malloc(R * sizeof(int32_t));
+    c->thrM = (uint32_t *)malloc(sizeof(uint32_t) * T * d);
+    c->sgn = (int *)calloc((size_t)T, sizeof(int));
+    c->attempts = (uint64_t *)calloc((size_t)S * 2 * T, sizeof(uint64_t));
+    c->accepts = (uint64_t *)calloc((size_t)S * 2 * T, sizeof(uint64_t));
+    c->last_size = (uint32_t *)calloc((size_t)S * T, sizeof(uint32_t));
+    c->cum_size = (uint64_t *)calloc((size_t)S * T, sizeof(uint64_t));
+    c->nbr = (int *)malloc(sizeof(int) * N * 2 * d);
+    c->queue = (int *)malloc(sizeof(int) * N);
+    c->mark = (uint8_t *)malloc(N);
+    build_neighbours(c);
+
+    for (int s = 0; s < S; ++s) {
+        uint32_t g = sample_offset + (uint32_t)s;
+        /* 1. couplings: domain 1, p = 1/2 exactly (Eq. (2)) */
+        for (int mu = 0; mu < d; ++mu)
+            for (int i = 0; i < c->N; ++i)
+                c->J[((size_t)s * d + mu) * N + i] = sign_of(draw(c, (uint32_t)i >> 2, 0, g, 1, mu, 0, 0, i & 3));
+        /* 2. spins: domain 2 (R17);  3. identity permutations */
+        for (int ch = 0; ch < 2; ++ch)
+            for (int r = 0; r < T; ++r) {
+                int8_t *sp = spins_of(c, s, ch, r);
+                for (int i = 0; i < c->N; ++i)
+                    sp[i] = sign_of(draw(c, (uint32_t)i >> 2, 0, g, 2, 0, ch, r, i & 3));
+                c->temp_of_slot[rep(c, s, ch, r)] = r;
+                c->slot_of_temp[rep(c, s, ch, r)] = r;
+            }
+    }
+    /* 4. energies */
+    recompute_all(c);
+    /* 5. Metropolis thresholds thrM[t][k] = THR(-(beta_t * 4k)), k = 1..d */
+    for (int t = 0; t < T; ++t)
+        for (int k = 1; k <= d; ++k)
+            c->thrM[t * d + (k - 1)] = ref_threshold(-(betas[t] * (double)(4 * k)));
+    /* 6. swap sign sgn[t] = sign(beta_{t+1} - beta_t); thrX evaluated on demand */
+    for (int t = 0; t + 1 < T; ++t)
+        c->sgn[t] = (betas[t + 1] > betas[t]) - (betas[t + 1] < betas[t]);
+    return c;
+}
+
+void ref_destroy(ref_ctx *c)
+{
+    if (!c) return;
+    free(c->betas); free(c->J); free(c->spin); free(c->E); free(c->temp_of_slot); free(c->slot_of_temp);
+    free(c->thrM); free(c->sgn); free(c->attempts); free(c->accepts); free(c->last_size); free(c->cum_size);
+    free(c->nbr); free(c->queue); free(c->mark);
+    free(c);
+}
+
+/* ---------------------------------------------------------------- Metropolis sweep (8(c).3, R1, R2, R4) */
+
+int ref_sweep(ref_ctx *c, int n)
+{
+    if (!c || n < 0) return -1;
+    if ((uint64_t)c->n_sweep + (uint64_t)n > 4294967295ull) return -3;
+    int d = c->d, N = c->N;
+    for (int it = 0; it < n; ++it) {
+        for (int p = 0; p < 2; ++p)                       /* black (x+y+z even) first, then white */
+            for (int s = 0; s < c->S; ++s) {
+                uint32_t g = c->sample_offset + (uint32_t)s;
+                const int8_t *J = c->J + (size_t)s * d * N;
+                for (int ch = 0; ch < 2; ++ch)
+                    for (int r = 0; r < c->T; ++r) {
+                        int8_t *sp = spins_of(c, s, ch, r);
+                        int t = c->temp_of_slot[rep(c, s, ch, r)];
+                        for (int i = 0; i < N; ++i) {
+                            if (colour_of(c, i) != p) continue;
+                            int h = 0;
+                            for (int mu = 0; mu < d; ++mu) {
+                                int up = c->nbr[i * 2 * d + 2 * mu], dn = c->nbr[i * 2 * d + 2 * mu + 1];
+                                h += J[mu * N + i] * sp[up] + J[mu * N + dn] * sp[dn];
+                            }
+                            int a = sp[i] * h;            /* Delta E = 2a */
+                            uint32_t u = draw(c, (uint32_t)i >> 3, c->n_sweep, g, 3, p, ch, r, (i >> 1) & 3);
+                            if (a <= 0 || u < c->thrM[t * d + (a / 2 - 1)]) {
+                                sp[i] = (int8_t)-sp[i];
+                                c->E[rep(c, s, ch, r)] += 2 * a;
+                            }
+                        }
+                    }
+            }
+        c->n_sweep += 1;
+    }
+    return 0;
+}
+
+/* ---------------------------------------------------------------- PT pass (8(c).4; Eq. (5), R9, R10) */
+
+int ref_exchange(ref_ctx *c)
+{
+    if (!c) return -1;
+    if (c->n_exchange == 4294967295u) return -3;
+    int T = c->T;
+    for (int s = 0; s < c->S; ++s) {
+        uint32_t g = c->sample_offset + (uint32_t)s;
+        for (int ch = 0; ch < 2; ++ch) {
+            int32_t *sot = c->slot_of_temp + rep(c, s, ch, 0);
+            int32_t *tos = c->temp_of_slot + rep(c, s, ch, 0);
+            int32_t *E = c->E + rep(c, s, ch, 0);
+            for (int t = 0; t + 1 < T; ++t) {
+                int ra = sot[t], rb = sot[t + 1];
+                long dE = (long)E[ra] - (long)E[rb];      /* multiple of 4 (R22b) */
+                if (dE % 4 != 0) abort();
+                uint32_t u = draw(c, (uint32_t)t, c->n_exchange, g, 4, 0, ch, 0, 0);
+                size_t k = ((size_t)s * 2 + ch) * (T - 1) + t;
+                c->attempts[k] += 1;
+                if (c->sgn[t] * dE <= 0 || u < thrX_of(c, t, labs(dE) / 4)) {
+                    sot[t] = rb; sot[t + 1] = ra; tos[ra] = t + 1; tos[rb] = t;
+                    c->accepts[k] += 1;
+                }
+            }
+        }
+    }
+    c->n_exchange += 1;
+    return 0;
+}
+
+/* ---------------------------------------------------------------- Houdayer cluster exchange (8(c).5; Eq. (10), R12, R13) */
+
+int ref_houdayer(ref_ctx *c)
+{
+    if (!c) return -1;
+    if (c->n_houdayer == 4294967295u) return -3;
+    int d = c->d, N = c->N, T = c->T;
+    for (int s = 0; s < c->S; ++s) {
+        uint32_t g = c->sample_offset + (uint32_t)s;
+        const int8_t *J = c->J + (size_t)s * d * N;
+        for (int t = 0; t < T; ++t) {
+            int ra = c->slot_of_temp[rep(c, s, 0, t)], rb = c->slot_of_temp[rep(c, s, 1, t)];
+            int8_t *A = spins_of(c, s, 0, ra), *B = spins_of(c, s, 1, rb);
+            int n_neg = 0;
+            for (int i = 0; i < N; ++i) n_neg += (A[i] * B[i] == -1);
+            uint32_t u = draw(c, 0, c->n_houdayer, g, 5, 0, 0, t, 0);
+            if (n_neg == 0) { c->last_size[(size_t)s * T + t] = 0; continue; }
+            int k = (int)(((uint64_t)u * (uint64_t)n_neg) >> 32), i0 = -1;
+            for (int i = 0, seen = 0; i < N; ++i)
+                if (A[i] * B[i] == -1) { if (seen == k) { i0 = i; break; } ++seen; }
+            /* breadth-first search over q = -1 sites */
+            memset(c->mark, 0, (size_t)N);
+            int head = 0, tail = 0;
+            c->queue[tail++] = i0; c->mark[i0] = 1;
+            while (head < tail) {
+                int i = c->queue[head++];
+                for (int k2 = 0; k2 < 2 * d; ++k2) {
+                    int j = c->nbr[i * 2 * d + k2];
+                    if (!c->mark[j] && A[j] * B[j] == -1) { c->mark[j] = 1; c->queue[tail++] = j; }
+                }
+            }
+            /* delta = 2 * sum over boundary bonds (i in cluster, j not) of J_ij A_i A_j, old spins */
+            int32_t delta = 0;
+            for (int i = 0; i < N; ++i) {
+                if (!c->mark[i]) continue;
+                for (int mu = 0; mu < d; ++mu) {
+                    int up = c->nbr[i * 2 * d + 2 * mu], dn = c->nbr[i * 2 * d + 2 * mu + 1];
+                    if (!c->mark[up]) delta += 2 * J[mu * N + i] * A[i] * A[up];
+                    if (!c->mark[dn]) delta += 2 * J[mu * N + dn] * A[i] * A[dn];
+                }
+            }
+            for (int i = 0; i < N; ++i)
+                if (c->mark[i]) { A[i] = (int8_t)-A[i]; B[i] = (int8_t)-B[i]; }
+            c->E[rep(c, s, 0, ra)] += delta;
+            c->E[rep(c, s, 1, rb)] -= delta;
+            c->last_size[(size_t)s * T + t] = (uint32_t)tail;
+            c->cum_size[(size_t)s * T + t] += (uint64_t)tail;
+        }
+    }
+    c->n_houdayer += 1;
+    return 0;
+}
+
+/* ---------------------------------------------------------------- MCS in the paper's order (8(c).7, R15) */
+
+int ref_mcs(ref_ctx *c, int n_mcs, int n_metro, int do_houdayer, int do_exchange)
+{
+    if (!c || n_mcs < 0 || n_metro < 0) return -1;
+    for (int m = 0; m < n_mcs; ++m) {
+        int rc = ref_sweep(c, n_metro);
+        if (rc) return rc;
+        if (do_houdayer && (rc = ref_houdayer(c))) return rc;
+        if (do_exchange && (rc = ref_exchange(c))) return rc;
+    }
+    return 0;
+}
+
+/* ---------------------------------------------------------------- observables (8(c).6) */
+
+int ref_get_energy(const ref_ctx *c, int32_t *E)
+{
+    if (!c || !E) return -1;
+    for (int s = 0; s < c->S; ++s)
+        for (int ch = 0; ch < 2; ++ch)
+            for (int t = 0; t < c->T; ++t)
+                E[rep(c, s, ch, t)] = c->E[rep(c, s, ch, c->slot_of_temp[rep(c, s, ch, t)])];
+    return 0;
+}
+
+/* Q = sum_i q_i (Eq. (4) x N);  QL = sum_{mu,i} q_i q_{i+e_mu} (R14) */
+int ref_measure_overlap(const ref_ctx *c, int32_t *Q, int32_t *QL)
+{
+    if (!c || !Q) return -1;
+    for (int s = 0; s < c->S; ++s)
+        for (int t = 0; t < c->T; ++t) {
+            const int8_t *A = spins_of(c, s, 0, c->slot_of_temp[rep(c, s, 0, t)]);
+            const int8_t *B = spins_of(c, s, 1, c->slot_of_temp[rep(c, s, 1, t)]);
+            int32_t q = 0, ql = 0;
+            for (int i = 0; i < c->N; ++i) {
+                q += A[i] * B[i];
+                for (int mu = 0; mu < c->d; ++mu) {
+                    int j = c->nbr[i * 2 * c->d + 2 * mu];
+                    ql += A[i] * B[i] * A[j] * B[j];
+                }
+            }
+            Q[(size_t)s * c->T + t] = q;
+            if (QL) QL[(size_t)s * c->T + t] = ql;
+        }
+    return 0;
+}
+
+int ref_get_swap_counts(const ref_ctx *c, uint64_t *attempts, uint64_t *accepts)
+{
+    if (!c) return -1;
+    size_t n = (size_t)c->S * 2 * (c->T - 1);
+    if (attempts) memcpy(attempts, c->attempts, n * sizeof(uint64_t));
+    if (accepts) memcpy(accepts, c->accepts, n * sizeof(uint64_t));
+    return 0;
+}
+
+int ref_get_cluster_sizes(const ref_ctx *c, uint32_t *last, uint64_t *cumulative)
+{
+    if (!c) return -1;
+    size_t n = (size_t)c->S * c->T;
+    if (last) memcpy(last, c->last_size, n * sizeof(uint32_t));
+    if (cumulative) memcpy(cumulative, c->cum_size, n * sizeof(uint64_t));
+    return 0;
+}
+
+int ref_get_perm(const ref_ctx *c, int32_t *temp_of_slot, int32_t *slot_of_temp)
+{
+    if (!c) return -1;
+    size_t n = (size_t)c->S * 2 * c->T;
+    if (temp_of_slot) memcpy(temp_of_slot, c->temp_of_slot, n * sizeof(int32_t));
+    if (slot_of_temp) memcpy(slot_of_temp, c->slot_of_temp, n * sizeof(int32_t));
+    return 0;
+}
+
+int ref_get_spins(const ref_ctx *c, int8_t *spins)
+{
+    if (!c || !spins) return -1;
+    memcpy(spins, c->spin, (size_t)c->S * 2 * c->T * c->N);
+    return 0;
+}
+
+int ref_get_couplings(const ref_ctx *c, int8_t *J)
+{
+    if (!c || !J) return -1;
+    memcpy(J, c->J, (size_t)c->S * c->d * c->N);
+    return 0;
+}
+
+int ref_get_thresholds(const ref_ctx *c, uint32_t *thrM, uint32_t *thrX, size_t stride)
+{
+    if (!c) return -1;
+    if (thrM) memcpy(thrM, c->thrM, sizeof(uint32_t) * c->T * c->d);
+    if (thrX)
+        for (int t = 0; t + 1 < c->T; ++t)
+            for (size_t m = 0; m < stride; ++m)
+                thrX[(size_t)t * stride + m] = thrX_of(c, t, (long)m);
+    return 0;
+}
+
+int ref_get_counters(const ref_ctx *c, uint32_t *n_sweep, uint32_t *n_exchange, uint32_t *n_houdayer)
+{
+    if (!c) return -1;
+    if (n_sweep) *n_sweep = c->n_sweep;
+    if (n_exchange) *n_exchange = c->n_exchange;
+    if (n_houdayer) *n_houdayer = c->n_houdayer;
+    return 0;
+}
+
+int ref_set_spins(ref_ctx *c, const int8_t *spins)
+{
+    if (!c || !spins) return -1;
+    size_t n = (size_t)c->S * 2 * c->T * c->N;
+    for (size_t k = 0; k < n; ++k)
+        if (spins[k] != 1 && spins[k] != -1) return -1;
+    memcpy(c->spin, spins, n);
+    recompute_all(c);
+    return 0;
+}
+
+int ref_set_couplings(ref_ctx *c, const int8_t *J)
+{
+    if (!c || !J) return -1;
+    size_t n = (size_t)c->S * c->d * c->N;
+    for (size_t k = 0; k < n; ++k)
+        if (J[k] != 1 && J[k] != -1) return -1;
+    memcpy(c->J, J, n);
+    recompute_all(c);
+    return 0;
+}
+
+int ref_recompute_energy(const ref_ctx *c, int32_t *E_slot_order, int *mismatch_count)
+{
+    if (!c) return -1;
+    int bad = 0;
+    for (int s = 0; s < c->S; ++s)
+        for (int ch = 0; ch < 2; ++ch)
+            for (int r = 0; r < c->T; ++r) {
+                int32_t e = energy_of(c, c->J + (size_t)s * c->d * c->N, spins_of(c, s, ch, r));
+                if (E_slot_order) E_slot_order[rep(c, s, ch, r)] = e;
+                bad += (e != c->E[rep(c, s, ch, r)]);
+            }
+    if (mismatch_count) *mismatch_count = bad;
+    return 0;
+}
