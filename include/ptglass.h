@@ -1,0 +1,143 @@
+/*
+ * ptglass.h -- C ABI of the B200-native parallel-tempering Monte Carlo library for Edwards-Anderson +-J Ising
+ * spin glasses: the data-parallel hot path of arXiv 2003.04621 (Kumar, Gross, Janke, Weigel).
+ *
+ * "P:n" cites line n of the paper text; "Rk" a reading listed in DESIGN.md section 3.
+ *
+ * MODEL (Eq. (1)-(2)): H = -sum_<ij> J_ij s_i s_j, s_i = +-1, J_ij = +-1 with p = 1/2, zero field,
+ * d-dimensional (d = 2 square, d = 3 simple cubic) periodic lattice of linear size L (even, R3), N = L^d sites,
+ * site index i = x + L*y (+ L*L*z), colour p(i) = (x+y+z)&1, bond (mu,i) joins i and i+e_mu.
+ * ENSEMBLE: S disorder samples x T temperatures x C = 2 replica chains.  A "slot" r in [0,T) is a
+ * fixed spin configuration of chain c of sample s; its current temperature index is temp_of_slot[s][c][r], the
+ * inverse map is slot_of_temp[s][c][t] (the "two arrays" of P:169).
+ * RANDOM NUMBERS (R11): Philox4x32-10, key = seed, counter = (index, step, global sample, tag); every
+ * result is a pure function of (L, d, S, T, betas, seed, sample_offset, sequence of calls), independent of how
+ * the work is mapped to threads, CTAs or GPUs.
+ *
+ * CONVENTIONS
+ *  - Every call returns 0 (PT_OK) or a negative PT_ERR_* code; nothing throws or aborts.  pt_last_error()
+ *    returns a static NUL-terminated message describing the last failing call.
+ *  - One process-global simulation context (the calls carry no handle).  Calling an update / observable before
+ *    pt_init or after pt_free returns PT_ERR_STATE.
+ *  - DEVICE MEMORY IS CALLER-OWNED: the caller (PyTorch) allocates one workspace of pt_workspace_bytes() bytes,
+ *    256-byte aligned, and passes its raw device pointer and a cudaStream_t to pt_bind(); the library never
+ *    allocates or frees device memory and launches everything on that stream.
+ *  - All `const T *` inputs are HOST pointers, caller-owned, copied during the call.  All output pointers are
+ *    HOST buffers, caller-allocated with the documented shape (C order), filled after a stream synchronise.
+ *    The *_device variants take DEVICE pointers instead and do not synchronise.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns PT_ERR_CUDA.
+ */
+#ifndef PTGLASS_H
+#define PTGLASS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PT_OK            0
+#define PT_ERR_ARG      -1   /* invalid argument (see each call) */
+#define PT_ERR_STATE    -2   /* not bound / not initialised / workspace too small */
+#define PT_ERR_OVERFLOW -3   /* a uint32 step counter would pass 2^32-1 (R21); state unchanged */
+#define PT_ERR_CUDA     -4   /* CUDA runtime failure; message carries cudaGetErrorString */
+
+/* ---- sizes & binding ------------------------------------------------------------------------------------ */
+
+/* Bytes of device workspace needed for a problem of this shape (includes an int8 staging area for the
+ * state get/set calls).  PT_ERR_ARG for shapes pt_init would reject. */
+int pt_workspace_bytes(int L, int d, int n_samples, int n_temps, size_t *bytes_out);
+
+/* Bind the caller's device workspace (device pointer, >= pt_workspace_bytes, 256-byte aligned) and CUDA stream
+ * (a cudaStream_t passed as void*; NULL = default stream).  Must precede pt_init.  Re-binding frees the context. */
+int pt_bind(void *device_workspace, size_t bytes, void *cuda_stream);
+
+/* ---- life cycle ----------------------------------------------------------------------------------------- */
+
+/* Initialise: couplings J[s][mu][i] and spins from Philox (domains 1, 2), identity permutations,
+ * energies E = -sum J s s (Eq. (1)), zero counters; acceptance tables computed HERE ON THE HOST in double
+ * (R5, R6):  thrM[t][k] = THR(-(betas[t]*4k)), k = 1..d;  thrX[t][m] = THR(-(|betas[t+1]-betas[t]|*4m));
+ * THR(x) = min(2^32-1, floor(2^32 exp(x))).
+ * betas: HOST array [n_temps], any order, duplicates allowed (R7); index t = position in this array.
+ * PT_ERR_ARG: d not in {2,3}; L < 2 or odd (checkerboard needs a bipartite periodic lattice, R3); n_samples < 1;
+ * n_temps < 1 or > 65535; betas NULL, negative or non-finite; N*d > 2^31-1; sample_offset+n_samples > 2^32.
+ * PT_ERR_STATE: no workspace bound or workspace too small. */
+int pt_init(int L, int d, int n_samples, int n_temps, const double *betas, uint64_t seed);
+/* Same, for a shard holding global samples [sample_offset, sample_offset + n_samples) (multi-GPU). */
+int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas, uint64_t seed,
+                  uint32_t sample_offset);
+int pt_free(void);
+
+/* ---- updates -------------------------------------------------------------------------------- */
+
+/* n >= 0 checkerboard Metropolis sweeps of every replica (R1, R2, R4): for colour p = 0 then 1, for
+ * every site i of colour p: a = s_i * sum_{2d nbrs} J s_j; flip iff a <= 0 or u < thrM[temp][a/2], u = the
+ * site's Philox word (domain 3: index i>>3, step = sweep number, tag (p, chain, slot), word (i>>1)&3).
+ * E[slot] is updated by 2a per accepted flip.  Asynchronous on the bound stream. */
+int pt_sweep(int n);
+
+/* One parallel-tempering pass (Eq. (5); R9, R10): for every (sample, chain), for t = 0..T-2 in
+ * order, each step seeing the previous: dE = E[slot_of_temp[t]] - E[slot_of_temp[t+1]]; accept iff
+ * sgn(beta[t+1]-beta[t])*dE <= 0 or u < thrX[t][|dE|/4]; on accept swap the entries of both maps.  Spins and
+ * E[slot] are untouched (only temperatures are exchanged). */
+int pt_exchange(void);
+
+/* One Houdayer cluster exchange per (sample, temperature) (Eq. (10); R12, R13): the two slots at
+ * temperature t (one per chain); q_i = s1_i s2_i; the k-th q = -1 site in index order, k = (u*n_neg)>>32; its
+ * connected component among q = -1 sites is negated in both configurations; E1 += delta, E2 -= delta. */
+int houdayer_step(void);
+
+/* Fused Monte Carlo steps in the paper's order (R15): n_mcs x [ pt_sweep(n_metro);
+ * houdayer_step() if do_houdayer; pt_exchange() if do_exchange ].  Bit-identical to the separate calls. */
+int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange);
+
+/* ---- observables: all integer, indexed by TEMPERATURE index t ------------------------------------------- */
+
+int pt_get_energy(int32_t *E /* [S][2][T]: E of the configuration currently at temperature t (Eq. (3) x N) */);
+/* Q = sum_i s1_i s2_i (Eq. (4) x N), QL = sum_{mu,i} q_i q_{i+e_mu} (R14); [S][T] each; QL may be NULL.
+ * Consumes no random numbers and advances no counter (R26). */
+int pt_measure_overlap(int32_t *Q, int32_t *QL);
+int pt_get_swap_counts(uint64_t *attempts, uint64_t *accepts /* [S][2][T-1] since init; either may be NULL */);
+int pt_get_cluster_sizes(uint32_t *last, uint64_t *cumulative /* [S][T]; either may be NULL */);
+int pt_get_perm(int32_t *temp_of_slot, int32_t *slot_of_temp /* [S][2][T] each; either may be NULL */);
+
+/* Device-resident variants (DEVICE pointers, same shapes, no host synchronisation): for callers that keep
+ * observables on the GPU. */
+int pt_get_energy_device(int32_t *E_dev);
+int pt_measure_overlap_device(int32_t *Q_dev, int32_t *QL_dev);
+
+/* ---- state access in SLOT order (parity tests, checkpointing) ------------------------------------------- */
+
+int pt_get_spins(int8_t *spins /* [S][2][T(slot)][N], +1/-1 */);
+int pt_get_couplings(int8_t *J /* [S][d][N], J[mu][i] = bond i -> i+e_mu, +1/-1 */);
+int pt_get_thresholds(uint32_t *thrM /* [T][d], k=1..d at [t][k-1]; may be NULL */,
+                      uint32_t *thrX /* [T-1][thrX_stride], entry m = |dE|/4; may be NULL */, size_t thrX_stride);
+int pt_get_counters(uint32_t *n_sweep, uint32_t *n_exchange, uint32_t *n_houdayer);
+int pt_set_spins(const int8_t *spins);      /* values must be +1/-1 (PT_ERR_ARG otherwise); recomputes E */
+int pt_set_couplings(const int8_t *J);      /* values must be +1/-1; recomputes E */
+/* Recompute every E from scratch and count slots whose tracked E differs (invariant check; must be 0). */
+int pt_recompute_energy(int32_t *E_slot_order /* [S][2][T] or NULL */, int *mismatch_count /* or NULL */);
+
+/* ---- diagnostics ---------------------------------------------------------------------------------------- */
+
+int pt_synchronize(void);                          /* cudaStreamSynchronize on the bound stream */
+int pt_get_launch_count(uint64_t *n_launches);     /* kernels launched by this library since pt_bind */
+/* Which code path the bound problem uses: 1 = word-parallel kernels specialised for L a power of two >= 8,
+ * 0 = general-L kernels.  force = -1 leaves the choice to the library, 0 forces the general path (tests). */
+int pt_get_path(int *fast);
+int pt_force_general_path(int force);
+/* Philox4x32-10 evaluated by the device code for n counters (HOST arrays ctr[n][4], out[n][4]); test hook. */
+int pt_philox_selftest(const uint32_t key[2], const uint32_t *ctr, uint32_t *out, int n);
+/* INT32 issue-rate microbenchmark, the roofline denominator of the sweep kernel:
+ * kind 0 = IMAD.WIDE.U32, 1 = LOP3, 2 = IADD3 carry pair, 3 = IMAD.WIDE+LOP3 mix, 4 = whole Philox4x32-10 blocks
+ * (40 ops each).  Launches 256-thread CTAs, ctas_per_sm per SM, on cuda_stream; device_scratch: >= 4 bytes of
+ * DEVICE memory.  Returns sustained thread-operations per ns (best of 3 after a warm-up) and the kernel time. */
+int pt_microbench(int kind, int ctas_per_sm, int iters, void *device_scratch, void *cuda_stream,
+                  double *thread_ops_per_ns, double *ms_out);
+const char *pt_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

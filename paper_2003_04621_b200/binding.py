@@ -1,0 +1,301 @@
+"""Thin Python binding of the C ABI in include/ptglass.h: same names, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libptglass.so.  PyTorch is used for exactly two things: the
+device workspace (one uint8 tensor) and the CUDA stream.  There is no CPU fallback: if the shared library is
+missing this module raises at import of the first call, and on a box without a CUDA device every compute call
+fails with PT_ERR_CUDA.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libptglass.so")
+
+PT_OK, PT_ERR_ARG, PT_ERR_STATE, PT_ERR_OVERFLOW, PT_ERR_CUDA = 0, -1, -2, -3, -4
+
+# every symbol include/ptglass.h declares: name -> (restype, argtypes)
+_vp, _i, _sz = C.c_void_p, C.c_int, C.c_size_t
+SYMBOLS = {
+    "pt_workspace_bytes": (_i, [_i, _i, _i, _i, C.POINTER(_sz)]),
+    "pt_bind": (_i, [_vp, _sz, _vp]),
+    "pt_init": (_i, [_i, _i, _i, _i, _vp, C.c_uint64]),
+    "pt_init_shard": (_i, [_i, _i, _i, _i, _vp, C.c_uint64, C.c_uint32]),
+    "pt_free": (_i, []),
+    "pt_sweep": (_i, [_i]),
+    "pt_exchange": (_i, []),
+    "houdayer_step": (_i, []),
+    "pt_mcs": (_i, [_i, _i, _i, _i]),
+    "pt_get_energy": (_i, [_vp]),
+    "pt_measure_overlap": (_i, [_vp, _vp]),
+    "pt_get_swap_counts": (_i, [_vp, _vp]),
+    "pt_get_cluster_sizes": (_i, [_vp, _vp]),
+    "pt_get_perm": (_i, [_vp, _vp]),
+    "pt_get_energy_device": (_i, [_vp]),
+    "pt_measure_overlap_device": (_i, [_vp, _vp]),
+    "pt_get_spins": (_i, [_vp]),
+    "pt_get_couplings": (_i, [_vp]),
+    "pt_get_thresholds": (_i, [_vp, _vp, _sz]),
+    "pt_get_counters": (_i, [_vp, _vp, _vp]),
+    "pt_set_spins": (_i, [_vp]),
+    "pt_set_couplings": (_i, [_vp]),
+    "pt_recompute_energy": (_i, [_vp, _vp]),
+    "pt_synchronize": (_i, []),
+    "pt_get_launch_count": (_i, [_vp]),
+    "pt_get_path": (_i, [_vp]),
+    "pt_force_general_path": (_i, [_i]),
+    "pt_philox_selftest": (_i, [_vp, _vp, _vp, _i]),
+    "pt_microbench": (_i, [_i, _i, _i, _vp, _vp, _vp, _vp]),
+    "pt_last_error": (C.c_char_p, []),
+}
+
+_lib = None
+
+
+class PTError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("ptglass error %d: %s" % (code, msg))
+        self.code = code
+
+
+def lib():
+    """Load libptglass.so (built in-tree by paper_2003_04621_b200.build).  Fails loudly if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("%s not found: run `python -m paper_2003_04621_b200.build` (nvcc, sm_100a) first; "
+                              "there is no CPU fallback" % LIB_PATH)
+        L = C.CDLL(LIB_PATH)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _ck(rc):
+    if rc != PT_OK:
+        raise PTError(rc, lib().pt_last_error().decode())
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data
+
+
+# shape of the bound problem, kept only to size the numpy output buffers
+_shape = dict(L=0, d=0, S=0, T=0, N=0)
+_workspace = None     # keeps the torch tensor alive while bound
+
+
+def pt_last_error() -> str:
+    return lib().pt_last_error().decode()
+
+
+def pt_workspace_bytes(L, d, n_samples, n_temps) -> int:
+    out = _sz()
+    _ck(lib().pt_workspace_bytes(L, d, n_samples, n_temps, C.byref(out)))
+    return out.value
+
+
+def pt_bind(workspace, stream=None):
+    """workspace: a CUDA uint8 torch tensor; stream: torch.cuda.Stream or None (current stream)."""
+    global _workspace
+    import torch
+
+    assert workspace.is_cuda and workspace.dtype == torch.uint8 and workspace.is_contiguous()
+    s = torch.cuda.current_stream(workspace.device) if stream is None else stream
+    _ck(lib().pt_bind(workspace.data_ptr(), workspace.numel(), s.cuda_stream))
+    _workspace = (workspace, s)
+
+
+def pt_init(L, d, n_samples, n_temps, betas, seed, sample_offset=None):
+    b = np.ascontiguousarray(betas, dtype=np.float64)
+    if b.shape != (n_temps,):
+        raise PTError(PT_ERR_ARG, "betas must have shape (n_temps,)")
+    if sample_offset is None:
+        _ck(lib().pt_init(L, d, n_samples, n_temps, _p(b), seed))
+    else:
+        _ck(lib().pt_init_shard(L, d, n_samples, n_temps, _p(b), seed, sample_offset))
+    _shape.update(L=L, d=d, S=n_samples, T=n_temps, N=L ** d)
+
+
+def pt_init_shard(L, d, n_samples, n_temps, betas, seed, sample_offset):
+    pt_init(L, d, n_samples, n_temps, betas, seed, sample_offset)
+
+
+def pt_free():
+    global _workspace
+    _ck(lib().pt_free())
+    _workspace = None
+
+
+def pt_open(L, d, n_samples, n_temps, betas, seed, sample_offset=0, device="cuda:0", stream=None, general=False):
+    """Convenience: allocate the workspace with torch, bind it and initialise.  Returns the workspace tensor."""
+    import torch
+
+    ws = torch.empty(pt_workspace_bytes(L, d, n_samples, n_temps), dtype=torch.uint8, device=device)
+    with torch.cuda.device(ws.device):
+        pt_bind(ws, stream)
+        if general:
+            pt_force_general_path(0)
+        pt_init(L, d, n_samples, n_temps, betas, seed, sample_offset)
+    return ws
+
+
+def pt_sweep(n=1):
+    _ck(lib().pt_sweep(n))
+
+
+def pt_exchange():
+    _ck(lib().pt_exchange())
+
+
+def houdayer_step():
+    _ck(lib().houdayer_step())
+
+
+def pt_mcs(n_mcs, n_metro=1, do_houdayer=False, do_exchange=True):
+    _ck(lib().pt_mcs(n_mcs, n_metro, int(do_houdayer), int(do_exchange)))
+
+
+def pt_get_energy(out=None):
+    E = np.empty((_shape["S"], 2, _shape["T"]), dtype=np.int32) if out is None else out
+    _ck(lib().pt_get_energy(_p(E)))
+    return E
+
+
+def pt_measure_overlap(link=True):
+    Q = np.empty((_shape["S"], _shape["T"]), dtype=np.int32)
+    QL = np.empty((_shape["S"], _shape["T"]), dtype=np.int32) if link else None
+    _ck(lib().pt_measure_overlap(_p(Q), _p(QL)))
+    return Q, QL
+
+
+def pt_get_energy_device(E_dev):
+    _ck(lib().pt_get_energy_device(E_dev.data_ptr()))
+
+
+def pt_measure_overlap_device(Q_dev, QL_dev=None):
+    _ck(lib().pt_measure_overlap_device(Q_dev.data_ptr(), None if QL_dev is None else QL_dev.data_ptr()))
+
+
+def pt_get_swap_counts():
+    a = np.zeros((_shape["S"], 2, max(_shape["T"] - 1, 0)), dtype=np.uint64)
+    b = np.zeros_like(a)
+    _ck(lib().pt_get_swap_counts(_p(a), _p(b)))
+    return a, b
+
+
+def pt_get_cluster_sizes():
+    last = np.empty((_shape["S"], _shape["T"]), dtype=np.uint32)
+    cum = np.empty((_shape["S"], _shape["T"]), dtype=np.uint64)
+    _ck(lib().pt_get_cluster_sizes(_p(last), _p(cum)))
+    return last, cum
+
+
+def pt_get_perm():
+    tos = np.empty((_shape["S"], 2, _shape["T"]), dtype=np.int32)
+    sot = np.empty((_shape["S"], 2, _shape["T"]), dtype=np.int32)
+    _ck(lib().pt_get_perm(_p(tos), _p(sot)))
+    return tos, sot
+
+
+def pt_get_spins(out=None):
+    s = np.empty((_shape["S"], 2, _shape["T"], _shape["N"]), dtype=np.int8) if out is None else out
+    _ck(lib().pt_get_spins(_p(s)))
+    return s
+
+
+def pt_get_couplings():
+    J = np.empty((_shape["S"], _shape["d"], _shape["N"]), dtype=np.int8)
+    _ck(lib().pt_get_couplings(_p(J)))
+    return J
+
+
+def pt_get_thresholds(thrX_stride):
+    thrM = np.zeros((_shape["T"], _shape["d"]), dtype=np.uint32)
+    thrX = np.zeros((max(_shape["T"] - 1, 0), thrX_stride), dtype=np.uint32)
+    _ck(lib().pt_get_thresholds(_p(thrM), _p(thrX), thrX_stride))
+    return thrM, thrX
+
+
+def pt_get_counters():
+    a, b, c = C.c_uint32(), C.c_uint32(), C.c_uint32()
+    _ck(lib().pt_get_counters(C.byref(a), C.byref(b), C.byref(c)))
+    return a.value, b.value, c.value
+
+
+def pt_set_spins(spins):
+    s = np.ascontiguousarray(spins, dtype=np.int8)
+    if s.shape != (_shape["S"], 2, _shape["T"], _shape["N"]):
+        raise PTError(PT_ERR_ARG, "spins must have shape [S][2][T][N]")
+    _ck(lib().pt_set_spins(_p(s)))
+
+
+def pt_set_couplings(J):
+    j = np.ascontiguousarray(J, dtype=np.int8)
+    if j.shape != (_shape["S"], _shape["d"], _shape["N"]):
+        raise PTError(PT_ERR_ARG, "J must have shape [S][d][N]")
+    _ck(lib().pt_set_couplings(_p(j)))
+
+
+def pt_recompute_energy():
+    E = np.empty((_shape["S"], 2, _shape["T"]), dtype=np.int32)
+    bad = C.c_int()
+    _ck(lib().pt_recompute_energy(_p(E), C.byref(bad)))
+    return E, bad.value
+
+
+def pt_synchronize():
+    _ck(lib().pt_synchronize())
+
+
+def pt_get_launch_count() -> int:
+    n = C.c_uint64()
+    _ck(lib().pt_get_launch_count(C.byref(n)))
+    return n.value
+
+
+def pt_get_path() -> int:
+    f = C.c_int()
+    _ck(lib().pt_get_path(C.byref(f)))
+    return f.value
+
+
+def pt_force_general_path(force):
+    _ck(lib().pt_force_general_path(force))
+
+
+def pt_philox_selftest(key, ctr):
+    k = np.ascontiguousarray(key, dtype=np.uint32)
+    c = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+    out = np.empty_like(c)
+    _ck(lib().pt_philox_selftest(_p(k), _p(c), _p(out), c.shape[0]))
+    return out
+
+
+def pt_microbench(kind, ctas_per_sm=8, iters=2000, device="cuda:0"):
+    """Returns (thread-ops per ns, kernel ms) of INT32 microbenchmark `kind` (see ptglass.h)."""
+    import torch
+
+    scratch = torch.zeros(64, dtype=torch.uint8, device=device)
+    ops, ms = C.c_double(), C.c_double()
+    with torch.cuda.device(scratch.device):
+        st = torch.cuda.current_stream().cuda_stream
+        rc = lib().pt_microbench(kind, ctas_per_sm, iters, scratch.data_ptr(), st, C.byref(ops), C.byref(ms))
+    if rc != PT_OK:
+        raise PTError(rc, "pt_microbench failed")
+    return ops.value, ms.value
+
+
+def state():
+    """Everything the parity tests compare (same keys as oracle.ref.Oracle.state)."""
+    tos, sot = pt_get_perm()
+    att, acc = pt_get_swap_counts()
+    last, cum = pt_get_cluster_sizes()
+    return dict(spins=pt_get_spins(), energy=pt_get_energy(), temp_of_slot=tos, slot_of_temp=sot,
+                attempts=att, accepts=acc, last_size=last, cum_size=cum,
+                counters=np.array(pt_get_counters(), dtype=np.uint32))

@@ -1,0 +1,594 @@
+// CUDA kernels of the hot path.  sm_100a; integer only; no tensor cores (nothing here is
+// a dense contraction).  Every kernel is written once over the lattice interface of lattice.cuh and
+// instantiated for FastLat<D, LOG2L> (word-parallel) and GenLat<D> (general L).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "lattice.cuh"
+#include "philox.cuh"
+
+namespace ptg {
+
+// Device arrays, all carved from the caller's workspace (ptglass.cu: carve()).
+struct DevPtrs {
+    uint32_t *spin;             // [S][2][T][2][W]   slot order; colour; word.  bit = 1 <=> s = -1
+    uint32_t *Jn;               // [S][2][2D][W]     colour; direction k; word. bit = 1 <=> J = -1
+    int32_t *E;                 // [S][2][T]         slot order
+    int32_t *tos;               // temp_of_slot [S][2][T]
+    int32_t *sot;               // slot_of_temp [S][2][T]
+    uint32_t *thrM;             // [T][4]            k = 1..D at [t][k-1]
+    uint32_t *thrX;             // [T-1][strideX]    entry m = |dE|/4; entries >= strideX are 0
+    int32_t *sgn;               // [T-1]
+    unsigned long long *accepts;// [S][2][T-1]
+    uint32_t *last;             // [S][T]
+    unsigned long long *cum;    // [S][T]
+    int32_t *outE;              // [S][2][T] scratch for observables
+    int32_t *outQ, *outQL;      // [S][T]
+    int *mismatch;              // [1]
+    int8_t *stage;              // int8 staging for get/set: max(S*2*T*N, S*D*N) bytes
+};
+
+struct Params {
+    int L, D, S, T, N, NH, W;
+    uint32_t g0;                // sample_offset: global sample index = g0 + s
+    uint32_t strideX;
+    RoundKeys rk;
+    DevPtrs d;
+};
+
+__device__ __forceinline__ size_t rep_index(const Params &P, int s, int c, int r) { return ((size_t)s * 2 + c) * P.T + r; }
+__device__ __forceinline__ uint32_t *spin_words(const Params &P, size_t rep, int p) { return P.d.spin + (rep * 2 + p) * P.W; }
+__device__ __forceinline__ const uint32_t *J_words(const Params &P, int s, int p, int k)
+{
+    return P.d.Jn + (((size_t)s * 2 + p) * (2 * P.D) + k) * P.W;
+}
+
+__device__ __forceinline__ uint32_t maj3(uint32_t a, uint32_t b, uint32_t c) { return (a & b) | (c & (a | b)); }
+
+// =========================================================================================================
+// init / pack / unpack (general coordinate arithmetic; not on the timed path)
+// =========================================================================================================
+
+// couplings from Philox domain 1 into the int8 staging area [S][D][N]   (Eq. (2), p = 1/2 P:195)
+__global__ void k_draw_couplings(Params P)
+{
+    const int n4 = P.N / 4;
+    const long total = (long)P.S * P.D * n4;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        const int i4 = (int)(id % n4);
+        const int mu = (int)((id / n4) % P.D);
+        const int s = (int)(id / ((long)n4 * P.D));
+        uint32_t w[4];
+        philox4x32_10((uint32_t)i4, 0u, P.g0 + (uint32_t)s, make_tag(DOM_J, mu, 0, 0), P.rk, w[0], w[1], w[2], w[3]);
+        int8_t *dst = P.d.stage + ((size_t)s * P.D + mu) * P.N + 4 * (size_t)i4;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) dst[j] = (w[j] >> 31) ? -1 : 1;
+    }
+}
+
+// spins from Philox domain 2 into staging [S][2][T][N]   (R17)
+__global__ void k_draw_spins(Params P)
+{
+    const int n4 = P.N / 4;
+    const long total = (long)P.S * 2 * P.T * n4;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        const int i4 = (int)(id % n4);
+        const long rep = id / n4;
+        const int r = (int)(rep % P.T);
+        const int c = (int)((rep / P.T) & 1);
+        const int s = (int)(rep / (2L * P.T));
+        uint32_t w[4];
+        philox4x32_10((uint32_t)i4, 0u, P.g0 + (uint32_t)s, make_tag(DOM_SPIN, 0, c, r), P.rk, w[0], w[1], w[2], w[3]);
+        int8_t *dst = P.d.stage + (size_t)rep * P.N + 4 * (size_t)i4;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) dst[j] = (w[j] >> 31) ? -1 : 1;
+    }
+}
+
+// staging int8 J[S][D][N] -> per-colour, per-direction bit arrays (Jn must be zeroed first)
+__global__ void k_pack_couplings(Params P)
+{
+    const long total = (long)P.S * P.D * P.N;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        const int i = (int)(id % P.N);
+        const int mu = (int)((id / P.N) % P.D);
+        const int s = (int)(id / ((long)P.N * P.D));
+        if (P.d.stage[id] >= 0) continue;
+        const int pi = colour_of_site(i, P.L, P.D);
+        const int j = neighbour_site(i, 2 * mu, P.L, P.D);
+        const int hi = i >> 1, hj = j >> 1;
+        uint32_t *Ji = P.d.Jn + (((size_t)s * 2 + pi) * (2 * P.D) + 2 * mu) * P.W;            // +mu seen from i
+        uint32_t *Jj = P.d.Jn + (((size_t)s * 2 + (1 - pi)) * (2 * P.D) + 2 * mu + 1) * P.W;  // -mu seen from j
+        atomicOr(Ji + (hi >> 5), 1u << (hi & 31));
+        atomicOr(Jj + (hj >> 5), 1u << (hj & 31));
+    }
+}
+
+__global__ void k_unpack_couplings(Params P)
+{
+    const long total = (long)P.S * P.D * P.N;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        const int i = (int)(id % P.N);
+        const int mu = (int)((id / P.N) % P.D);
+        const int s = (int)(id / ((long)P.N * P.D));
+        const int pi = colour_of_site(i, P.L, P.D), hi = i >> 1;
+        const uint32_t *Ji = P.d.Jn + (((size_t)s * 2 + pi) * (2 * P.D) + 2 * mu) * P.W;
+        P.d.stage[id] = ((Ji[hi >> 5] >> (hi & 31)) & 1u) ? -1 : 1;
+    }
+}
+
+// staging int8 spins [S][2][T][N] -> bit words; one thread per (replica, colour, word)
+__global__ void k_pack_spins(Params P)
+{
+    const long total = (long)P.S * 2 * P.T * 2 * P.W;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        const int w = (int)(id % P.W);
+        const int p = (int)((id / P.W) & 1);
+        const long rep = id / (2L * P.W);
+        const int8_t *src = P.d.stage + (size_t)rep * P.N;
+        uint32_t word = 0;
+        for (int b = 0; b < 32; ++b) {
+            const int h = 32 * w + b;
+            if (h >= P.NH) break;
+            if (src[site_of(h, p, P.L, P.D)] < 0) word |= 1u << b;
+        }
+        P.d.spin[id] = word;
+    }
+}
+
+__global__ void k_unpack_spins(Params P)
+{
+    const long total = (long)P.S * 2 * P.T * P.N;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        const int i = (int)(id % P.N);
+        const long rep = id / P.N;
+        const int p = colour_of_site(i, P.L, P.D), h = i >> 1;
+        const uint32_t *sw = P.d.spin + ((size_t)rep * 2 + p) * P.W;
+        P.d.stage[id] = ((sw[h >> 5] >> (h & 31)) & 1u) ? -1 : 1;
+    }
+}
+
+__global__ void k_identity_perm(Params P)
+{
+    const long total = (long)P.S * 2 * P.T;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        P.d.tos[id] = (int32_t)(id % P.T);
+        P.d.sot[id] = (int32_t)(id % P.T);
+    }
+}
+
+__global__ void k_philox_selftest(RoundKeys rk, const uint32_t *ctr, uint32_t *out, int n)
+{
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= n) return;
+    uint32_t o0, o1, o2, o3;
+    philox4x32_10(ctr[4 * id], ctr[4 * id + 1], ctr[4 * id + 2], ctr[4 * id + 3], rk, o0, o1, o2, o3);
+    out[4 * id] = o0; out[4 * id + 1] = o1; out[4 * id + 2] = o2; out[4 * id + 3] = o3;
+}
+
+// =========================================================================================================
+// energy from scratch:  E = -sum J s s = 2 * #unsatisfied - D*N   (Eq. (1)).  Each bond has exactly one
+// black endpoint, so summing the 2D directions over black sites counts every bond once (also at L = 2, R3).
+// One warp per replica.  mode 0: write E;  mode 1: write outE (slot order) and count mismatches against E.
+// =========================================================================================================
+template <class LAT>
+__global__ void k_energy(LAT lat, Params P, int mode)
+{
+    const int warps_per_block = blockDim.x >> 5;
+    const long rep = (long)blockIdx.x * warps_per_block + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (rep >= (long)P.S * 2 * P.T) return;
+    const int s = (int)(rep / (2L * P.T));
+    const uint32_t *Sb = spin_words(P, (size_t)rep, 0), *Sw = spin_words(P, (size_t)rep, 1);
+    int unsat = 0;
+    for (int w = lane; w < lat.words(); w += 32) {
+        uint32_t nb[2 * LAT::D];
+        lat.gather(Sw, w, 0, nb);
+        const uint32_t sb = Sb[w], v = lat.valid(w);
+#pragma unroll
+        for (int k = 0; k < 2 * LAT::D; ++k) unsat += __popc((sb ^ nb[k] ^ J_words(P, s, 0, k)[w]) & v);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) unsat += __shfl_xor_sync(0xFFFFFFFFu, unsat, o);
+    if (lane == 0) {
+        const int32_t e = 2 * unsat - P.D * P.N;
+        if (mode == 0) {
+            P.d.E[rep] = e;
+        } else {
+            P.d.outE[rep] = e;
+            if (P.d.E[rep] != e) atomicAdd(P.d.mismatch, 1);
+        }
+    }
+}
+
+// E in temperature order: outE[s][c][t] = E[s][c][slot_of_temp[t]]
+__global__ void k_energy_by_temp(Params P, int32_t *out)
+{
+    const long total = (long)P.S * 2 * P.T;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        const long base = (id / P.T) * P.T;
+        out[id] = P.d.E[base + P.d.sot[id]];
+    }
+}
+
+// =========================================================================================================
+// a1-a3  Metropolis sweeps
+//
+// One CTA = R replicas of one sample, resident in shared memory together with the sample's coupling bits for
+// n_sweeps sweeps.  Work item = one 32-bit word = 32 same-colour sites of one replica:
+//   * local fields bit-sliced: unsat_k = s ^ nbr_k ^ Jneg_k (1 LOP3 per direction per 32 sites), then a
+//     carry-save adder tree gives the number n_u of unsatisfied bonds per site as bit planes;
+//     a = s_i h_i = 2D - 2 n_u, so "a <= 0" <=> n_u >= D and threshold class k = a/2 = D - n_u;
+//   * 8 Philox4x32-10 blocks = 32 words u_j; per site one unsigned compare per class, packed into words C_k;
+//   * flip = always | OR_k (class_k & C_k); s ^= flip; dE = 4 * sum_flipped (D - n_u) by popcounts.
+// =========================================================================================================
+template <int D>
+struct Classes {
+    uint32_t always;        // n_u >= D
+    uint32_t m[D];          // m[k-1]: n_u == D - k  (threshold thrM[t][k])
+    uint32_t b0, b1, b2;    // bit planes of n_u
+};
+
+template <int D>
+__device__ __forceinline__ Classes<D> classify(const uint32_t un[2 * D])
+{
+    Classes<D> c;
+    if constexpr (D == 2) {
+        const uint32_t s1 = un[0] ^ un[1] ^ un[2];
+        const uint32_t c1 = maj3(un[0], un[1], un[2]);
+        const uint32_t c2 = s1 & un[3];
+        c.b0 = s1 ^ un[3];
+        c.b1 = c1 ^ c2;
+        c.b2 = c1 & c2;
+        c.always = c1 | c2;                 // n_u >= 2
+        c.m[0] = c.b0 & ~c.always;          // n_u == 1 -> k = 1
+        c.m[1] = ~(c.b0 | c.always);        // n_u == 0 -> k = 2
+    } else {
+        const uint32_t sA = un[0] ^ un[1] ^ un[2], cA = maj3(un[0], un[1], un[2]);
+        const uint32_t sB = un[3] ^ un[4] ^ un[5], cB = maj3(un[3], un[4], un[5]);
+        const uint32_t c0 = sA & sB;
+        c.b0 = sA ^ sB;
+        c.b1 = cA ^ cB ^ c0;
+        c.b2 = maj3(cA, cB, c0);
+        c.always = c.b2 | (c.b1 & c.b0);    // n_u >= 3
+        c.m[0] = c.b1 & ~c.b0 & ~c.b2;      // n_u == 2 -> k = 1
+        c.m[1] = c.b0 & ~c.b1 & ~c.b2;      // n_u == 1 -> k = 2
+        c.m[2] = ~(c.b0 | c.b1 | c.b2);     // n_u == 0 -> k = 3
+    }
+    return c;
+}
+
+// Accept bits for the 32 sites of word w: bit j of C[k-1] = (u_j < thr[k-1]), u_j = word (j & 3) of Philox block
+// 8w + (j >> 2) of the Metropolis stream (domain 3).
+template <int D>
+__device__ __forceinline__ void accept_bits(uint32_t w, uint32_t step, uint32_t g, uint32_t tag, const RoundKeys &rk,
+                                            const uint32_t thr[D], uint32_t C[D])
+{
+#pragma unroll
+    for (int k = 0; k < D; ++k) C[k] = 0;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+        uint32_t u[4];
+        philox4x32_10(8u * w + (uint32_t)b, step, g, tag, rk, u[0], u[1], u[2], u[3]);
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int k = 0; k < D; ++k) C[k] |= (uint32_t)(u[j] < thr[k]) << (4 * b + j);
+    }
+}
+
+// One work item.  Returns the energy change of the replica caused by this word's flips.
+template <class LAT>
+__device__ __forceinline__ int update_word(const LAT &lat, uint32_t *Sown, const uint32_t *Soth, const uint32_t *Jp,
+                                           int W, int w, int p, const uint32_t thr[LAT::D], uint32_t step, uint32_t g,
+                                           uint32_t tag, const RoundKeys &rk)
+{
+    constexpr int D = LAT::D;
+    uint32_t nb[2 * D], un[2 * D];
+    lat.gather(Soth, w, p, nb);
+    const uint32_t s = Sown[w];
+#pragma unroll
+    for (int k = 0; k < 2 * D; ++k) un[k] = s ^ nb[k] ^ Jp[k * W + w];
+    const Classes<D> cl = classify<D>(un);
+    uint32_t C[D];
+    accept_bits<D>((uint32_t)w, step, g, tag, rk, thr, C);
+    uint32_t flip = cl.always;
+#pragma unroll
+    for (int k = 0; k < D; ++k) flip |= cl.m[k] & C[k];
+    flip &= lat.valid(w);
+    Sown[w] = s ^ flip;
+    // dE = sum_flipped 2a = 4 * sum_flipped (D - n_u)
+    return 4 * (D * __popc(flip) - __popc(flip & cl.b0) - 2 * __popc(flip & cl.b1) - 4 * __popc(flip & cl.b2));
+}
+
+// grid: (2T/R groups, S).  dynamic smem: [2][2D][W] couplings | [R][2][W] spins | [R][4] thresholds | [R] dE
+template <class LAT>
+__global__ void __launch_bounds__(256) k_sweep(LAT lat, Params P, int R, uint32_t step0, int n_sweeps)
+{
+    constexpr int D = LAT::D;
+    extern __shared__ uint32_t smem[];
+    const int W = lat.words();
+    uint32_t *sJ = smem;                       // [2][2D][W]
+    uint32_t *sS = sJ + 2 * 2 * D * W;         // [R][2][W]
+    uint32_t *sThr = sS + R * 2 * W;           // [R][4]
+    int *sdE = (int *)(sThr + R * 4);          // [R]
+    const int s = blockIdx.y;
+    const int q0 = blockIdx.x * R;             // first replica (q = c*T + r) of this CTA
+    const size_t rep0 = (size_t)s * 2 * P.T + q0;
+    const uint32_t g = P.g0 + (uint32_t)s;
+
+    for (int i = threadIdx.x; i < 2 * 2 * D * W; i += blockDim.x) sJ[i] = P.d.Jn[(size_t)s * 2 * 2 * D * W + i];
+    for (int i = threadIdx.x; i < R * 2 * W; i += blockDim.x) sS[i] = P.d.spin[rep0 * 2 * W + i];
+    for (int i = threadIdx.x; i < R; i += blockDim.x) {
+        const int t = P.d.tos[rep0 + i];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) sThr[4 * i + k] = P.d.thrM[4 * t + k];
+        sdE[i] = 0;
+    }
+    __syncthreads();
+
+    const int items = R * W;
+    for (int it = 0; it < n_sweeps; ++it) {
+        for (int p = 0; p < 2; ++p) {
+            for (int item = threadIdx.x; item < items; item += blockDim.x) {
+                const int qi = item / W, w = item - qi * W;
+                const int q = q0 + qi;
+                const int c = (q >= P.T) ? 1 : 0, r = q - c * P.T;
+                uint32_t thr[D];
+#pragma unroll
+                for (int k = 0; k < D; ++k) thr[k] = sThr[4 * qi + k];
+                const int dE = update_word(lat, sS + (qi * 2 + p) * W, sS + (qi * 2 + (1 - p)) * W, sJ + p * 2 * D * W,
+                                           W, w, p, thr, step0 + (uint32_t)it, g, make_tag(DOM_METRO, p, c, r), P.rk);
+                if (dE != 0) atomicAdd(sdE + qi, dE);
+            }
+            __syncthreads();
+        }
+    }
+    for (int i = threadIdx.x; i < R * 2 * W; i += blockDim.x) P.d.spin[rep0 * 2 * W + i] = sS[i];
+    for (int i = threadIdx.x; i < R; i += blockDim.x) P.d.E[rep0 + i] += sdE[i];
+}
+
+// =========================================================================================================
+// a4  parallel-tempering pass (Eq. (5)).  One warp per (sample, chain):
+// the lanes draw the T-1 Philox words in parallel, lane 0 walks the ladder sequentially on a temperature-ordered
+// copy of the energies in shared memory.  Only the two index arrays change.
+// =========================================================================================================
+__device__ __forceinline__ uint32_t thrX_lookup(const Params &P, int t, uint32_t m)
+{
+    return (m < P.strideX) ? __ldg(P.d.thrX + (size_t)t * P.strideX + m) : 0u;
+}
+
+// dynamic smem: per warp [T] energies by temperature + [T] slot_of_temp.  GLOBAL_SCRATCH (very long ladders):
+// the same walk on outE / slot_of_temp in global memory.
+template <bool GLOBAL_SCRATCH>
+__global__ void k_exchange(Params P, uint32_t step)
+{
+    extern __shared__ int32_t xsm[];
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+    const long chain = (long)blockIdx.x * wpb + wib;
+    if (chain >= (long)P.S * 2) return;
+    const int s = (int)(chain >> 1), c = (int)(chain & 1);
+    const uint32_t g = P.g0 + (uint32_t)s;
+    const int T = P.T;
+    const size_t base = (size_t)chain * T;
+    int32_t *Et = GLOBAL_SCRATCH ? P.d.outE + base : xsm + (size_t)wib * 2 * T;
+    int32_t *so = GLOBAL_SCRATCH ? P.d.sot + base : Et + T;
+    for (int t = lane; t < T; t += 32) {
+        const int r = P.d.sot[base + t];
+        if (!GLOBAL_SCRATCH) so[t] = r;
+        Et[t] = P.d.E[base + r];
+    }
+    __syncwarp();
+    int32_t ea = 0, ra = 0;
+    if (lane == 0) { ea = Et[0]; ra = so[0]; }
+    for (int tb = 0; tb < T - 1; tb += 32) {
+        const int tl = tb + lane;
+        uint32_t u_l = 0, o1, o2, o3;
+        if (tl < T - 1) philox4x32_10((uint32_t)tl, step, g, make_tag(DOM_SWAP, 0, c, 0), P.rk, u_l, o1, o2, o3);
+        const int nstep = min(32, T - 1 - tb);
+        for (int j = 0; j < nstep; ++j) {
+            const uint32_t u = __shfl_sync(0xFFFFFFFFu, u_l, j);
+            if (lane == 0) {
+                const int t = tb + j;
+                const int32_t eb = Et[t + 1], rb = so[t + 1];
+                const int32_t dE = ea - eb;
+                const int sg = P.d.sgn[t];
+                const uint32_t m = (uint32_t)(dE < 0 ? -dE : dE) >> 2;
+                const bool acc = ((long long)sg * dE <= 0) || (u < thrX_lookup(P, t, m));
+                if (acc) {
+                    Et[t] = eb; so[t] = rb;                 // position t is final; (ea, ra) moves up to t+1
+                    P.d.accepts[(size_t)chain * (T - 1) + t] += 1ull;
+                } else {
+                    Et[t] = ea; so[t] = ra;
+                    ea = eb; ra = rb;
+                }
+            }
+        }
+    }
+    if (lane == 0) { Et[T - 1] = ea; so[T - 1] = ra; }
+    __syncwarp();
+    for (int t = lane; t < T; t += 32) {
+        const int r = so[t];
+        P.d.sot[base + t] = r;
+        P.d.tos[base + r] = t;
+    }
+}
+
+// =========================================================================================================
+// a5  Houdayer cluster exchange (Eq. (10)).  One CTA per (sample, t).
+// The q = -1 cluster is grown on bit maps: C_p |= (OR of the neighbour bits of C_{1-p}) & Neg_p, alternating
+// colours until nothing changes -- the fixed point is exactly the connected component of the seed.
+// =========================================================================================================
+// dynamic smem: Neg[2][W] | Cl[2][W] | scan[blockDim/32 + 2]
+template <class LAT>
+__global__ void __launch_bounds__(128) k_houdayer(LAT lat, Params P, uint32_t step)
+{
+    constexpr int D = LAT::D;
+    extern __shared__ uint32_t hsm[];
+    const int W = lat.words();
+    uint32_t *Neg = hsm, *Cl = hsm + 2 * W;
+    int *scan = (int *)(Cl + 2 * W);           // [0..nwarps): warp totals; [nwarps]: seed word; [nwarps+1]: seed colour|bit
+    const int t = blockIdx.x, s = blockIdx.y;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nwarps = blockDim.x >> 5;
+    const size_t repA = rep_index(P, s, 0, P.d.sot[rep_index(P, s, 0, t)]);
+    const size_t repB = rep_index(P, s, 1, P.d.sot[rep_index(P, s, 1, t)]);
+    uint32_t *A[2] = {spin_words(P, repA, 0), spin_words(P, repA, 1)};
+    uint32_t *B[2] = {spin_words(P, repB, 0), spin_words(P, repB, 1)};
+
+    // q_i = -1 bits; per-thread chunk of consecutive words for the prefix count in site-index order
+    const int cpt = (W + blockDim.x - 1) / blockDim.x;
+    const int w_lo = min(W, tid * cpt), w_hi = min(W, w_lo + cpt);
+    int local = 0;
+    for (int w = w_lo; w < w_hi; ++w) {
+        const uint32_t v = lat.valid(w);
+        const uint32_t n0 = (A[0][w] ^ B[0][w]) & v, n1 = (A[1][w] ^ B[1][w]) & v;
+        Neg[w] = n0; Neg[W + w] = n1;
+        Cl[w] = 0; Cl[W + w] = 0;
+        local += __popc(n0) + __popc(n1);
+    }
+    int incl = local;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    if (lane == 31) scan[wid] = incl;
+    __syncthreads();
+    int warp_off = 0, n_neg = 0;
+    for (int i = 0; i < nwarps; ++i) {
+        if (i < wid) warp_off += scan[i];
+        n_neg += scan[i];
+    }
+    const int excl = warp_off + incl - local;
+    if (n_neg == 0) {
+        if (tid == 0) P.d.last[(size_t)s * P.T + t] = 0;
+        return;
+    }
+    uint32_t u, o1, o2, o3;
+    philox4x32_10(0u, step, P.g0 + (uint32_t)s, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
+    const int kth = (int)(((unsigned long long)u * (unsigned long long)n_neg) >> 32);
+    if (kth >= excl && kth < excl + local) {
+        // this thread's chunk holds the seed: walk words, then the 32 half-indices of the word in site order
+        int rem = kth - excl;
+        for (int w = w_lo; w < w_hi; ++w) {
+            const int cw = __popc(Neg[w]) + __popc(Neg[W + w]);
+            if (rem >= cw) { rem -= cw; continue; }
+            for (int b = 0; b < 32; ++b) {
+                const int h = 32 * w + b;
+                const int first = colour_of_site(2 * h, P.L, P.D);     // colour of site 2h; site 2h+1 has the other
+                const uint32_t f = (Neg[first * W + w] >> b) & 1u, g2 = (Neg[(1 - first) * W + w] >> b) & 1u;
+                if (f) { if (rem == 0) { Cl[first * W + w] = 1u << b; break; } --rem; }
+                if (g2) { if (rem == 0) { Cl[(1 - first) * W + w] = 1u << b; break; } --rem; }
+            }
+            break;
+        }
+    }
+    __syncthreads();
+
+    // grow to the fixed point
+    for (;;) {
+        int changed = 0;
+#pragma unroll 1
+        for (int p = 0; p < 2; ++p) {
+            for (int w = tid; w < W; w += blockDim.x) {
+                const uint32_t neg = Neg[p * W + w], cur = Cl[p * W + w];
+                if (neg & ~cur) {
+                    uint32_t nb[2 * D];
+                    lat.gather(Cl + (1 - p) * W, w, p, nb);
+                    uint32_t any = 0;
+#pragma unroll
+                    for (int k = 0; k < 2 * D; ++k) any |= nb[k];
+                    const uint32_t nw = cur | (any & neg);
+                    if (nw != cur) { Cl[p * W + w] = nw; changed = 1; }
+                }
+            }
+            __syncthreads();
+        }
+        if (!__syncthreads_or(changed)) break;
+    }
+
+    // size, delta = 2 * sum over boundary bonds of J A_i A_j = 2 * (#boundary - 2 #boundary&unsatisfied) (old spins),
+    // each bond seen from its black endpoint; then negate the cluster in both configurations
+    int size = 0, delta = 0;
+    for (int w = tid; w < W; w += blockDim.x) {
+        const uint32_t cb = Cl[w], cwh = Cl[W + w], v = lat.valid(w);
+        size += __popc(cb) + __popc(cwh);
+        uint32_t nbC[2 * D], nbA[2 * D];
+        lat.gather(Cl + W, w, 0, nbC);
+        lat.gather(A[1], w, 0, nbA);
+        const uint32_t ab = A[0][w];
+#pragma unroll
+        for (int k = 0; k < 2 * D; ++k) {
+            const uint32_t bnd = (cb ^ nbC[k]) & v;
+            const uint32_t uns = ab ^ nbA[k] ^ J_words(P, s, 0, k)[w];
+            delta += 2 * (__popc(bnd) - 2 * __popc(bnd & uns));
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        size += __shfl_xor_sync(0xFFFFFFFFu, size, o);
+        delta += __shfl_xor_sync(0xFFFFFFFFu, delta, o);
+    }
+    __syncthreads();                 // all reads of the old A done before anyone writes; scan[] reusable
+    if (lane == 0) { scan[wid] = size; scan[nwarps + wid] = delta; }
+    __syncthreads();
+    for (int p = 0; p < 2; ++p)
+        for (int w = tid; w < W; w += blockDim.x) {
+            const uint32_t c = Cl[p * W + w];
+            if (c) { A[p][w] ^= c; B[p][w] ^= c; }
+        }
+    if (tid == 0) {
+        int sz = 0, dl = 0;
+        for (int i = 0; i < nwarps; ++i) { sz += scan[i]; dl += scan[nwarps + i]; }
+        P.d.E[repA] += dl;
+        P.d.E[repB] -= dl;
+        P.d.last[(size_t)s * P.T + t] = (uint32_t)sz;
+        P.d.cum[(size_t)s * P.T + t] += (unsigned long long)sz;
+    }
+}
+
+// =========================================================================================================
+// a6  two-replica measurement (Eq. (4); link overlap R14).  One CTA per (sample, t).
+//   Q = N - 2 #(q_i = -1);   QL = D*N - 2 #(bonds with q_i != q_j), each bond seen from its black endpoint.
+// dynamic smem: NegW[W] | red[2]
+// =========================================================================================================
+template <class LAT>
+__global__ void __launch_bounds__(128) k_measure(LAT lat, Params P, int32_t *outQ, int32_t *outQL)
+{
+    constexpr int D = LAT::D;
+    extern __shared__ uint32_t msm[];
+    const int W = lat.words();
+    uint32_t *NegW = msm;
+    int *red = (int *)(msm + W);
+    const int t = blockIdx.x, s = blockIdx.y, tid = threadIdx.x;
+    const size_t repA = rep_index(P, s, 0, P.d.sot[rep_index(P, s, 0, t)]);
+    const size_t repB = rep_index(P, s, 1, P.d.sot[rep_index(P, s, 1, t)]);
+    const uint32_t *Ab = spin_words(P, repA, 0), *Aw = spin_words(P, repA, 1);
+    const uint32_t *Bb = spin_words(P, repB, 0), *Bw = spin_words(P, repB, 1);
+    if (tid < 2) red[tid] = 0;
+    for (int w = tid; w < W; w += blockDim.x) NegW[w] = (Aw[w] ^ Bw[w]) & lat.valid(w);
+    __syncthreads();
+    int nneg = 0, ndiff = 0;
+    for (int w = tid; w < W; w += blockDim.x) {
+        const uint32_t v = lat.valid(w), nbk = (Ab[w] ^ Bb[w]) & v;
+        nneg += __popc(nbk) + __popc(NegW[w]);
+        uint32_t nb[2 * D];
+        lat.gather(NegW, w, 0, nb);
+#pragma unroll
+        for (int k = 0; k < 2 * D; ++k) ndiff += __popc((nbk ^ nb[k]) & v);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        nneg += __shfl_xor_sync(0xFFFFFFFFu, nneg, o);
+        ndiff += __shfl_xor_sync(0xFFFFFFFFu, ndiff, o);
+    }
+    if ((tid & 31) == 0) { atomicAdd(red, nneg); atomicAdd(red + 1, ndiff); }
+    __syncthreads();
+    if (tid == 0) {
+        outQ[(size_t)s * P.T + t] = P.N - 2 * red[0];
+        if (outQL) outQL[(size_t)s * P.T + t] = P.D * P.N - 2 * red[1];
+    }
+}
+
+}  // namespace ptg

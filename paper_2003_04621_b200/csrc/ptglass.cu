@@ -1,0 +1,664 @@
+// Host side of the C ABI declared in include/ptglass.h: argument checks, host-computed acceptance tables,
+// workspace carving, kernel dispatch.  No device memory is allocated here (the caller owns the workspace) and
+// there is no CPU fallback: every step of the path runs in the kernels of kernels.cuh.
+#include "../../include/ptglass.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "kernels.cuh"
+
+using namespace ptg;
+
+namespace {
+
+struct Context {
+    void *ws = nullptr;
+    size_t ws_bytes = 0;
+    cudaStream_t stream = nullptr;
+    bool bound = false, inited = false;
+    int force_general = -1;
+    bool fast = false;
+    Params P{};
+    std::vector<double> betas;
+    uint64_t seed = 0;
+    uint32_t n_sweep = 0, n_exchange = 0, n_houdayer = 0;
+    uint64_t launches = 0;
+    size_t stage_bytes = 0;
+};
+
+Context G;
+char g_err[512] = "";
+
+int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CK(call)                                                                                       \
+    do {                                                                                               \
+        cudaError_t e_ = (call);                                                                       \
+        if (e_ != cudaSuccess) return fail(PT_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_));      \
+    } while (0)
+
+#define NEED_INIT()                                                                  \
+    do {                                                                             \
+        if (!G.inited) return fail(PT_ERR_STATE, "%s: pt_init has not been called", __func__); \
+    } while (0)
+
+int check_shape(int L, int d, int S, int T)
+{
+    if (d != 2 && d != 3) return fail(PT_ERR_ARG, "d must be 2 or 3 (got %d)", d);
+    if (L < 2 || (L & 1)) return fail(PT_ERR_ARG, "L must be even and >= 2 (got %d): checkerboard needs a bipartite lattice", L);
+    if (S < 1) return fail(PT_ERR_ARG, "n_samples must be >= 1 (got %d)", S);
+    if (T < 1 || T > 65535) return fail(PT_ERR_ARG, "n_temps must be in [1, 65535] (got %d)", T);
+    const double Nd = std::pow((double)L, d) * d;
+    if (Nd > 2147483647.0) return fail(PT_ERR_ARG, "N*d overflows int32");
+    return PT_OK;
+}
+
+size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// THR(x) = min(2^32-1, floor(2^32 exp(x)))   (R5, R6)
+uint32_t THR(double x)
+{
+    const double v = std::floor(std::ldexp(std::exp(x), 32));
+    if (v >= 4294967295.0) return 4294967295u;
+    if (v <= 0.0) return 0u;
+    return (uint32_t)v;
+}
+
+double thrX_arg(const std::vector<double> &b, int t, uint64_t m) { return -(std::fabs(b[t + 1] - b[t]) * (double)(4 * m)); }
+
+// entries per pair of the stored swap table: the prefix on which any pair's threshold is non-zero
+uint32_t swap_stride(const std::vector<double> &b, int d, long N)
+{
+    const uint64_t m_max = (uint64_t)d * (uint64_t)N / 2;     // |dE| <= 2 d N
+    uint64_t need = 1;
+    for (size_t t = 0; t + 1 < b.size(); ++t) {
+        const double db = std::fabs(b[t + 1] - b[t]);
+        if (db == 0.0) continue;                              // sgn = 0: always accepted, table unused
+        uint64_t lo = 0, hi = m_max + 1;                      // first m with THR == 0 (THR is non-increasing in m)
+        while (lo < hi) {
+            const uint64_t mid = (lo + hi) / 2;
+            if (THR(-(db * (double)(4 * mid))) == 0) hi = mid; else lo = mid + 1;
+        }
+        if (lo > need) need = lo;
+    }
+    if (need > m_max + 1) need = m_max + 1;
+    return (uint32_t)need;
+}
+
+struct Carve {
+    size_t off = 0;
+    template <class T> T *take(void *base, size_t n)
+    {
+        T *p = base ? (T *)((char *)base + off) : nullptr;
+        off = align_up(off + n * sizeof(T));
+        return p;
+    }
+};
+
+// Lay the device arrays out in the workspace; with base == nullptr only the total size is computed.
+size_t carve(void *base, int L, int d, int S, int T, uint32_t strideX, DevPtrs *out, size_t *stage_bytes)
+{
+    const size_t N = (d == 2) ? (size_t)L * L : (size_t)L * L * L;
+    const size_t W = (size_t)words_per_colour((int)N);
+    const size_t R = (size_t)S * 2 * T;
+    Carve c;
+    DevPtrs p{};
+    p.spin = c.take<uint32_t>(base, R * 2 * W);
+    p.Jn = c.take<uint32_t>(base, (size_t)S * 2 * 2 * d * W);
+    p.E = c.take<int32_t>(base, R);
+    p.tos = c.take<int32_t>(base, R);
+    p.sot = c.take<int32_t>(base, R);
+    p.thrM = c.take<uint32_t>(base, (size_t)T * 4);
+    p.thrX = c.take<uint32_t>(base, (size_t)(T > 1 ? T - 1 : 1) * strideX);
+    p.sgn = c.take<int32_t>(base, (size_t)T);
+    p.accepts = c.take<unsigned long long>(base, (size_t)S * 2 * T);
+    p.last = c.take<uint32_t>(base, (size_t)S * T);
+    p.cum = c.take<unsigned long long>(base, (size_t)S * T);
+    p.outE = c.take<int32_t>(base, R);
+    p.outQ = c.take<int32_t>(base, (size_t)S * T);
+    p.outQL = c.take<int32_t>(base, (size_t)S * T);
+    p.mismatch = c.take<int>(base, 64);
+    const size_t sb = std::max(R * N, (size_t)S * d * N);
+    p.stage = c.take<int8_t>(base, sb);
+    if (out) *out = p;
+    if (stage_bytes) *stage_bytes = sb;
+    return c.off;
+}
+
+// upper bound of strideX used for sizing before the betas are known: the full table
+uint32_t full_stride(int L, int d)
+{
+    const uint64_t N = (d == 2) ? (uint64_t)L * L : (uint64_t)L * L * L;
+    return (uint32_t)((uint64_t)d * N / 2 + 1);
+}
+
+bool fast_supported(int L, int d)
+{
+    if (L < 8 || (L & (L - 1))) return false;
+    int lg = 0;
+    while ((1 << lg) < L) ++lg;
+    return d == 2 ? (lg >= 3 && lg <= 8) : (lg >= 3 && lg <= 5);
+}
+
+int grid_for(long total, int block) { return (int)std::min<long>((total + block - 1) / block, 148L * 32); }
+
+// Run `body` with `lat` bound to the lattice implementation of the current problem.
+#define FAST_CASE(DD, LG)                                  \
+    if (G.P.D == DD && G.P.L == (1 << LG)) {               \
+        FastLat<DD, LG> lat;                               \
+        body(lat);                                         \
+        return;                                            \
+    }
+
+template <class F> void with_lattice(F body)
+{
+    if (G.fast) {
+        FAST_CASE(2, 3) FAST_CASE(2, 4) FAST_CASE(2, 5) FAST_CASE(2, 6) FAST_CASE(2, 7) FAST_CASE(2, 8)
+        FAST_CASE(3, 3) FAST_CASE(3, 4) FAST_CASE(3, 5)
+    }
+    if (G.P.D == 2) { GenLat<2> lat(G.P.L); body(lat); }
+    else            { GenLat<3> lat(G.P.L); body(lat); }
+}
+
+template <class K> cudaError_t allow_smem(K kernel, size_t bytes)
+{
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+cudaError_t launch_energy(int mode)
+{
+    cudaError_t err = cudaSuccess;
+    with_lattice([&](auto lat) {
+        const long reps = (long)G.P.S * 2 * G.P.T;
+        const int wpb = 4;
+        k_energy<<<(unsigned)((reps + wpb - 1) / wpb), wpb * 32, 0, G.stream>>>(lat, G.P, mode);
+        ++G.launches;
+        err = cudaGetLastError();
+    });
+    return err;
+}
+
+// replicas per CTA of the sweep kernel: the largest divisor of 2T with R*W <= 1024 work items
+int sweep_group(int T, int W)
+{
+    int best = 1;
+    for (int R = 1; R <= 2 * T; ++R)
+        if ((2 * T) % R == 0 && (long)R * W <= 1024) best = R;
+    return best;
+}
+
+cudaError_t launch_sweep(int n)
+{
+    cudaError_t err = cudaSuccess;
+    with_lattice([&](auto lat) {
+        using LAT = decltype(lat);
+        const int W = G.P.W, D = G.P.D;
+        const int R = sweep_group(G.P.T, W);
+        const size_t smem = ((size_t)2 * 2 * D * W + (size_t)R * 2 * W + (size_t)R * 4 + (size_t)R) * 4;
+        err = allow_smem(k_sweep<LAT>, smem);
+        if (err != cudaSuccess) return;
+        dim3 grid((unsigned)(2 * G.P.T / R), (unsigned)G.P.S);
+        k_sweep<LAT><<<grid, 256, smem, G.stream>>>(lat, G.P, R, G.n_sweep, n);
+        ++G.launches;
+        err = cudaGetLastError();
+    });
+    return err;
+}
+
+cudaError_t launch_exchange()
+{
+    const int T = G.P.T;
+    const long chains = (long)G.P.S * 2;
+    int wpb = 4;
+    while (wpb > 1 && (size_t)wpb * 2 * T * 4 > 64 * 1024) wpb >>= 1;
+    const size_t smem = (size_t)wpb * 2 * T * 4;
+    if (smem > 64 * 1024) {      // very long ladders: walk on global scratch instead of shared memory
+        k_exchange<true><<<(unsigned)chains, 32, 0, G.stream>>>(G.P, G.n_exchange);
+    } else {
+        cudaError_t err = allow_smem(k_exchange<false>, smem);
+        if (err != cudaSuccess) return err;
+        k_exchange<false><<<(unsigned)((chains + wpb - 1) / wpb), wpb * 32, smem, G.stream>>>(G.P, G.n_exchange);
+    }
+    ++G.launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_houdayer()
+{
+    cudaError_t err = cudaSuccess;
+    with_lattice([&](auto lat) {
+        using LAT = decltype(lat);
+        const int threads = 128;
+        const size_t smem = ((size_t)4 * G.P.W + 2 * (threads / 32) + 2) * 4;
+        err = allow_smem(k_houdayer<LAT>, smem);
+        if (err != cudaSuccess) return;
+        dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
+        k_houdayer<LAT><<<grid, threads, smem, G.stream>>>(lat, G.P, G.n_houdayer);
+        ++G.launches;
+        err = cudaGetLastError();
+    });
+    return err;
+}
+
+cudaError_t launch_measure(int32_t *Q, int32_t *QL)
+{
+    cudaError_t err = cudaSuccess;
+    with_lattice([&](auto lat) {
+        using LAT = decltype(lat);
+        const size_t smem = ((size_t)G.P.W + 2) * 4;
+        dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
+        k_measure<LAT><<<grid, 128, smem, G.stream>>>(lat, G.P, Q, QL);
+        ++G.launches;
+        err = cudaGetLastError();
+    });
+    return err;
+}
+
+int d2h(void *dst, const void *src, size_t bytes)
+{
+    CK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, G.stream));
+    CK(cudaStreamSynchronize(G.stream));
+    return PT_OK;
+}
+
+int pack_spins_and_energy()
+{
+    const long total = (long)G.P.S * 2 * G.P.T * 2 * G.P.W;
+    k_pack_spins<<<grid_for(total, 256), 256, 0, G.stream>>>(G.P);
+    ++G.launches;
+    CK(cudaGetLastError());
+    CK(launch_energy(0));
+    return PT_OK;
+}
+
+int pack_couplings()
+{
+    CK(cudaMemsetAsync(G.P.d.Jn, 0, (size_t)G.P.S * 2 * 2 * G.P.D * G.P.W * 4, G.stream));
+    k_pack_couplings<<<grid_for((long)G.P.S * G.P.D * G.P.N, 256), 256, 0, G.stream>>>(G.P);
+    ++G.launches;
+    CK(cudaGetLastError());
+    return PT_OK;
+}
+
+}  // namespace
+
+// ============================================================================================================
+extern "C" {
+
+const char *pt_last_error(void) { return g_err; }
+
+int pt_workspace_bytes(int L, int d, int n_samples, int n_temps, size_t *bytes_out)
+{
+    if (!bytes_out) return fail(PT_ERR_ARG, "bytes_out is NULL");
+    const int rc = check_shape(L, d, n_samples, n_temps);
+    if (rc) return rc;
+    *bytes_out = carve(nullptr, L, d, n_samples, n_temps, full_stride(L, d), nullptr, nullptr);
+    return PT_OK;
+}
+
+int pt_bind(void *device_workspace, size_t bytes, void *cuda_stream)
+{
+    if (!device_workspace) return fail(PT_ERR_ARG, "device_workspace is NULL");
+    if (((uintptr_t)device_workspace & 255) != 0) return fail(PT_ERR_ARG, "device_workspace must be 256-byte aligned");
+    G = Context{};
+    G.ws = device_workspace;
+    G.ws_bytes = bytes;
+    G.stream = (cudaStream_t)cuda_stream;
+    G.bound = true;
+    return PT_OK;
+}
+
+int pt_force_general_path(int force)
+{
+    if (force != -1 && force != 0) return fail(PT_ERR_ARG, "force must be -1 or 0");
+    if (G.inited) return fail(PT_ERR_STATE, "pt_force_general_path must precede pt_init");
+    G.force_general = force;
+    return PT_OK;
+}
+
+int pt_get_path(int *fast)
+{
+    NEED_INIT();
+    if (fast) *fast = G.fast ? 1 : 0;
+    return PT_OK;
+}
+
+int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas, uint64_t seed, uint32_t sample_offset)
+{
+    if (!G.bound) return fail(PT_ERR_STATE, "pt_init: no workspace bound (call pt_bind first)");
+    G.inited = false;
+    int rc = check_shape(L, d, n_samples, n_temps);
+    if (rc) return rc;
+    if (!betas) return fail(PT_ERR_ARG, "betas is NULL");
+    for (int t = 0; t < n_temps; ++t)
+        if (!std::isfinite(betas[t]) || betas[t] < 0.0) return fail(PT_ERR_ARG, "betas[%d] is negative or not finite", t);
+    if ((uint64_t)sample_offset + (uint64_t)n_samples > 4294967296ull)
+        return fail(PT_ERR_ARG, "sample_offset + n_samples overflows 2^32");
+
+    G.betas.assign(betas, betas + n_temps);
+    G.seed = seed;
+    Params &P = G.P;
+    P = Params{};
+    P.L = L; P.D = d; P.S = n_samples; P.T = n_temps;
+    P.N = (d == 2) ? L * L : L * L * L;
+    P.NH = P.N / 2;
+    P.W = words_per_colour(P.N);
+    P.g0 = sample_offset;
+    P.rk = make_round_keys((uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32));
+    P.strideX = swap_stride(G.betas, d, P.N);
+    const size_t need = carve(G.ws, L, d, n_samples, n_temps, P.strideX, &P.d, &G.stage_bytes);
+    if (need > G.ws_bytes)
+        return fail(PT_ERR_STATE, "workspace too small: %zu bytes bound, %zu needed", G.ws_bytes, need);
+    G.fast = (G.force_general != 0) && fast_supported(L, d);
+    G.n_sweep = G.n_exchange = G.n_houdayer = 0;
+
+    // acceptance tables on the host, in double (R5, R6)
+    std::vector<uint32_t> thrM((size_t)n_temps * 4, 0u);
+    for (int t = 0; t < n_temps; ++t)
+        for (int k = 1; k <= d; ++k) thrM[(size_t)t * 4 + (k - 1)] = THR(-(betas[t] * (double)(4 * k)));
+    std::vector<uint32_t> thrX((size_t)(n_temps > 1 ? n_temps - 1 : 1) * P.strideX, 0u);
+    std::vector<int32_t> sgn((size_t)n_temps, 0);
+    for (int t = 0; t + 1 < n_temps; ++t) {
+        sgn[t] = (betas[t + 1] > betas[t]) - (betas[t + 1] < betas[t]);
+        for (uint32_t m = 0; m < P.strideX; ++m) thrX[(size_t)t * P.strideX + m] = THR(thrX_arg(G.betas, t, m));
+    }
+    CK(cudaMemcpyAsync(P.d.thrM, thrM.data(), thrM.size() * 4, cudaMemcpyHostToDevice, G.stream));
+    CK(cudaMemcpyAsync(P.d.thrX, thrX.data(), thrX.size() * 4, cudaMemcpyHostToDevice, G.stream));
+    CK(cudaMemcpyAsync(P.d.sgn, sgn.data(), sgn.size() * 4, cudaMemcpyHostToDevice, G.stream));
+    CK(cudaStreamSynchronize(G.stream));       // the host vectors go out of scope
+    CK(cudaMemsetAsync(P.d.accepts, 0, (size_t)P.S * 2 * P.T * 8, G.stream));
+    CK(cudaMemsetAsync(P.d.last, 0, (size_t)P.S * P.T * 4, G.stream));
+    CK(cudaMemsetAsync(P.d.cum, 0, (size_t)P.S * P.T * 8, G.stream));
+    CK(cudaMemsetAsync(P.d.mismatch, 0, 64 * sizeof(int), G.stream));
+
+    // couplings, spins (Philox domains 1, 2), identity permutations, energies
+    k_draw_couplings<<<grid_for((long)P.S * P.D * (P.N / 4), 256), 256, 0, G.stream>>>(P);
+    ++G.launches;
+    CK(cudaGetLastError());
+    if ((rc = pack_couplings())) return rc;
+    k_draw_spins<<<grid_for((long)P.S * 2 * P.T * (P.N / 4), 256), 256, 0, G.stream>>>(P);
+    ++G.launches;
+    CK(cudaGetLastError());
+    k_identity_perm<<<grid_for((long)P.S * 2 * P.T, 256), 256, 0, G.stream>>>(P);
+    ++G.launches;
+    CK(cudaGetLastError());
+    if ((rc = pack_spins_and_energy())) return rc;
+    CK(cudaStreamSynchronize(G.stream));
+    G.inited = true;
+    return PT_OK;
+}
+
+int pt_init(int L, int d, int n_samples, int n_temps, const double *betas, uint64_t seed)
+{
+    return pt_init_shard(L, d, n_samples, n_temps, betas, seed, 0u);
+}
+
+int pt_free(void)
+{
+    if (G.bound && G.stream) cudaStreamSynchronize(G.stream);
+    G.inited = false;
+    return PT_OK;
+}
+
+// ---- updates ---------------------------------------------------------------------------------------------
+
+int pt_sweep(int n)
+{
+    NEED_INIT();
+    if (n < 0) return fail(PT_ERR_ARG, "pt_sweep: n must be >= 0");
+    if ((uint64_t)G.n_sweep + (uint64_t)n > 4294967295ull) return fail(PT_ERR_OVERFLOW, "sweep counter would overflow");
+    if (n == 0) return PT_OK;
+    CK(launch_sweep(n));
+    G.n_sweep += (uint32_t)n;
+    return PT_OK;
+}
+
+int pt_exchange(void)
+{
+    NEED_INIT();
+    if (G.n_exchange == 4294967295u) return fail(PT_ERR_OVERFLOW, "exchange counter would overflow");
+    CK(launch_exchange());
+    G.n_exchange += 1;
+    return PT_OK;
+}
+
+int houdayer_step(void)
+{
+    NEED_INIT();
+    if (G.n_houdayer == 4294967295u) return fail(PT_ERR_OVERFLOW, "Houdayer counter would overflow");
+    CK(launch_houdayer());
+    G.n_houdayer += 1;
+    return PT_OK;
+}
+
+int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
+{
+    NEED_INIT();
+    if (n_mcs < 0 || n_metro < 0) return fail(PT_ERR_ARG, "pt_mcs: n_mcs and n_metro must be >= 0");
+    const uint64_t M = (uint64_t)n_mcs;
+    if ((uint64_t)G.n_sweep + M * (uint64_t)n_metro > 4294967295ull ||
+        (do_exchange && (uint64_t)G.n_exchange + M > 4294967295ull) ||
+        (do_houdayer && (uint64_t)G.n_houdayer + M > 4294967295ull))
+        return fail(PT_ERR_OVERFLOW, "a step counter would overflow");
+    for (int m = 0; m < n_mcs; ++m) {
+        if (n_metro > 0) { CK(launch_sweep(n_metro)); G.n_sweep += (uint32_t)n_metro; }
+        if (do_houdayer) { CK(launch_houdayer()); G.n_houdayer += 1; }
+        if (do_exchange) { CK(launch_exchange()); G.n_exchange += 1; }
+    }
+    return PT_OK;
+}
+
+// ---- observables -----------------------------------------------------------------------------------------
+
+int pt_get_energy_device(int32_t *E_dev)
+{
+    NEED_INIT();
+    if (!E_dev) return fail(PT_ERR_ARG, "E is NULL");
+    k_energy_by_temp<<<grid_for((long)G.P.S * 2 * G.P.T, 256), 256, 0, G.stream>>>(G.P, E_dev);
+    ++G.launches;
+    CK(cudaGetLastError());
+    return PT_OK;
+}
+
+int pt_get_energy(int32_t *E)
+{
+    NEED_INIT();
+    if (!E) return fail(PT_ERR_ARG, "E is NULL");
+    const int rc = pt_get_energy_device(G.P.d.outE);
+    if (rc) return rc;
+    return d2h(E, G.P.d.outE, (size_t)G.P.S * 2 * G.P.T * 4);
+}
+
+int pt_measure_overlap_device(int32_t *Q_dev, int32_t *QL_dev)
+{
+    NEED_INIT();
+    if (!Q_dev) return fail(PT_ERR_ARG, "Q is NULL");
+    CK(launch_measure(Q_dev, QL_dev));
+    return PT_OK;
+}
+
+int pt_measure_overlap(int32_t *Q, int32_t *QL)
+{
+    NEED_INIT();
+    if (!Q) return fail(PT_ERR_ARG, "Q is NULL");
+    CK(launch_measure(G.P.d.outQ, QL ? G.P.d.outQL : nullptr));
+    int rc = d2h(Q, G.P.d.outQ, (size_t)G.P.S * G.P.T * 4);
+    if (rc) return rc;
+    if (QL) rc = d2h(QL, G.P.d.outQL, (size_t)G.P.S * G.P.T * 4);
+    return rc;
+}
+
+int pt_get_swap_counts(uint64_t *attempts, uint64_t *accepts)
+{
+    NEED_INIT();
+    const size_t n = (size_t)G.P.S * 2 * (G.P.T - 1);
+    if (accepts && n) {
+        const int rc = d2h(accepts, G.P.d.accepts, n * 8);
+        if (rc) return rc;
+    }
+    if (attempts)                                   // every pass proposes every neighbouring pair once (R9)
+        for (size_t k = 0; k < n; ++k) attempts[k] = G.n_exchange;
+    return PT_OK;
+}
+
+int pt_get_cluster_sizes(uint32_t *last, uint64_t *cumulative)
+{
+    NEED_INIT();
+    const size_t n = (size_t)G.P.S * G.P.T;
+    int rc = PT_OK;
+    if (last) rc = d2h(last, G.P.d.last, n * 4);
+    if (!rc && cumulative) rc = d2h(cumulative, G.P.d.cum, n * 8);
+    return rc;
+}
+
+int pt_get_perm(int32_t *temp_of_slot, int32_t *slot_of_temp)
+{
+    NEED_INIT();
+    const size_t n = (size_t)G.P.S * 2 * G.P.T;
+    int rc = PT_OK;
+    if (temp_of_slot) rc = d2h(temp_of_slot, G.P.d.tos, n * 4);
+    if (!rc && slot_of_temp) rc = d2h(slot_of_temp, G.P.d.sot, n * 4);
+    return rc;
+}
+
+// ---- state access ----------------------------------------------------------------------------------------
+
+int pt_get_spins(int8_t *spins)
+{
+    NEED_INIT();
+    if (!spins) return fail(PT_ERR_ARG, "spins is NULL");
+    const size_t n = (size_t)G.P.S * 2 * G.P.T * G.P.N;
+    k_unpack_spins<<<grid_for((long)n, 256), 256, 0, G.stream>>>(G.P);
+    ++G.launches;
+    CK(cudaGetLastError());
+    return d2h(spins, G.P.d.stage, n);
+}
+
+int pt_get_couplings(int8_t *J)
+{
+    NEED_INIT();
+    if (!J) return fail(PT_ERR_ARG, "J is NULL");
+    const size_t n = (size_t)G.P.S * G.P.D * G.P.N;
+    k_unpack_couplings<<<grid_for((long)n, 256), 256, 0, G.stream>>>(G.P);
+    ++G.launches;
+    CK(cudaGetLastError());
+    return d2h(J, G.P.d.stage, n);
+}
+
+int pt_get_thresholds(uint32_t *thrM, uint32_t *thrX, size_t thrX_stride)
+{
+    NEED_INIT();
+    const int T = G.P.T, d = G.P.D;
+    if (thrM)
+        for (int t = 0; t < T; ++t)
+            for (int k = 1; k <= d; ++k) thrM[(size_t)t * d + (k - 1)] = THR(-(G.betas[t] * (double)(4 * k)));
+    if (thrX)
+        for (int t = 0; t + 1 < T; ++t)
+            for (size_t m = 0; m < thrX_stride; ++m) thrX[(size_t)t * thrX_stride + m] = THR(thrX_arg(G.betas, t, m));
+    return PT_OK;
+}
+
+int pt_get_counters(uint32_t *n_sweep, uint32_t *n_exchange, uint32_t *n_houdayer)
+{
+    NEED_INIT();
+    if (n_sweep) *n_sweep = G.n_sweep;
+    if (n_exchange) *n_exchange = G.n_exchange;
+    if (n_houdayer) *n_houdayer = G.n_houdayer;
+    return PT_OK;
+}
+
+static int check_pm1(const int8_t *a, size_t n, const char *what)
+{
+    for (size_t k = 0; k < n; ++k)
+        if (a[k] != 1 && a[k] != -1) return fail(PT_ERR_ARG, "%s[%zu] = %d is not +1/-1", what, k, (int)a[k]);
+    return PT_OK;
+}
+
+int pt_set_spins(const int8_t *spins)
+{
+    NEED_INIT();
+    if (!spins) return fail(PT_ERR_ARG, "spins is NULL");
+    const size_t n = (size_t)G.P.S * 2 * G.P.T * G.P.N;
+    int rc = check_pm1(spins, n, "spins");
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(G.P.d.stage, spins, n, cudaMemcpyHostToDevice, G.stream));
+    if ((rc = pack_spins_and_energy())) return rc;
+    CK(cudaStreamSynchronize(G.stream));       // the caller may reuse `spins` as soon as we return
+    return PT_OK;
+}
+
+int pt_set_couplings(const int8_t *J)
+{
+    NEED_INIT();
+    if (!J) return fail(PT_ERR_ARG, "J is NULL");
+    const size_t n = (size_t)G.P.S * G.P.D * G.P.N;
+    int rc = check_pm1(J, n, "J");
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(G.P.d.stage, J, n, cudaMemcpyHostToDevice, G.stream));
+    if ((rc = pack_couplings())) return rc;
+    CK(launch_energy(0));
+    CK(cudaStreamSynchronize(G.stream));
+    return PT_OK;
+}
+
+int pt_recompute_energy(int32_t *E_slot_order, int *mismatch_count)
+{
+    NEED_INIT();
+    CK(cudaMemsetAsync(G.P.d.mismatch, 0, sizeof(int), G.stream));
+    CK(launch_energy(1));
+    int bad = 0;
+    int rc = d2h(&bad, G.P.d.mismatch, sizeof(int));
+    if (rc) return rc;
+    if (mismatch_count) *mismatch_count = bad;
+    if (E_slot_order) rc = d2h(E_slot_order, G.P.d.outE, (size_t)G.P.S * 2 * G.P.T * 4);
+    return rc;
+}
+
+// ---- diagnostics -----------------------------------------------------------------------------------------
+
+int pt_synchronize(void)
+{
+    if (!G.bound) return fail(PT_ERR_STATE, "not bound");
+    CK(cudaStreamSynchronize(G.stream));
+    return PT_OK;
+}
+
+int pt_get_launch_count(uint64_t *n_launches)
+{
+    if (!n_launches) return fail(PT_ERR_ARG, "n_launches is NULL");
+    *n_launches = G.launches;
+    return PT_OK;
+}
+
+int pt_philox_selftest(const uint32_t key[2], const uint32_t *ctr, uint32_t *out, int n)
+{
+    if (!G.bound) return fail(PT_ERR_STATE, "pt_philox_selftest: no workspace bound");
+    if (!key || !ctr || !out || n < 1) return fail(PT_ERR_ARG, "bad arguments");
+    // scratch: the staging area when initialised, else the start of the workspace
+    char *scratch = G.inited ? (char *)G.P.d.stage : (char *)G.ws;
+    const size_t avail = G.inited ? G.stage_bytes : G.ws_bytes;
+    if ((size_t)n * 32 > avail) return fail(PT_ERR_ARG, "n too large for the scratch area");
+    uint32_t *dctr = (uint32_t *)scratch, *dout = dctr + (size_t)n * 4;
+    CK(cudaMemcpyAsync(dctr, ctr, (size_t)n * 16, cudaMemcpyHostToDevice, G.stream));
+    k_philox_selftest<<<(n + 127) / 128, 128, 0, G.stream>>>(make_round_keys(key[0], key[1]), dctr, dout, n);
+    ++G.launches;
+    CK(cudaGetLastError());
+    return d2h(out, dout, (size_t)n * 16);
+}
+
+}  // extern "C"

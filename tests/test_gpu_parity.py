@@ -1,0 +1,205 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, bit for bit, on the same seeded
+inputs: spins, couplings, thresholds, energies, both permutation arrays, swap counts, cluster sizes, overlaps.
+Run on the B200 box with `-m gpu`."""
+import numpy as np
+import pytest
+
+from oracle import ref
+from paper_2003_04621_b200 import binding as B
+from paper_2003_04621_b200 import build as build_mod
+from paper_2003_04621_b200 import workloads as wl
+from tests import helpers as H
+
+pytestmark = pytest.mark.gpu
+SEED = wl.SEED
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    build_mod.build()
+    yield
+    B.pt_free()
+
+
+def assert_same_state(o, tag=""):
+    a, b = o.state(), B.state()
+    for k in a:
+        if not np.array_equal(a[k], b[k]):
+            bad = np.argwhere(a[k] != b[k])
+            raise AssertionError("%s %s differs at %d places, first %s: oracle %s gpu %s" % (
+                tag, k, len(bad), bad[0], a[k][tuple(bad[0])], b[k][tuple(bad[0])]))
+    Qo, QLo = o.measure_overlap()
+    Qg, QLg = B.pt_measure_overlap()
+    assert np.array_equal(Qo, Qg) and np.array_equal(QLo, QLg), tag + " overlaps differ"
+    assert B.pt_recompute_energy()[1] == 0, tag + " tracked energy != recomputed"
+
+
+def open_both(L, d, S, T, betas, offset=0, general=False):
+    o = ref.Oracle(L, d, S, T, betas, SEED, offset)
+    B.pt_open(L, d, S, T, betas, SEED, offset, general=general)
+    return o
+
+
+def test_philox_device_known_answers_and_oracle():
+    import json, os
+    B.pt_open(32, 2, 8, 8, wl.betas_linear(0.2, 1.0, 8), SEED)      # staging area doubles as the scratch
+    with open(os.path.join(os.path.dirname(__file__), "golden", "philox_known_answers.json")) as f:
+        vecs = json.load(f)["vectors"]
+    for v in vecs:
+        out = B.pt_philox_selftest([int(k, 16) for k in v["key"]], [[int(c, 16) for c in v["ctr"]]])
+        assert ["%08x" % x for x in out[0]] == v["out"]
+    rng = np.random.default_rng(3)
+    ctr = rng.integers(0, 2 ** 32, size=(1000, 4), dtype=np.uint64).astype(np.uint32)
+    key = np.array([0xdeadbeef, 0x12345678], dtype=np.uint32)
+    got = B.pt_philox_selftest(key, ctr)
+    assert np.array_equal(got, H.philox_np(key, ctr))
+    for n in range(0, 1000, 97):
+        assert np.array_equal(got[n], ref.philox(key, ctr[n]))
+
+
+# (L, d, S, T): fast path = L a power of two >= 8; the others run the general-L kernels
+SHAPES = [(8, 2, 4, 8), (16, 2, 3, 5), (32, 2, 3, 6), (64, 2, 2, 3), (128, 2, 1, 3),
+          (8, 3, 3, 4), (16, 3, 2, 3),
+          (2, 2, 2, 3), (4, 2, 3, 4), (6, 2, 2, 5), (10, 2, 2, 3), (12, 2, 1, 2), (20, 2, 1, 2),
+          (2, 3, 3, 3), (4, 3, 2, 4), (6, 3, 2, 3), (10, 3, 1, 2)]
+
+
+@pytest.mark.parametrize("L,d,S,T", SHAPES)
+def test_init_state_matches_oracle(L, d, S, T):
+    betas = wl.betas_geometric(0.3, 1.6, T)
+    o = open_both(L, d, S, T, betas, offset=5)
+    assert np.array_equal(o.get_couplings(), B.pt_get_couplings())
+    tm_o, tx_o = o.get_thresholds(64)
+    tm_g, tx_g = B.pt_get_thresholds(64)
+    assert np.array_equal(tm_o, tm_g) and np.array_equal(tx_o, tx_g)
+    assert_same_state(o, "init")
+    assert B.pt_get_path() == int(L >= 8 and (L & (L - 1)) == 0 and ((d == 2 and L <= 256) or (d == 3 and L <= 32)))
+
+
+@pytest.mark.parametrize("L,d,S,T", SHAPES)
+def test_sweep_exchange_houdayer_match_oracle(L, d, S, T):
+    betas = wl.betas_geometric(0.3, 1.6, T)
+    o = open_both(L, d, S, T, betas, offset=1)
+    for step in range(6):
+        o.sweep(1); B.pt_sweep(1)
+        assert_same_state(o, "sweep %d" % step)
+        o.houdayer_step(); B.houdayer_step()
+        assert_same_state(o, "houdayer %d" % step)
+        o.exchange(); B.pt_exchange()
+        assert_same_state(o, "exchange %d" % step)
+    o.sweep(3); B.pt_sweep(3)               # several sweeps in one residency
+    assert_same_state(o, "sweep(3)")
+    o.mcs(5, 2, True, True); B.pt_mcs(5, 2, True, True)
+    assert_same_state(o, "mcs")
+
+
+@pytest.mark.parametrize("L,d", [(8, 2), (16, 2), (32, 2), (64, 2), (8, 3), (16, 3)])
+def test_general_path_equals_fast_path_and_oracle(L, d):
+    S, T = 2, 4
+    betas = wl.betas_linear(0.2, 1.4, T)
+    o = open_both(L, d, S, T, betas, general=True)
+    assert B.pt_get_path() == 0
+    o.mcs(4, 1, True, True); B.pt_mcs(4, 1, True, True)
+    assert_same_state(o, "general")
+    general = B.state()
+    B.pt_open(L, d, S, T, betas, SEED, 0)
+    assert B.pt_get_path() == 1
+    B.pt_mcs(4, 1, True, True)
+    fast = B.state()
+    for k in fast:
+        assert np.array_equal(fast[k], general[k]), k
+
+
+def test_config_C1_full_run():
+    w = wl.C1
+    o = open_both(w.L, w.d, w.S, w.T, w.betas())
+    done = 0
+    for upto in (1, 2, 10, 100, 1000):
+        o.mcs(upto - done, 1, False, True); B.pt_mcs(upto - done, 1, False, True)
+        done = upto
+        assert_same_state(o, "C1 after %d MCS" % upto)
+    # the survey's worked example W1 (tests/golden/survey_worked_examples.json)
+    assert H.crc(B.pt_get_spins()) == "15a1d815"
+    assert B.pt_get_swap_counts()[1].sum(axis=(0, 1)).tolist() == [536, 1136, 2482, 3973, 5292, 6483, 7319]
+
+
+def test_worked_example_W3_with_houdayer_3d():
+    b3 = np.array([0.4 * pow(1.1 / 0.4, t / 3.0) for t in range(4)])
+    o = open_both(4, 3, 2, 4, b3)
+    o.mcs(100, 1, True, True); B.pt_mcs(100, 1, True, True)
+    assert_same_state(o, "W3")
+    assert H.crc(B.pt_get_spins()) == "b4e49247"
+    assert B.pt_get_cluster_sizes()[1].sum() == 25733
+
+
+@pytest.mark.parametrize("name,S,n_mcs", [("C2", 6, 40), ("C3", 6, 40), ("C4", 2, 12), ("C5", 1, 6)])
+def test_config_shapes_subset(name, S, n_mcs):
+    """BASELINE configs C2-C5 at full L, T and beta ladder on the first S samples (every sample is a pure
+    function of (seed, global sample index), so a subset run equals the same samples of the full run)."""
+    w = wl.CONFIGS[name]
+    o = open_both(w.L, w.d, S, w.T, w.betas())
+    rec_o, rec_g = [], []
+    for m in range(1, n_mcs + 1):
+        o.mcs(1, 1, w.houdayer, True); B.pt_mcs(1, 1, w.houdayer, True)
+        if w.measure_every and m % w.measure_every == 0:
+            rec_o.append(o.measure_overlap()); rec_g.append(B.pt_measure_overlap())
+        if m in (1, 2, n_mcs // 2):
+            assert_same_state(o, "%s MCS %d" % (name, m))
+    assert_same_state(o, "%s end" % name)
+    for a, b in zip(rec_o, rec_g):
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_sharding_invariance_and_offsets():
+    w = wl.C3
+    T = 6
+    betas = wl.betas_geometric(0.4, 1.1, T)
+    B.pt_open(w.L, w.d, 4, T, betas, SEED, 0)
+    B.pt_mcs(10, 1, True, True)
+    full = B.state()
+    B.pt_open(w.L, w.d, 2, T, betas, SEED, 2)
+    B.pt_mcs(10, 1, True, True)
+    part = B.state()
+    for k in full:
+        if k != "counters":
+            assert np.array_equal(full[k][2:], part[k]), k
+
+
+def test_special_cases_and_set_hooks():
+    L, d, S, T = 16, 2, 2, 3
+    betas = np.array([0.0, 0.0, 0.0])
+    o = open_both(L, d, S, T, betas)
+    s0 = B.pt_get_spins()
+    B.pt_sweep(1)
+    assert np.array_equal(B.pt_get_spins(), -s0)              # beta = 0: every site flips
+    B.pt_exchange()
+    assert np.array_equal(B.pt_get_perm()[1][0, 0], [1, 2, 0])   # equal betas: cyclic shift
+    # B = -A: whole lattice exchanged; B = A: nothing happens
+    s = s0.copy(); s[:, 1] = -s[:, 0]
+    B.pt_set_spins(s)
+    E0 = B.pt_get_energy()
+    B.houdayer_step()
+    assert (B.pt_get_cluster_sizes()[0] == L * L).all()
+    assert np.array_equal(B.pt_get_energy(), E0)
+    Q, QL = B.pt_measure_overlap()
+    assert (Q == -L * L).all() and (QL == d * L * L).all()
+    s[:, 1] = s[:, 0]
+    B.pt_set_spins(s)
+    B.houdayer_step()
+    assert (B.pt_get_cluster_sizes()[0] == 0).all() and np.array_equal(B.pt_get_spins(), s)
+    # ferromagnet through pt_set_couplings
+    B.pt_set_couplings(np.ones((S, d, L * L), dtype=np.int8))
+    B.pt_set_spins(np.ones((S, 2, T, L * L), dtype=np.int8))
+    assert (B.pt_recompute_energy()[0] == -d * L * L).all()
+    with pytest.raises(B.PTError):
+        B.pt_set_spins(np.zeros((S, 2, T, L * L), dtype=np.int8))
+
+
+def test_single_temperature_and_counters():
+    o = open_both(8, 3, 2, 1, np.array([0.7]))
+    o.mcs(3, 1, True, True); B.pt_mcs(3, 1, True, True)
+    assert_same_state(o, "T=1")
+    assert B.pt_get_counters() == (3, 3, 3)
+    with pytest.raises(B.PTError) as e:
+        B.pt_sweep(-1)
+    assert e.value.code == B.PT_ERR_ARG
