@@ -123,6 +123,11 @@ int pt_recompute_energy(int32_t *E_slot_order /* [S][2][T] or NULL */, int *mism
 
 int pt_synchronize(void);                          /* cudaStreamSynchronize on the bound stream */
 int pt_get_launch_count(uint64_t *n_launches);     /* kernels launched by this library since pt_bind */
+/* Per-kernel-class device times: when on, every launch of the sweep (class 0), Houdayer (1), exchange (2) and
+ * measurement (3) kernels is bracketed by CUDA events on the bound stream.  pt_set_profiling resets the sums;
+ * pt_get_kernel_times synchronises and returns the summed milliseconds and launch counts since then. */
+int pt_set_profiling(int on);
+int pt_get_kernel_times(double ms[4], uint64_t launches[4]);
 /* Which code path the bound problem uses: 1 = word-parallel kernels specialised for L a power of two >= 8,
  * 0 = general-L kernels.  force = -1 leaves the choice to the library, 0 forces the general path (tests). */
 int pt_get_path(int *fast);

@@ -45,6 +45,8 @@ SYMBOLS = {
     "pt_recompute_energy": (_i, [_vp, _vp]),
     "pt_synchronize": (_i, []),
     "pt_get_launch_count": (_i, [_vp]),
+    "pt_set_profiling": (_i, [_i]),
+    "pt_get_kernel_times": (_i, [_vp, _vp]),
     "pt_get_path": (_i, [_vp]),
     "pt_force_general_path": (_i, [_i]),
     "pt_philox_selftest": (_i, [_vp, _vp, _vp, _i]),
@@ -257,6 +259,18 @@ def pt_get_launch_count() -> int:
     n = C.c_uint64()
     _ck(lib().pt_get_launch_count(C.byref(n)))
     return n.value
+
+
+def pt_set_profiling(on):
+    _ck(lib().pt_set_profiling(int(on)))
+
+
+def pt_get_kernel_times():
+    """(ms[4], launches[4]) for the sweep, Houdayer, exchange and measurement kernels since pt_set_profiling."""
+    ms = np.zeros(4, dtype=np.float64)
+    n = np.zeros(4, dtype=np.uint64)
+    _ck(lib().pt_get_kernel_times(_p(ms), _p(n)))
+    return ms, n
 
 
 def pt_get_path() -> int:

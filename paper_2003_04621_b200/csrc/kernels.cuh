@@ -149,6 +149,15 @@ __global__ void k_unpack_spins(Params P)
     }
 }
 
+// counts staged bytes that are not +1/-1 (input validation of pt_set_spins / pt_set_couplings)
+__global__ void k_check_pm1(const int8_t *a, size_t n, int *bad)
+{
+    int local = 0;
+    for (size_t i = (blockIdx.x * (size_t)blockDim.x + threadIdx.x) * 16; i < n; i += (size_t)gridDim.x * blockDim.x * 16)
+        for (size_t j = i; j < i + 16 && j < n; ++j) local += (a[j] != 1 && a[j] != -1);
+    if (local) atomicAdd(bad, local);
+}
+
 __global__ void k_identity_perm(Params P)
 {
     const long total = (long)P.S * 2 * P.T;

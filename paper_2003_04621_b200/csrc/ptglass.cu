@@ -36,6 +36,56 @@ struct Context {
 Context G;
 char g_err[512] = "";
 
+// Optional per-kernel-class timing with CUDA events on the bound stream (pt_set_profiling): every launch of
+// a class is bracketed by two events; pt_get_kernel_times harvests them.  Classes: 0 sweep, 1 Houdayer,
+// 2 exchange, 3 measurement.
+struct Profiler {
+    bool on = false;
+    std::vector<cudaEvent_t> free_events;
+    struct Rec { int cls; cudaEvent_t a, b; };
+    std::vector<Rec> pending;
+    double ms[4] = {0, 0, 0, 0};
+    uint64_t n[4] = {0, 0, 0, 0};
+    cudaEvent_t get()
+    {
+        if (!free_events.empty()) { cudaEvent_t e = free_events.back(); free_events.pop_back(); return e; }
+        cudaEvent_t e = nullptr;
+        cudaEventCreate(&e);
+        return e;
+    }
+    void harvest()
+    {
+        for (const Rec &r : pending) {
+            float t = 0;
+            if (cudaEventSynchronize(r.b) == cudaSuccess && cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) {
+                ms[r.cls] += t;
+                n[r.cls] += 1;
+            }
+            free_events.push_back(r.a);
+            free_events.push_back(r.b);
+        }
+        pending.clear();
+    }
+};
+Profiler PROF;
+
+struct ProfScope {
+    int cls;
+    cudaEvent_t a = nullptr;
+    explicit ProfScope(int c) : cls(c)
+    {
+        if (PROF.on) { a = PROF.get(); cudaEventRecord(a, G.stream); }
+    }
+    ~ProfScope()
+    {
+        if (a) {
+            cudaEvent_t b = PROF.get();
+            cudaEventRecord(b, G.stream);
+            PROF.pending.push_back({cls, a, b});
+        }
+    }
+};
+
 int fail(int code, const char *fmt, ...)
 {
     va_list ap;
@@ -204,6 +254,7 @@ int sweep_group(int T, int W)
 
 cudaError_t launch_sweep(int n)
 {
+    ProfScope prof(0);
     cudaError_t err = cudaSuccess;
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
@@ -222,6 +273,7 @@ cudaError_t launch_sweep(int n)
 
 cudaError_t launch_exchange()
 {
+    ProfScope prof(2);
     const int T = G.P.T;
     const long chains = (long)G.P.S * 2;
     int wpb = 4;
@@ -240,6 +292,7 @@ cudaError_t launch_exchange()
 
 cudaError_t launch_houdayer()
 {
+    ProfScope prof(1);
     cudaError_t err = cudaSuccess;
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
@@ -257,6 +310,7 @@ cudaError_t launch_houdayer()
 
 cudaError_t launch_measure(int32_t *Q, int32_t *QL)
 {
+    ProfScope prof(3);
     cudaError_t err = cudaSuccess;
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
@@ -582,10 +636,17 @@ int pt_get_counters(uint32_t *n_sweep, uint32_t *n_exchange, uint32_t *n_houdaye
     return PT_OK;
 }
 
-static int check_pm1(const int8_t *a, size_t n, const char *what)
+// +-1 validation of the staged int8 input, on the device (k_check_pm1 counts offenders into mismatch[1])
+static int check_pm1_staged(size_t n, const char *what)
 {
-    for (size_t k = 0; k < n; ++k)
-        if (a[k] != 1 && a[k] != -1) return fail(PT_ERR_ARG, "%s[%zu] = %d is not +1/-1", what, k, (int)a[k]);
+    CK(cudaMemsetAsync(G.P.d.mismatch + 1, 0, sizeof(int), G.stream));
+    k_check_pm1<<<grid_for((long)((n + 15) / 16), 256), 256, 0, G.stream>>>(G.P.d.stage, n, G.P.d.mismatch + 1);
+    ++G.launches;
+    CK(cudaGetLastError());
+    int bad = 0;
+    const int rc = d2h(&bad, G.P.d.mismatch + 1, sizeof(int));
+    if (rc) return rc;
+    if (bad) return fail(PT_ERR_ARG, "%s: %d values are not +1/-1", what, bad);
     return PT_OK;
 }
 
@@ -594,9 +655,9 @@ int pt_set_spins(const int8_t *spins)
     NEED_INIT();
     if (!spins) return fail(PT_ERR_ARG, "spins is NULL");
     const size_t n = (size_t)G.P.S * 2 * G.P.T * G.P.N;
-    int rc = check_pm1(spins, n, "spins");
-    if (rc) return rc;
     CK(cudaMemcpyAsync(G.P.d.stage, spins, n, cudaMemcpyHostToDevice, G.stream));
+    int rc = check_pm1_staged(n, "spins");      // rejected input leaves the state unchanged
+    if (rc) return rc;
     if ((rc = pack_spins_and_energy())) return rc;
     CK(cudaStreamSynchronize(G.stream));       // the caller may reuse `spins` as soon as we return
     return PT_OK;
@@ -607,9 +668,9 @@ int pt_set_couplings(const int8_t *J)
     NEED_INIT();
     if (!J) return fail(PT_ERR_ARG, "J is NULL");
     const size_t n = (size_t)G.P.S * G.P.D * G.P.N;
-    int rc = check_pm1(J, n, "J");
-    if (rc) return rc;
     CK(cudaMemcpyAsync(G.P.d.stage, J, n, cudaMemcpyHostToDevice, G.stream));
+    int rc = check_pm1_staged(n, "J");
+    if (rc) return rc;
     if ((rc = pack_couplings())) return rc;
     CK(launch_energy(0));
     CK(cudaStreamSynchronize(G.stream));
@@ -635,6 +696,28 @@ int pt_synchronize(void)
 {
     if (!G.bound) return fail(PT_ERR_STATE, "not bound");
     CK(cudaStreamSynchronize(G.stream));
+    return PT_OK;
+}
+
+int pt_set_profiling(int on)
+{
+    if (!G.bound) return fail(PT_ERR_STATE, "not bound");
+    CK(cudaStreamSynchronize(G.stream));
+    PROF.harvest();
+    PROF.on = on != 0;
+    for (int k = 0; k < 4; ++k) { PROF.ms[k] = 0; PROF.n[k] = 0; }
+    return PT_OK;
+}
+
+int pt_get_kernel_times(double ms[4], uint64_t launches[4])
+{
+    if (!G.bound) return fail(PT_ERR_STATE, "not bound");
+    CK(cudaStreamSynchronize(G.stream));
+    PROF.harvest();
+    for (int k = 0; k < 4; ++k) {
+        if (ms) ms[k] = PROF.ms[k];
+        if (launches) launches[k] = PROF.n[k];
+    }
     return PT_OK;
 }
 
