@@ -276,15 +276,23 @@ __device__ __forceinline__ void accept_bits(uint32_t w, uint32_t step, uint32_t 
 {
 #pragma unroll
     for (int k = 0; k < D; ++k) C[k] = 0;
+    const Round0Shared r0 = philox_round0_shared(step, g, tag, rk);
+    // bits are shifted in from the least significant end, so the sites are visited from bit 31 down to bit 0;
+    // each compare is a subtract whose carry flag is shifted into C by an add-with-carry (2 instructions)
 #pragma unroll
-    for (int b = 0; b < 8; ++b) {
+    for (int b = 7; b >= 0; --b) {
         uint32_t u[4];
-        philox4x32_10(8u * w + (uint32_t)b, step, g, tag, rk, u[0], u[1], u[2], u[3]);
+        philox4x32_10_shared(8u * w + (uint32_t)b, r0, rk, u[0], u[1], u[2], u[3]);
 #pragma unroll
-        for (int j = 0; j < 4; ++j)
+        for (int j = 3; j >= 0; --j)
 #pragma unroll
-            for (int k = 0; k < D; ++k) C[k] |= (uint32_t)(u[j] < thr[k]) << (4 * b + j);
+            for (int k = 0; k < D; ++k)
+                asm("{\n\t.reg .u32 t;\n\tsub.cc.u32 t, %1, %2;\n\taddc.u32 %0, %0, %0;\n\t}"
+                    : "+r"(C[k]) : "r"(u[j]), "r"(thr[k]));
     }
+    // the flag left by sub.cc is the hardware carry of u + ~thr + 1, i.e. (u >= thr): invert once per word
+#pragma unroll
+    for (int k = 0; k < D; ++k) C[k] = ~C[k];
 }
 
 // One work item.  Returns the energy change of the replica caused by this word's flips.

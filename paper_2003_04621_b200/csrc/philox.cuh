@@ -53,4 +53,42 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     o0 = c0; o1 = c1; o2 = c2; o3 = c3;
 }
 
+// The Metropolis stream (domain 3) varies only c0 between the 8 blocks of a work item: c1 = sweep number,
+// c2 = global sample and c3 = tag are shared.  Round 0 therefore splits into a part that is constant per item
+// (Round0Shared: one multiply for many blocks) and one multiply + XOR per block; rounds 1..9 are unchanged.
+struct Round0Shared {
+    uint32_t n0;      // hi(M1*c2) ^ c1 ^ k0[0]
+    uint32_t n1;      // lo(M1*c2)
+    uint32_t x;       // c3 ^ k1[0]
+};
+
+__device__ __forceinline__ Round0Shared philox_round0_shared(uint32_t c1, uint32_t c2, uint32_t c3, const RoundKeys &rk)
+{
+    const unsigned long long p1 = (unsigned long long)PH_M1 * c2;
+    Round0Shared r;
+    r.n0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk.k0[0];
+    r.n1 = (uint32_t)p1;
+    r.x = c3 ^ rk.k1[0];
+    return r;
+}
+
+__device__ __forceinline__ void philox4x32_10_shared(uint32_t c0, const Round0Shared &s, const RoundKeys &rk,
+                                                     uint32_t &o0, uint32_t &o1, uint32_t &o2, uint32_t &o3)
+{
+    const unsigned long long q0 = (unsigned long long)PH_M0 * c0;
+    uint32_t a0 = s.n0, a1 = s.n1, a2 = (uint32_t)(q0 >> 32) ^ s.x, a3 = (uint32_t)q0;
+#pragma unroll
+    for (int r = 1; r < 10; ++r) {
+        const unsigned long long p0 = (unsigned long long)PH_M0 * a0;
+        const unsigned long long p1 = (unsigned long long)PH_M1 * a2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ a1 ^ rk.k0[r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ a3 ^ rk.k1[r];
+        a1 = (uint32_t)p1;
+        a3 = (uint32_t)p0;
+        a0 = n0;
+        a2 = n2;
+    }
+    o0 = a0; o1 = a1; o2 = a2; o3 = a3;
+}
+
 }  // namespace ptg
