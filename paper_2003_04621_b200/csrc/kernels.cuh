@@ -7,6 +7,7 @@
 
 #include "lattice.cuh"
 #include "philox.cuh"
+#include "houdayer.cuh"
 
 namespace ptg {
 
@@ -433,13 +434,14 @@ __global__ void k_exchange(Params P, uint32_t step)
 }
 
 // =========================================================================================================
-// a5  Houdayer cluster exchange (Eq. (10)).  One CTA per (sample, t).
+// a5  Houdayer cluster exchange, GENERAL path (Eq. (10)): any lattice
+// implementation, one CTA per (sample, t), one neighbour step per iteration on the colour layout.
 // The q = -1 cluster is grown on bit maps: C_p |= (OR of the neighbour bits of C_{1-p}) & Neg_p, alternating
 // colours until nothing changes -- the fixed point is exactly the connected component of the seed.
 // =========================================================================================================
 // dynamic smem: Neg[2][W] | Cl[2][W] | scan[blockDim/32 + 2]
 template <class LAT>
-__global__ void __launch_bounds__(128) k_houdayer(LAT lat, Params P, uint32_t step)
+__global__ void __launch_bounds__(128) k_houdayer_gen(LAT lat, Params P, uint32_t step)
 {
     constexpr int D = LAT::D;
     extern __shared__ uint32_t hsm[];
@@ -562,6 +564,32 @@ __global__ void __launch_bounds__(128) k_houdayer(LAT lat, Params P, uint32_t st
         P.d.E[repB] -= dl;
         P.d.last[(size_t)s * P.T + t] = (uint32_t)sz;
         P.d.cum[(size_t)s * P.T + t] += (unsigned long long)sz;
+    }
+}
+
+// =========================================================================================================
+// a5  Houdayer cluster exchange, FAST path: one warp per (sample, t) pair (houdayer.cuh).
+// grid: ceil(S*T / warps per CTA); dynamic smem: 4W words per warp.
+// =========================================================================================================
+template <class LAT>
+__global__ void __launch_bounds__(256) k_houdayer(LAT lat, Params P, uint32_t step)
+{
+    extern __shared__ uint32_t hsm[];
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+    const long pair = (long)blockIdx.x * wpb + wib;
+    if (pair >= (long)P.S * P.T) return;
+    const int s = (int)(pair / P.T), t = (int)(pair - (long)s * P.T);
+    const size_t repA = rep_index(P, s, 0, P.d.sot[rep_index(P, s, 0, t)]);
+    const size_t repB = rep_index(P, s, 1, P.d.sot[rep_index(P, s, 1, t)]);
+    uint32_t u, o1, o2, o3;
+    philox4x32_10(0u, step, P.g0 + (uint32_t)s, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
+    int delta;
+    const int size = houdayer_pair(lat, spin_words(P, repA, 0), spin_words(P, repA, 1), spin_words(P, repB, 0),
+                                   spin_words(P, repB, 1), J_words(P, s, 0, 0), hsm + (size_t)wib * 4 * LAT::W, u, lane, delta);
+    if (lane == 0) {
+        if (delta) { P.d.E[repA] += delta; P.d.E[repB] -= delta; }
+        P.d.last[pair] = (uint32_t)size;
+        P.d.cum[pair] += (unsigned long long)size;
     }
 }
 

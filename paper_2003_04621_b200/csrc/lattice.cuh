@@ -90,6 +90,7 @@ template <int D_, int LOG2L>
 struct FastLat {
     static constexpr int D = D_;
     static constexpr bool kFast = true;
+    static constexpr int kLog2L = LOG2L;
     static constexpr int L = 1 << LOG2L;
     static constexpr int Lh = L / 2;
     static constexpr int N = (D_ == 2) ? L * L : L * L * L;

@@ -296,12 +296,23 @@ cudaError_t launch_houdayer()
     cudaError_t err = cudaSuccess;
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
-        const int threads = 128;
-        const size_t smem = ((size_t)4 * G.P.W + 2 * (threads / 32) + 2) * 4;
-        err = allow_smem(k_houdayer<LAT>, smem);
-        if (err != cudaSuccess) return;
-        dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
-        k_houdayer<LAT><<<grid, threads, smem, G.stream>>>(lat, G.P, G.n_houdayer);
+        if constexpr (LAT::kFast) {
+            // one warp per pair; 4W words of shared memory per warp
+            int wpb = 8;
+            while (wpb > 1 && (size_t)wpb * 4 * G.P.W * 4 > 96 * 1024) wpb >>= 1;
+            const size_t smem = (size_t)wpb * 4 * G.P.W * 4;
+            err = allow_smem(k_houdayer<LAT>, smem);
+            if (err != cudaSuccess) return;
+            const long pairs = (long)G.P.S * G.P.T;
+            k_houdayer<LAT><<<(unsigned)((pairs + wpb - 1) / wpb), wpb * 32, smem, G.stream>>>(lat, G.P, G.n_houdayer);
+        } else {
+            const int threads = 128;
+            const size_t smem = ((size_t)4 * G.P.W + 2 * (threads / 32) + 2) * 4;
+            err = allow_smem(k_houdayer_gen<LAT>, smem);
+            if (err != cudaSuccess) return;
+            dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
+            k_houdayer_gen<LAT><<<grid, threads, smem, G.stream>>>(lat, G.P, G.n_houdayer);
+        }
         ++G.launches;
         err = cudaGetLastError();
     });
