@@ -269,6 +269,30 @@ __device__ __forceinline__ Classes<D> classify(const uint32_t un[2 * D])
     return c;
 }
 
+// C |= BIT iff u < thr: one unsigned compare + one predicated OR of an immediate.  Both issue on the alu pipe and
+// leave the fma pipe, which IMAD.WIDE saturates, to Philox (an add-with-carry chain compiles to IMAD.X there).
+template <uint32_t BIT>
+__device__ __forceinline__ void or_if_less(uint32_t &C, uint32_t u, uint32_t thr)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %1, %2;\n\t@p or.b32 %0, %0, %3;\n\t}" : "+r"(C) : "r"(u), "r"(thr), "n"(BIT));
+}
+
+// Philox block B of word w: accept bits of sites 4B..4B+3
+template <int D, int B>
+__device__ __forceinline__ void accept_block(uint32_t w, const Round0Shared &r0, const RoundKeys &rk, const uint32_t thr[D],
+                                             uint32_t C[D])
+{
+    uint32_t u0, u1, u2, u3;
+    philox4x32_10_shared(8u * w + (uint32_t)B, r0, rk, u0, u1, u2, u3);
+#pragma unroll
+    for (int k = 0; k < D; ++k) {
+        or_if_less<1u << (4 * B + 0)>(C[k], u0, thr[k]);
+        or_if_less<1u << (4 * B + 1)>(C[k], u1, thr[k]);
+        or_if_less<1u << (4 * B + 2)>(C[k], u2, thr[k]);
+        or_if_less<1u << (4 * B + 3)>(C[k], u3, thr[k]);
+    }
+}
+
 // Accept bits for the 32 sites of word w: bit j of C[k-1] = (u_j < thr[k-1]), u_j = word (j & 3) of Philox block
 // 8w + (j >> 2) of the Metropolis stream (domain 3).
 template <int D>
@@ -278,22 +302,14 @@ __device__ __forceinline__ void accept_bits(uint32_t w, uint32_t step, uint32_t 
 #pragma unroll
     for (int k = 0; k < D; ++k) C[k] = 0;
     const Round0Shared r0 = philox_round0_shared(step, g, tag, rk);
-    // bits are shifted in from the least significant end, so the sites are visited from bit 31 down to bit 0;
-    // each compare is a subtract whose carry flag is shifted into C by an add-with-carry (2 instructions)
-#pragma unroll
-    for (int b = 7; b >= 0; --b) {
-        uint32_t u[4];
-        philox4x32_10_shared(8u * w + (uint32_t)b, r0, rk, u[0], u[1], u[2], u[3]);
-#pragma unroll
-        for (int j = 3; j >= 0; --j)
-#pragma unroll
-            for (int k = 0; k < D; ++k)
-                asm("{\n\t.reg .u32 t;\n\tsub.cc.u32 t, %1, %2;\n\taddc.u32 %0, %0, %0;\n\t}"
-                    : "+r"(C[k]) : "r"(u[j]), "r"(thr[k]));
-    }
-    // the flag left by sub.cc is the hardware carry of u + ~thr + 1, i.e. (u >= thr): invert once per word
-#pragma unroll
-    for (int k = 0; k < D; ++k) C[k] = ~C[k];
+    accept_block<D, 0>(w, r0, rk, thr, C);
+    accept_block<D, 1>(w, r0, rk, thr, C);
+    accept_block<D, 2>(w, r0, rk, thr, C);
+    accept_block<D, 3>(w, r0, rk, thr, C);
+    accept_block<D, 4>(w, r0, rk, thr, C);
+    accept_block<D, 5>(w, r0, rk, thr, C);
+    accept_block<D, 6>(w, r0, rk, thr, C);
+    accept_block<D, 7>(w, r0, rk, thr, C);
 }
 
 // One work item.  Returns the energy change of the replica caused by this word's flips.
@@ -322,7 +338,7 @@ __device__ __forceinline__ int update_word(const LAT &lat, uint32_t *Sown, const
 
 // grid: (2T/R groups, S).  dynamic smem: [2][2D][W] couplings | [R][2][W] spins | [R][4] thresholds | [R] dE
 template <class LAT>
-__global__ void __launch_bounds__(256) k_sweep(LAT lat, Params P, int R, uint32_t step0, int n_sweeps)
+__global__ void __launch_bounds__(128, 7) k_sweep(LAT lat, Params P, int R, uint32_t step0, int n_sweeps)
 {
     constexpr int D = LAT::D;
     extern __shared__ uint32_t smem[];

@@ -243,12 +243,12 @@ cudaError_t launch_energy(int mode)
     return err;
 }
 
-// replicas per CTA of the sweep kernel: the largest divisor of 2T with R*W <= 1024 work items
+// replicas per CTA of the sweep kernel (128 threads): the largest divisor of 2T with R*W <= 512 work items
 int sweep_group(int T, int W)
 {
     int best = 1;
     for (int R = 1; R <= 2 * T; ++R)
-        if ((2 * T) % R == 0 && (long)R * W <= 1024) best = R;
+        if ((2 * T) % R == 0 && (long)R * W <= 512) best = R;
     return best;
 }
 
@@ -264,7 +264,7 @@ cudaError_t launch_sweep(int n)
         err = allow_smem(k_sweep<LAT>, smem);
         if (err != cudaSuccess) return;
         dim3 grid((unsigned)(2 * G.P.T / R), (unsigned)G.P.S);
-        k_sweep<LAT><<<grid, 256, smem, G.stream>>>(lat, G.P, R, G.n_sweep, n);
+        k_sweep<LAT><<<grid, 128, smem, G.stream>>>(lat, G.P, R, G.n_sweep, n);
         ++G.launches;
         err = cudaGetLastError();
     });
