@@ -89,8 +89,14 @@ int pt_exchange(void);
 int houdayer_step(void);
 
 /* Fused Monte Carlo steps in the paper's order (R15): n_mcs x [ pt_sweep(n_metro);
- * houdayer_step() if do_houdayer; pt_exchange() if do_exchange ].  Bit-identical to the separate calls. */
+ * houdayer_step() if do_houdayer; pt_exchange() if do_exchange ].  Bit-identical to the separate calls.
+ * Where a sample's whole state fits in shared memory this is ONE kernel launch that keeps each
+ * sample resident in one CTA for all n_mcs steps; otherwise it issues the separate kernels in order. */
 int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange);
+/* mode -1 (default): pt_mcs uses the fused kernel where eligible; 0: always the separate kernels (tests, profiling).
+ * pt_get_fused: 1 if pt_mcs of the bound problem runs fused. */
+int pt_set_fused(int mode);
+int pt_get_fused(int *fused);
 
 /* ---- observables: all integer, indexed by TEMPERATURE index t ------------------------------------------- */
 
@@ -123,11 +129,11 @@ int pt_recompute_energy(int32_t *E_slot_order /* [S][2][T] or NULL */, int *mism
 
 int pt_synchronize(void);                          /* cudaStreamSynchronize on the bound stream */
 int pt_get_launch_count(uint64_t *n_launches);     /* kernels launched by this library since pt_bind */
-/* Per-kernel-class device times: when on, every launch of the sweep (class 0), Houdayer (1), exchange (2) and
- * measurement (3) kernels is bracketed by CUDA events on the bound stream.  pt_set_profiling resets the sums;
+/* Per-kernel-class device times: when on, every launch of the sweep (class 0), Houdayer (1), exchange (2),
+ * measurement (3) and fused-MCS (4) kernels is bracketed by CUDA events on the bound stream.  pt_set_profiling resets the sums;
  * pt_get_kernel_times synchronises and returns the summed milliseconds and launch counts since then. */
 int pt_set_profiling(int on);
-int pt_get_kernel_times(double ms[4], uint64_t launches[4]);
+int pt_get_kernel_times(double ms[5], uint64_t launches[5]);
 /* Which code path the bound problem uses: 1 = word-parallel kernels specialised for L a power of two >= 8,
  * 0 = general-L kernels.  force = -1 leaves the choice to the library, 0 forces the general path (tests). */
 int pt_get_path(int *fast);

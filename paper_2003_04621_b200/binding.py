@@ -29,6 +29,8 @@ SYMBOLS = {
     "pt_exchange": (_i, []),
     "houdayer_step": (_i, []),
     "pt_mcs": (_i, [_i, _i, _i, _i]),
+    "pt_set_fused": (_i, [_i]),
+    "pt_get_fused": (_i, [_vp]),
     "pt_get_energy": (_i, [_vp]),
     "pt_measure_overlap": (_i, [_vp, _vp]),
     "pt_get_swap_counts": (_i, [_vp, _vp]),
@@ -163,6 +165,16 @@ def pt_mcs(n_mcs, n_metro=1, do_houdayer=False, do_exchange=True):
     _ck(lib().pt_mcs(n_mcs, n_metro, int(do_houdayer), int(do_exchange)))
 
 
+def pt_set_fused(mode):
+    _ck(lib().pt_set_fused(mode))
+
+
+def pt_get_fused() -> int:
+    f = C.c_int()
+    _ck(lib().pt_get_fused(C.byref(f)))
+    return f.value
+
+
 def pt_get_energy(out=None):
     E = np.empty((_shape["S"], 2, _shape["T"]), dtype=np.int32) if out is None else out
     _ck(lib().pt_get_energy(_p(E)))
@@ -266,9 +278,10 @@ def pt_set_profiling(on):
 
 
 def pt_get_kernel_times():
-    """(ms[4], launches[4]) for the sweep, Houdayer, exchange and measurement kernels since pt_set_profiling."""
-    ms = np.zeros(4, dtype=np.float64)
-    n = np.zeros(4, dtype=np.uint64)
+    """(ms[5], launches[5]) for the sweep, Houdayer, exchange, measurement and fused-MCS kernels since
+    pt_set_profiling."""
+    ms = np.zeros(5, dtype=np.float64)
+    n = np.zeros(5, dtype=np.uint64)
     _ck(lib().pt_get_kernel_times(_p(ms), _p(n)))
     return ms, n
 

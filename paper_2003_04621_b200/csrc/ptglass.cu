@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "kernels.cuh"
+#include "mcs.cuh"
 
 using namespace ptg;
 
@@ -24,6 +25,7 @@ struct Context {
     cudaStream_t stream = nullptr;
     bool bound = false, inited = false;
     int force_general = -1;
+    int fused_mode = -1;        // -1: fused pt_mcs where eligible, 0: always separate launches
     bool fast = false;
     Params P{};
     std::vector<double> betas;
@@ -38,14 +40,14 @@ char g_err[512] = "";
 
 // Optional per-kernel-class timing with CUDA events on the bound stream (pt_set_profiling): every launch of
 // a class is bracketed by two events; pt_get_kernel_times harvests them.  Classes: 0 sweep, 1 Houdayer,
-// 2 exchange, 3 measurement.
+// 2 exchange, 3 measurement, 4 fused MCS.
 struct Profiler {
     bool on = false;
     std::vector<cudaEvent_t> free_events;
     struct Rec { int cls; cudaEvent_t a, b; };
     std::vector<Rec> pending;
-    double ms[4] = {0, 0, 0, 0};
-    uint64_t n[4] = {0, 0, 0, 0};
+    double ms[5] = {0, 0, 0, 0, 0};
+    uint64_t n[5] = {0, 0, 0, 0, 0};
     cudaEvent_t get()
     {
         if (!free_events.empty()) { cudaEvent_t e = free_events.back(); free_events.pop_back(); return e; }
@@ -334,6 +336,41 @@ cudaError_t launch_measure(int32_t *Q, int32_t *QL)
     return err;
 }
 
+// Fused MCS (mcs.cuh): one CTA per sample, 128 threads, up to 7 CTAs per SM.  Eligible on the fast path when the
+// sample's state fits in shared memory with at least 4 CTAs per SM (else the separate kernels are faster).
+constexpr int kMcsThreads = 128, kMcsMinBlocks = 7;
+
+bool mcs_fused_eligible(size_t *smem_out)
+{
+    if (!G.fast || G.fused_mode == 0) return false;
+    const McsSmem lay(G.P.D, G.P.W, G.P.T, kMcsThreads / 32);
+    const size_t smem = (size_t)lay.words * 4;
+    if (smem_out) *smem_out = smem;
+    return (smem + 1024) * 4 <= 227 * 1024;
+}
+
+cudaError_t launch_mcs(const McsArgs &a)
+{
+    ProfScope prof(4);
+    cudaError_t err = cudaSuccess;
+    with_lattice([&](auto lat) {
+        using LAT = decltype(lat);
+        if constexpr (LAT::kFast) {
+            size_t smem = 0;
+            mcs_fused_eligible(&smem);
+            auto kern = k_mcs<LAT, kMcsThreads, kMcsMinBlocks>;
+            err = allow_smem(kern, smem);
+            if (err != cudaSuccess) return;
+            kern<<<(unsigned)G.P.S, kMcsThreads, smem, G.stream>>>(lat, G.P, a);
+            ++G.launches;
+            err = cudaGetLastError();
+        } else {
+            err = cudaErrorInvalidValue;
+        }
+    });
+    return err;
+}
+
 int d2h(void *dst, const void *src, size_t bytes)
 {
     CK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, G.stream));
@@ -520,11 +557,34 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
         (do_exchange && (uint64_t)G.n_exchange + M > 4294967295ull) ||
         (do_houdayer && (uint64_t)G.n_houdayer + M > 4294967295ull))
         return fail(PT_ERR_OVERFLOW, "a step counter would overflow");
+    if (n_mcs == 0 || (n_metro == 0 && !do_houdayer && !do_exchange)) return PT_OK;
+    if (mcs_fused_eligible(nullptr)) {
+        const McsArgs a{n_mcs, n_metro, do_houdayer ? 1 : 0, do_exchange ? 1 : 0, G.n_sweep, G.n_houdayer, G.n_exchange};
+        CK(launch_mcs(a));
+        G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
+        if (do_houdayer) G.n_houdayer += (uint32_t)M;
+        if (do_exchange) G.n_exchange += (uint32_t)M;
+        return PT_OK;
+    }
     for (int m = 0; m < n_mcs; ++m) {
         if (n_metro > 0) { CK(launch_sweep(n_metro)); G.n_sweep += (uint32_t)n_metro; }
         if (do_houdayer) { CK(launch_houdayer()); G.n_houdayer += 1; }
         if (do_exchange) { CK(launch_exchange()); G.n_exchange += 1; }
     }
+    return PT_OK;
+}
+
+int pt_set_fused(int mode)
+{
+    if (mode != -1 && mode != 0) return fail(PT_ERR_ARG, "mode must be -1 (fused where eligible) or 0 (separate launches)");
+    G.fused_mode = mode;
+    return PT_OK;
+}
+
+int pt_get_fused(int *fused)
+{
+    NEED_INIT();
+    if (fused) *fused = mcs_fused_eligible(nullptr) ? 1 : 0;
     return PT_OK;
 }
 
@@ -716,16 +776,16 @@ int pt_set_profiling(int on)
     CK(cudaStreamSynchronize(G.stream));
     PROF.harvest();
     PROF.on = on != 0;
-    for (int k = 0; k < 4; ++k) { PROF.ms[k] = 0; PROF.n[k] = 0; }
+    for (int k = 0; k < 5; ++k) { PROF.ms[k] = 0; PROF.n[k] = 0; }
     return PT_OK;
 }
 
-int pt_get_kernel_times(double ms[4], uint64_t launches[4])
+int pt_get_kernel_times(double ms[5], uint64_t launches[5])
 {
     if (!G.bound) return fail(PT_ERR_STATE, "not bound");
     CK(cudaStreamSynchronize(G.stream));
     PROF.harvest();
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < 5; ++k) {
         if (ms) ms[k] = PROF.ms[k];
         if (launches) launches[k] = PROF.n[k];
     }
