@@ -271,30 +271,44 @@ def main():
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (Metropolis sweep): INT32 issue, live CUDA-event kernel times
+    # ---- roofline of the dominant kernel of the timed region (INT32 issue; live CUDA-event launch times)
     peaks, peaks_kind = measured_peaks()
     f_ghz = (clocks["sm_mhz"] or peaks.get("sm_max_mhz", 1965.0)) / 1e3 if clocks else 1.965
-    sweep_ms = kms[0] / max(int(kn[0]), 1)
-    flips_per_sweep_launch = w.flips_per_sweep()
-    sweep_flips_ns = flips_per_sweep_launch / (sweep_ms * 1e6) if sweep_ms > 0 else 0.0
+    names = ["k_sweep", "k_houdayer", "k_exchange", "k_measure", "k_mcs"]
+    dom = int(np.argmax(kms))
+    if dom not in (0, 4):          # the roofline is quoted for the kernel that does the Metropolis sweeps
+        dom = 4 if kn[4] > 0 else 0
+    mcs_per_launch = 1 if dom == 0 else (w.measure_every if n_meas else a.mcs_per_step)
+    dom_ms = kms[dom] / max(int(kn[dom]), 1)
+    flips_per_launch = w.flips_per_sweep() * mcs_per_launch
+    dom_flips_ns = flips_per_launch / (dom_ms * 1e6) if dom_ms > 0 else 0.0
     A = ALGO_OPS_PER_FLIP[w.d]
     peak_ops = SM_COUNT * INT32_LANES_PER_SM_CLK * (peaks.get("sm_max_mhz", 1965.0) / 1e3)
     philox_ops, _ = B.pt_microbench(4, 8, 1000, device=dev)     # measured live: Philox-only ceiling
     roofline = {
-        "bound": "alu", "kernel": "k_sweep", "achieved": A * sweep_flips_ns, "peak": peak_ops, "unit": "Gop/s (INT32 thread-ops)",
-        "frac": A * sweep_flips_ns / peak_ops, "traffic": None,
-        "peak_how": "derived: 148 SMs x 128 INT32 lanes/clk (fma+alu pipes) x %.3f GHz max SM clock; A = %d algorithmic ops/flip" % (
-            peaks.get("sm_max_mhz", 1965.0) / 1e3, A),
-        "sweep_flips_per_ns": sweep_flips_ns, "sweep_ms_per_launch": sweep_ms, "sweep_launches": int(kn[0]),
+        "bound": "alu", "kernel": names[dom], "achieved": A * dom_flips_ns, "peak": peak_ops,
+        "unit": "Gop/s (INT32 thread-ops)", "frac": A * dom_flips_ns / peak_ops, "traffic": None,
+        "peak_how": "derived: 148 SMs x 128 INT32 lanes/clk (fma+alu pipes) x %.3f GHz max SM clock; A = %d algorithmic "
+                    "ops/flip (Philox 10 + field 2d + decide 6); a %s launch = %d MCS = %d attempted flips" % (
+                        peaks.get("sm_max_mhz", 1965.0) / 1e3, A, names[dom], mcs_per_launch, flips_per_launch),
+        "flips_per_ns": dom_flips_ns, "ms_per_launch": dom_ms, "launches": int(kn[dom]),
         "philox_only_flips_per_ns": philox_ops / 10.0,
-        "frac_of_philox_only": sweep_flips_ns / (philox_ops / 10.0) if philox_ops > 0 else None,
-        "hbm": {"algorithmic_bytes_per_flip": 0.25, "achieved_gbs": 0.25 * sweep_flips_ns,
+        "hbm": {"algorithmic_bytes_per_flip": 0.25 / mcs_per_launch, "achieved_gbs": 0.25 / mcs_per_launch * dom_flips_ns,
                 "peak_gbs": peaks.get("hbm_gbs"), "peak_kind": peaks_kind,
-                "frac": 0.25 * sweep_flips_ns / peaks.get("hbm_gbs", 6650.0)},
-        "kernel_ms_share": {"sweep": kms[0], "houdayer": kms[1], "exchange": kms[2], "measure": kms[3],
-                            "step_total": ms_total},
+                "frac": 0.25 / mcs_per_launch * dom_flips_ns / peaks.get("hbm_gbs", 6650.0)},
+        "kernel_ms": {n: float(kms[i]) for i, n in enumerate(names)}, "step_total_ms": ms_total,
         "clock_ghz_during_run": f_ghz,
     }
+    # the Metropolis sweeps alone (a1-a3; Eq. (11) normalisation), same state, after the timed region
+    B.pt_set_profiling(True)
+    for _ in range(5):
+        B.pt_sweep(a.mcs_per_step)
+    sms, sn = B.pt_get_kernel_times()
+    B.pt_set_profiling(False)
+    so = w.flips_per_sweep() * a.mcs_per_step / (sms[0] / max(int(sn[0]), 1) * 1e6)
+    roofline["sweep_only"] = {"kernel": "k_sweep", "flips_per_ns": so, "frac": A * so / peak_ops,
+                              "what": "pt_sweep(%d) launches, no Houdayer / exchange" % a.mcs_per_step}
+    assert B.pt_recompute_energy()[1] == 0
 
     cpu = None
     if not a.no_cpu_baseline:

@@ -1,0 +1,116 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (one pt_mcs call per step,
+whole S on the device): C2-C5.  The oracle cannot run a whole config, so
+  (i)  sampled samples g in {0, 1, S/2, S-1} are recomputed one by one by the oracle through `sample_offset`
+       (every sample is a pure function of (seed, g), pin P8) and compared bit for bit, and
+  (ii) size-independent invariants are checked on ALL samples: tracked E == recomputed E, the two maps are inverse
+       permutations, attempts == number of passes, accepts <= attempts, Houdayer conserves E1+E2 and Q.
+Run on the B200 box with `-m gpu`."""
+import numpy as np
+import pytest
+
+from oracle import ref
+from paper_2003_04621_b200 import binding as B
+from paper_2003_04621_b200 import build as build_mod
+from paper_2003_04621_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    build_mod.build()
+    yield
+    B.pt_free()
+
+
+def run_like_bench(w, n_mcs):
+    """The step of bench.py: pt_mcs in one call (or in chunks of measure_every with the measurement between)."""
+    recs = []
+    if w.measure_every:
+        for _ in range(n_mcs // w.measure_every):
+            B.pt_mcs(w.measure_every, 1, w.houdayer, True)
+            recs.append(B.pt_measure_overlap())
+    else:
+        B.pt_mcs(n_mcs, 1, w.houdayer, True)
+    return recs
+
+
+def oracle_sample(w, g, n_mcs):
+    o = ref.Oracle(w.L, w.d, 1, w.T, w.betas(), wl.SEED, g)
+    recs = []
+    for m in range(1, n_mcs + 1):
+        o.mcs(1, 1, w.houdayer, True)
+        if w.measure_every and m % w.measure_every == 0:
+            recs.append(o.measure_overlap())
+    return o, recs
+
+
+@pytest.mark.parametrize("name,n_mcs,n_check", [("C2", 100, 4), ("C3", 100, 4), ("C4", 40, 4), ("C5", 20, 3)])
+def test_full_size_sampled_parity_and_invariants(name, n_mcs, n_check):
+    w = wl.CONFIGS[name]
+    B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED)
+    recs = run_like_bench(w, n_mcs)
+    st = B.state()
+    Q, QL = B.pt_measure_overlap()
+
+    # (ii) invariants on every sample
+    assert B.pt_recompute_energy()[1] == 0
+    tos, sot = st["temp_of_slot"], st["slot_of_temp"]
+    ar = np.broadcast_to(np.arange(w.T), tos.shape)
+    assert np.array_equal(np.take_along_axis(tos, sot, axis=2), ar)
+    assert np.array_equal(np.take_along_axis(sot, tos, axis=2), ar)
+    assert (st["attempts"] == n_mcs).all() and (st["accepts"] <= st["attempts"]).all()
+    assert tuple(st["counters"]) == (n_mcs, n_mcs, n_mcs if w.houdayer else 0)
+    assert ((Q - w.N) % 2 == 0).all() and (abs(Q) <= w.N).all()
+    assert ((QL - w.d * w.N) % 2 == 0).all() and (abs(QL) <= w.d * w.N).all()
+    if w.houdayer:
+        assert (st["last_size"] <= w.N).all() and (st["cum_size"] >= st["last_size"]).all()
+
+    # (i) sampled samples against the oracle
+    for g in [0, 1, w.S // 2, w.S - 1][:n_check]:
+        o, orecs = oracle_sample(w, g, n_mcs)
+        a = o.state()
+        for k in a:
+            if k == "counters":
+                continue
+            assert np.array_equal(a[k][0], st[k][g]), "%s sample %d: %s differs" % (name, g, k)
+        Qo, QLo = o.measure_overlap()
+        assert np.array_equal(Qo[0], Q[g]) and np.array_equal(QLo[0], QL[g])
+        for (qa, qla), (qb, qlb) in zip(orecs, recs):
+            assert np.array_equal(qa[0], qb[g]) and np.array_equal(qla[0], qlb[g])
+        o.close()
+
+
+@pytest.mark.parametrize("name", ["C2", "C5"])
+def test_full_size_houdayer_conserves_pair_energy_and_overlap(name):
+    w = wl.CONFIGS[name]
+    B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED)
+    B.pt_mcs(5, 1, True, True)
+    E0 = B.pt_get_energy().astype(np.int64)
+    Q0, QL0 = B.pt_measure_overlap()
+    B.houdayer_step()
+    E1 = B.pt_get_energy().astype(np.int64)
+    Q1, QL1 = B.pt_measure_overlap()
+    assert np.array_equal(E0.sum(axis=1), E1.sum(axis=1))          # E1 + E2 per (sample, temperature)
+    assert np.array_equal(Q0, Q1) and np.array_equal(QL0, QL1)
+    assert B.pt_recompute_energy()[1] == 0
+    assert (B.pt_get_cluster_sizes()[0] > 0).any()
+
+
+def test_fused_and_separate_launches_agree_at_full_size():
+    """pt_mcs fused (one CTA per sample, state resident in shared memory) == the three separate kernels."""
+    w = wl.C2
+    B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED)
+    assert B.pt_get_fused() == 1
+    B.pt_mcs(12, 1, True, True)
+    fused = B.state()
+    try:
+        B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED)
+        B.pt_set_fused(0)
+        assert B.pt_get_fused() == 0
+        B.pt_mcs(12, 1, True, True)
+        sep = B.state()
+    finally:
+        B.pt_set_fused(-1)
+    for k in fused:
+        assert np.array_equal(fused[k], sep[k]), k
