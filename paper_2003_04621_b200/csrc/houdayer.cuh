@@ -106,28 +106,33 @@ struct NatLat {
         h1 = (od & ~m1) | (ev & m1);
     }
 
-    // OR of the cluster bits of the 2D neighbours of the 32 sites of word n (cur = Cl[n])
-    __device__ __forceinline__ static uint32_t neighbour_union(const uint32_t *Cl, int n, uint32_t cur)
+    // OR of the cluster bits of the 2D neighbours of the 32 sites of word n (cur = Cl[n]); ld(i) returns Cl[i]
+    template <class F>
+    __device__ __forceinline__ static uint32_t neighbour_union_f(F ld, int n, uint32_t cur)
     {
         uint32_t u;
         if constexpr (kSmall) {
             const int base = (D_ == 3) ? (n / PWN) * PWN : 0, j = n - base;
             u = ((cur << 1) & ~SEG_LSB) | ((cur >> (L - 1)) & SEG_LSB) | ((cur >> 1) & ~SEG_MSB) | ((cur << (L - 1)) & SEG_MSB);
-            const uint32_t nxt = Cl[base + ((j + 1) & (PWN - 1))], prv = Cl[base + ((j - 1) & (PWN - 1))];
+            const uint32_t nxt = ld(base + ((j + 1) & (PWN - 1))), prv = ld(base + ((j - 1) & (PWN - 1)));
             u |= __funnelshift_r(cur, nxt, L) | __funnelshift_l(prv, cur, L);
         } else {
             const int row = n / WR, j = n - row * WR;
             if constexpr (WR == 1) {
                 u = __funnelshift_l(cur, cur, 1) | __funnelshift_r(cur, cur, 1);
             } else {
-                const uint32_t pw = Cl[row * WR + ((j - 1) & (WR - 1))], nw = Cl[row * WR + ((j + 1) & (WR - 1))];
+                const uint32_t pw = ld(row * WR + ((j - 1) & (WR - 1))), nw = ld(row * WR + ((j + 1) & (WR - 1)));
                 u = __funnelshift_l(pw, cur, 1) | __funnelshift_r(cur, nw, 1);
             }
             const int base = (D_ == 3) ? (n / PWN) * PWN : 0, jj = n - base;
-            u |= Cl[base + ((jj + WR) & (PWN - 1))] | Cl[base + ((jj - WR) & (PWN - 1))];
+            u |= ld(base + ((jj + WR) & (PWN - 1))) | ld(base + ((jj - WR) & (PWN - 1)));
         }
-        if constexpr (D_ == 3) u |= Cl[(n + PWN) & (NW - 1)] | Cl[(n - PWN) & (NW - 1)];
+        if constexpr (D_ == 3) u |= ld((n + PWN) & (NW - 1)) | ld((n - PWN) & (NW - 1));
         return u;
+    }
+    __device__ __forceinline__ static uint32_t neighbour_union(const uint32_t *Cl, int n, uint32_t cur)
+    {
+        return neighbour_union_f([Cl](int i) { return Cl[i]; }, n, cur);
     }
 
     // upward fill of the runs of `neg` (within row segments) that contain a bit of `seeds` (seeds subset of neg)

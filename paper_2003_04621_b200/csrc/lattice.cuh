@@ -111,6 +111,13 @@ struct FastLat {
 
     __device__ __forceinline__ void gather(const uint32_t *O, int w, int p, uint32_t nb[2 * D_]) const
     {
+        gather_f([O](int i) { return O[i]; }, w, p, nb);
+    }
+
+    // same, the other colour's words read through ld(i) (strided or padded layouts)
+    template <class F>
+    __device__ __forceinline__ void gather_f(F ld, int w, int p, uint32_t nb[2 * D_]) const
+    {
         if constexpr (Lh < 32) {
             constexpr int PW = (L * Lh) / 32;                       // words per xy-plane (>= 1)
             constexpr uint32_t SEG_LSB = rep_mask(1u, Lh);          // bit 0 of every row segment
@@ -118,39 +125,39 @@ struct FastLat {
             constexpr uint32_t ODD = rep_mask(((1u << Lh) - 1u) << Lh, 2 * Lh);   // bits in rows of odd y
             const int z = (D_ == 3) ? (w / PW) : 0;
             const int base = z * PW, j = w - base;
-            const uint32_t same = O[w];
+            const uint32_t same = ld(w);
             const uint32_t rl = ((same << 1) & ~SEG_LSB) | ((same >> (Lh - 1)) & SEG_LSB);   // bit k <- k-1
             const uint32_t rr = ((same >> 1) & ~SEG_MSB) | ((same << (Lh - 1)) & SEG_MSB);   // bit k <- k+1
             const uint32_t x0m = ((p + z) & 1) ? ~ODD : ODD;        // sites with odd x
             nb[0] = (same & ~x0m) | (rr & x0m);                     // +x
             nb[1] = (rl & ~x0m) | (same & x0m);                     // -x
-            const uint32_t wn = O[base + ((j + 1) & (PW - 1))];
-            const uint32_t wp = O[base + ((j - 1) & (PW - 1))];
+            const uint32_t wn = ld(base + ((j + 1) & (PW - 1)));
+            const uint32_t wp = ld(base + ((j - 1) & (PW - 1)));
             nb[2] = __funnelshift_r(same, wn, Lh);                  // +y: bit b <- bit b + Lh (cyclic in plane)
             nb[3] = __funnelshift_l(wp, same, Lh);                  // -y
             if constexpr (D_ == 3) {
-                nb[4] = O[(w + PW) & (W - 1)];
-                nb[5] = O[(w - PW) & (W - 1)];
+                nb[4] = ld((w + PW) & (W - 1));
+                nb[5] = ld((w - PW) & (W - 1));
             }
         } else {
             constexpr int WR = Lh / 32;                             // words per row
             constexpr int PW = L * WR;                              // words per plane
             const int row = w / WR, j = w - row * WR;
             const int y = row & (L - 1), z = row >> LOG2L;
-            const uint32_t same = O[w];
+            const uint32_t same = ld(w);
             if ((p + y + z) & 1) {
                 nb[1] = same;
-                nb[0] = __funnelshift_r(same, O[row * WR + ((j + 1) & (WR - 1))], 1);
+                nb[0] = __funnelshift_r(same, ld(row * WR + ((j + 1) & (WR - 1))), 1);
             } else {
                 nb[0] = same;
-                nb[1] = __funnelshift_l(O[row * WR + ((j - 1) & (WR - 1))], same, 1);
+                nb[1] = __funnelshift_l(ld(row * WR + ((j - 1) & (WR - 1))), same, 1);
             }
             const int base = z * PW, jj = w - base;
-            nb[2] = O[base + ((jj + WR) & (PW - 1))];
-            nb[3] = O[base + ((jj - WR) & (PW - 1))];
+            nb[2] = ld(base + ((jj + WR) & (PW - 1)));
+            nb[3] = ld(base + ((jj - WR) & (PW - 1)));
             if constexpr (D_ == 3) {
-                nb[4] = O[(w + PW) & (W - 1)];
-                nb[5] = O[(w - PW) & (W - 1)];
+                nb[4] = ld((w + PW) & (W - 1));
+                nb[5] = ld((w - PW) & (W - 1));
             }
         }
     }

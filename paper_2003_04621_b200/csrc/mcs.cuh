@@ -2,10 +2,13 @@
 // its 2T replicas, its couplings, tracked energies, both index maps and the per-slot thresholds -- resident in
 // shared memory for n_mcs whole MCS:  [ n_metro sweeps -> Houdayer exchange per temperature -> PT pass ] x n_mcs.
 // Samples never interact (P:7), so there is no grid-wide synchronisation; the state is read from and
-// written back to global memory once per call.  The phases are the same device functions the separate kernels
-// use (update_word, houdayer_pair) and the exchange walk of k_exchange, so the results are bit-identical.
+// written back to global memory once per call.  The sweep is the device function the separate kernel uses
+// (update_word); the Houdayer phase runs one LANE per temperature where the lattice allows it
+// (houdayer_lanes.cuh), else one warp per temperature (houdayer.cuh); the exchange walk is done by one lane per
+// chain.  All of them compute exactly what the separate kernels compute, so the results are bit-identical.
 #pragma once
 #include "kernels.cuh"
+#include "houdayer_lanes.cuh"
 
 namespace ptg {
 
@@ -14,23 +17,35 @@ struct McsArgs {
     uint32_t sweep0, houd0, exch0;          // counter values at the start of the call
 };
 
-// shared-memory carve-up, shared by host (size) and device (pointers); all offsets in 32-bit words
+// shared-memory carve-up, shared by host (size) and device (pointers); all offsets in 32-bit words.
+// A replica occupies RS = 2W + 1 words (colour 0 | colour 1 | pad): the odd stride lets 32 lanes that each own a
+// different replica (lane-per-pair Houdayer) hit 32 different banks.
 struct McsSmem {
-    int oJ, oS, oE, oTos, oSot, oThr, oAcc, oLast, oCum, oScr, words;
-    __host__ __device__ McsSmem(int D, int W, int T, int nwarps)
+    int RS, oJ, oS, oE, oTos, oSot, oThr, oAcc, oLast, oCum, oU, oSgn, oScr, words;
+    __host__ __device__ McsSmem(int D, int W, int T, int nwarps, bool lanes)
     {
+        RS = 2 * W + 1;
         int o = 0;
         oJ = o;    o += 2 * 2 * D * W;
-        oS = o;    o += 2 * T * 2 * W;
+        oS = o;    o += 2 * T * RS;
         oE = o;    o += 2 * T;
         oTos = o;  o += 2 * T;
         oSot = o;  o += 2 * T;
-        oThr = o;  o += 2 * T * 4;
+        o = (o + 3) & ~3;
+        oThr = o;  o += 2 * T * 4;          // 16-byte aligned rows
         oAcc = o;  o += 2 * T;              // accepted swaps of this call per (chain, pair)
         oLast = o; o += T;
         o = (o + 1) & ~1;
         oCum = o;  o += 2 * T;              // 64-bit
-        oScr = o;  o += nwarps * 4 * W;
+        oU = o;    o += 2 * T;              // PT draws of the current pass, [chain][pair]
+        oSgn = o;  o += T;
+        oScr = o;
+        if (lanes) {
+            const int groups = (T + 31) / 32;
+            o += (groups < nwarps ? groups : nwarps) * 2 * (2 * W) * kLaneStride;
+        } else {
+            o += nwarps * 4 * W;
+        }
         words = o;
     }
 };
@@ -39,19 +54,24 @@ template <class LAT, int NT, int MINB>
 __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
 {
     constexpr int D = LAT::D, W = LAT::W, NWARPS = NT / 32;
+    constexpr bool LANES = LaneHoudayer<LAT>::kEligible;
     extern __shared__ __align__(16) uint32_t msm[];
     const int T = P.T, R = 2 * T;
-    const McsSmem L(D, W, T, NWARPS);
+    const McsSmem L(D, W, T, NWARPS, LANES);
+    constexpr int RS = 2 * W + 1;
     uint32_t *sJ = msm + L.oJ, *sS = msm + L.oS, *sThr = msm + L.oThr, *sAcc = msm + L.oAcc, *sLast = msm + L.oLast;
-    int *sE = (int *)(msm + L.oE), *sTos = (int *)(msm + L.oTos), *sSot = (int *)(msm + L.oSot);
+    uint32_t *sU = msm + L.oU;
+    int *sE = (int *)(msm + L.oE), *sTos = (int *)(msm + L.oTos), *sSot = (int *)(msm + L.oSot), *sSgn = (int *)(msm + L.oSgn);
     unsigned long long *sCum = (unsigned long long *)(msm + L.oCum);
-    uint32_t *scratch = msm + L.oScr + (threadIdx.x >> 5) * 4 * W;
     const int s = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const uint32_t g = P.g0 + (uint32_t)s;
     const size_t rep0 = (size_t)s * R;
 
     for (int i = tid; i < 2 * 2 * D * W; i += NT) sJ[i] = P.d.Jn[(size_t)s * 2 * 2 * D * W + i];
-    for (int i = tid; i < R * 2 * W; i += NT) sS[i] = P.d.spin[rep0 * 2 * W + i];
+    for (int i = tid; i < R * 2 * W; i += NT) {
+        const int q = i / (2 * W), j = i - q * (2 * W);
+        sS[q * RS + j] = P.d.spin[rep0 * 2 * W + i];
+    }
     for (int i = tid; i < R; i += NT) {
         const int t = P.d.tos[rep0 + i];
         sTos[i] = t;
@@ -61,7 +81,11 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
 #pragma unroll
         for (int k = 0; k < 4; ++k) sThr[4 * i + k] = P.d.thrM[4 * t + k];
     }
-    for (int i = tid; i < T; i += NT) { sLast[i] = P.d.last[(size_t)s * T + i]; sCum[i] = 0ull; }
+    for (int i = tid; i < T; i += NT) {
+        sLast[i] = P.d.last[(size_t)s * T + i];
+        sCum[i] = 0ull;
+        sSgn[i] = (i < T - 1) ? P.d.sgn[i] : 0;
+    }
     __syncthreads();
 
     for (int m = 0; m < a.n_mcs; ++m) {
@@ -76,84 +100,109 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                     uint32_t thr[D];
 #pragma unroll
                     for (int k = 0; k < D; ++k) thr[k] = sThr[4 * q + k];
-                    const int dE = update_word(lat, sS + (q * 2 + p) * W, sS + (q * 2 + (1 - p)) * W, sJ + p * 2 * D * W, W, w,
+                    const int dE = update_word(lat, sS + q * RS + p * W, sS + q * RS + (1 - p) * W, sJ + p * 2 * D * W, W, w,
                                                p, thr, step, g, make_tag(DOM_METRO, p, c, r), P.rk);
                     if (dE != 0) atomicAdd(sE + q, dE);
                 }
                 __syncthreads();
             }
         }
-        // ---- a5: Houdayer exchange, one warp per temperature
+        // ---- a5: Houdayer exchange
         if (a.do_houdayer) {
             const uint32_t step = a.houd0 + (uint32_t)m;
-            for (int t = wid; t < T; t += NWARPS) {
-                const int ra = sSot[t], rb = T + sSot[T + t];
-                uint32_t u, o1, o2, o3;
-                philox4x32_10(0u, step, g, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
-                int delta;
-                const int size = houdayer_pair(lat, sS + (ra * 2) * W, sS + (ra * 2 + 1) * W, sS + (rb * 2) * W,
-                                               sS + (rb * 2 + 1) * W, sJ, scratch, u, lane, delta);
-                if (lane == 0) {
-                    sE[ra] += delta;
-                    sE[rb] -= delta;
-                    sLast[t] = (uint32_t)size;
-                    sCum[t] += (unsigned long long)size;
+            if constexpr (LANES) {
+                // one LANE per temperature: warp k takes temperatures [32k, 32k+32), then strides by the warps in use
+                const int groups = (T + 31) / 32, hw = groups < NWARPS ? groups : NWARPS;
+                if (wid < hw) {
+                    uint32_t *col = msm + L.oScr + wid * LaneHoudayer<LAT>::kScratchWords + lane;
+                    for (int t0 = wid * 32; t0 < T; t0 += hw * 32) {
+                        const int t = t0 + lane;
+                        const bool active = t < T;
+                        int ra = 0, rb = T;
+                        uint32_t u = 0, o1, o2, o3;
+                        if (active) {
+                            ra = sSot[t];
+                            rb = T + sSot[T + t];
+                            philox4x32_10(0u, step, g, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
+                        }
+                        int delta;
+                        const int size = houdayer_lane(lat, sS + ra * RS, sS + ra * RS + W, sS + rb * RS, sS + rb * RS + W,
+                                                       sJ, col, u, active, delta);
+                        if (active) {
+                            sE[ra] += delta;
+                            sE[rb] -= delta;
+                            sLast[t] = (uint32_t)size;
+                            sCum[t] += (unsigned long long)size;
+                        }
+                    }
+                }
+            } else {
+                // one WARP per temperature
+                uint32_t *scratch = msm + L.oScr + wid * 4 * W;
+                for (int t = wid; t < T; t += NWARPS) {
+                    const int ra = sSot[t], rb = T + sSot[T + t];
+                    uint32_t u, o1, o2, o3;
+                    philox4x32_10(0u, step, g, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
+                    int delta;
+                    const int size = houdayer_pair(lat, sS + ra * RS, sS + ra * RS + W, sS + rb * RS, sS + rb * RS + W, sJ,
+                                                   scratch, u, lane, delta);
+                    if (lane == 0) {
+                        sE[ra] += delta;
+                        sE[rb] -= delta;
+                        sLast[t] = (uint32_t)size;
+                        sCum[t] += (unsigned long long)size;
+                    }
                 }
             }
             __syncthreads();
         }
-        // ---- a4: PT pass, one warp per chain (R9: sequential walk, each step seeing the previous)
+        // ---- a4: PT pass (R9: sequential walk, each step seeing the previous).  Warp 0: all lanes draw the Philox
+        // words, then one lane per chain walks its ladder; only the two index maps change.
         if (a.do_exchange && T > 1) {
             const uint32_t step = a.exch0 + (uint32_t)m;
-            for (int c = wid; c < 2; c += NWARPS) {
-                int *so = sSot + c * T;
-                const int *Ec = sE + c * T;
-                int ea = 0, ra = 0;
-                if (lane == 0) { ra = so[0]; ea = Ec[ra]; }
-                for (int tb = 0; tb < T - 1; tb += 32) {
-                    const int tl = tb + lane;
-                    uint32_t u_l = 0, o1, o2, o3;
-                    int rb_l = 0, eb_l = 0, sg_l = 0;
-                    if (tl < T - 1) {
-                        philox4x32_10((uint32_t)tl, step, g, make_tag(DOM_SWAP, 0, c, 0), P.rk, u_l, o1, o2, o3);
-                        rb_l = so[tl + 1];              // positions > t are not modified before they are read
-                        eb_l = Ec[rb_l];
-                        sg_l = P.d.sgn[tl];
-                    }
-                    __syncwarp();
-                    const int nstep = min(32, T - 1 - tb);
-                    uint32_t accmask = 0;
-                    for (int j = 0; j < nstep; ++j) {
-                        const uint32_t u = __shfl_sync(0xFFFFFFFFu, u_l, j);
-                        const int rb = __shfl_sync(0xFFFFFFFFu, rb_l, j), eb = __shfl_sync(0xFFFFFFFFu, eb_l, j);
-                        const int sg = __shfl_sync(0xFFFFFFFFu, sg_l, j);
-                        if (lane == 0) {
-                            const int t = tb + j;
-                            const int dE = ea - eb;
-                            const uint32_t mm = (uint32_t)(dE < 0 ? -dE : dE) >> 2;
-                            const bool acc = ((long long)sg * dE <= 0) || (u < thrX_lookup(P, t, mm));
-                            if (acc) { so[t] = rb; accmask |= 1u << j; }
-                            else     { so[t] = ra; ea = eb; ra = rb; }
-                        }
-                    }
-                    accmask = __shfl_sync(0xFFFFFFFFu, accmask, 0);
-                    if (tl < T - 1 && ((accmask >> lane) & 1u)) sAcc[c * T + tl] += 1u;
+            if (wid == 0) {
+                for (int i = lane; i < 2 * (T - 1); i += 32) {
+                    const int c = i / (T - 1), t = i - c * (T - 1);
+                    uint32_t u, o1, o2, o3;
+                    philox4x32_10((uint32_t)t, step, g, make_tag(DOM_SWAP, 0, c, 0), P.rk, u, o1, o2, o3);
+                    sU[c * T + t] = u;
                 }
-                if (lane == 0) so[T - 1] = ra;
                 __syncwarp();
-                for (int t = lane; t < T; t += 32) sTos[c * T + so[t]] = t;
+                if (lane < 2) {
+                    const int c = lane;
+                    int *so = sSot + c * T;
+                    const int *Ec = sE + c * T;
+                    int ra = so[0], ea = Ec[ra];
+                    int rb = so[1], eb = Ec[rb];
+                    for (int t = 0; t < T - 1; ++t) {
+                        int rbn = 0, ebn = 0;
+                        if (t + 2 < T) { rbn = so[t + 2]; ebn = Ec[rbn]; }     // positions > t are not modified before they are read
+                        const int dE = ea - eb;
+                        bool acc = sSgn[t] * dE <= 0;
+                        if (!acc) acc = sU[c * T + t] < thrX_lookup(P, t, (uint32_t)(dE < 0 ? -dE : dE) >> 2);
+                        if (acc) { so[t] = rb; sAcc[c * T + t] += 1u; }        // position t is final; (ea, ra) moves up
+                        else     { so[t] = ra; ea = eb; ra = rb; }
+                        rb = rbn; eb = ebn;
+                    }
+                    so[T - 1] = ra;
+                }
+                __syncwarp();
+                for (int i = lane; i < R; i += 32) {
+                    const int c = i / T, t = i - c * T;
+                    sTos[c * T + sSot[i]] = t;
+                }
             }
             __syncthreads();
-            for (int i = tid; i < R; i += NT) {
-                const int t = sTos[i];
-#pragma unroll
-                for (int k = 0; k < 4; ++k) sThr[4 * i + k] = P.d.thrM[4 * t + k];
-            }
+            for (int i = tid; i < R; i += NT)
+                *(uint4 *)(sThr + 4 * i) = __ldg((const uint4 *)(P.d.thrM + 4 * sTos[i]));
             __syncthreads();
         }
     }
 
-    for (int i = tid; i < R * 2 * W; i += NT) P.d.spin[rep0 * 2 * W + i] = sS[i];
+    for (int i = tid; i < R * 2 * W; i += NT) {
+        const int q = i / (2 * W), j = i - q * (2 * W);
+        P.d.spin[rep0 * 2 * W + i] = sS[q * RS + j];
+    }
     for (int i = tid; i < R; i += NT) {
         P.d.E[rep0 + i] = sE[i];
         P.d.tos[rep0 + i] = sTos[i];

@@ -343,7 +343,7 @@ constexpr int kMcsThreads = 128, kMcsMinBlocks = 7;
 bool mcs_fused_eligible(size_t *smem_out)
 {
     if (!G.fast || G.fused_mode == 0) return false;
-    const McsSmem lay(G.P.D, G.P.W, G.P.T, kMcsThreads / 32);
+    const McsSmem lay(G.P.D, G.P.W, G.P.T, kMcsThreads / 32, 2 * G.P.W <= 32);
     const size_t smem = (size_t)lay.words * 4;
     if (smem_out) *smem_out = smem;
     return (smem + 1024) * 4 <= 227 * 1024;
