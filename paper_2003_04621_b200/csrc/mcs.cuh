@@ -14,6 +14,7 @@ namespace ptg {
 
 struct McsArgs {
     int n_mcs, n_metro, do_houdayer, do_exchange;
+    int split_chains;                       // 1: one CTA per (sample, chain) -- only without Houdayer moves (the chains never meet)
     uint32_t sweep0, houd0, exch0;          // counter values at the start of the call
 };
 
@@ -22,12 +23,13 @@ struct McsArgs {
 // different replica (lane-per-pair Houdayer) hit 32 different banks.
 struct McsSmem {
     int RS, oJ, oS, oE, oTos, oSot, oThr, oAcc, oLast, oCum, oU, oSgn, oScr, words;
-    __host__ __device__ McsSmem(int D, int W, int T, int nwarps, bool lanes)
+    // nch: chains held by the CTA (2 = the whole sample, 1 = one chain)
+    __host__ __device__ McsSmem(int D, int W, int T, int nwarps, bool lanes, int nch)
     {
         RS = 2 * W + 1;
         int o = 0;
         oJ = o;    o += 2 * 2 * D * W;
-        oS = o;    o += 2 * T * RS;
+        oS = o;    o += nch * T * RS;
         oE = o;    o += 2 * T;
         oTos = o;  o += 2 * T;
         oSot = o;  o += 2 * T;
@@ -40,7 +42,9 @@ struct McsSmem {
         oU = o;    o += 2 * T;              // PT draws of the current pass, [chain][pair]
         oSgn = o;  o += T;
         oScr = o;
-        if (lanes) {
+        if (nch < 2) {
+            // no Houdayer phase, no scratch
+        } else if (lanes) {
             const int groups = (T + 31) / 32;
             o += (groups < nwarps ? groups : nwarps) * 2 * (2 * W) * kLaneStride;
         } else {
@@ -56,16 +60,20 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
     constexpr int D = LAT::D, W = LAT::W, NWARPS = NT / 32;
     constexpr bool LANES = LaneHoudayer<LAT>::kEligible;
     extern __shared__ __align__(16) uint32_t msm[];
-    const int T = P.T, R = 2 * T;
-    const McsSmem L(D, W, T, NWARPS, LANES);
+    const int T = P.T;
+    const int NCH = a.split_chains ? 1 : 2;         // chains in this CTA
+    const int R = NCH * T;                          // replicas in this CTA
+    const McsSmem L(D, W, T, NWARPS, LANES, NCH);
     constexpr int RS = 2 * W + 1;
     uint32_t *sJ = msm + L.oJ, *sS = msm + L.oS, *sThr = msm + L.oThr, *sAcc = msm + L.oAcc, *sLast = msm + L.oLast;
     uint32_t *sU = msm + L.oU;
     int *sE = (int *)(msm + L.oE), *sTos = (int *)(msm + L.oTos), *sSot = (int *)(msm + L.oSot), *sSgn = (int *)(msm + L.oSgn);
     unsigned long long *sCum = (unsigned long long *)(msm + L.oCum);
-    const int s = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int s = a.split_chains ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
+    const int c0 = a.split_chains ? (int)(blockIdx.x & 1) : 0;      // first chain of this CTA
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const uint32_t g = P.g0 + (uint32_t)s;
-    const size_t rep0 = (size_t)s * R;
+    const size_t rep0 = ((size_t)s * 2 + c0) * T;
 
     for (int i = tid; i < 2 * 2 * D * W; i += NT) sJ[i] = P.d.Jn[(size_t)s * 2 * 2 * D * W + i];
     for (int i = tid; i < R * 2 * W; i += NT) {
@@ -96,7 +104,7 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
 #pragma unroll 1
                 for (int item = tid; item < R * W; item += NT) {
                     const int q = item / W, w = item - q * W;
-                    const int c = (q >= T) ? 1 : 0, r = q - c * T;
+                    const int cl = (q >= T) ? 1 : 0, r = q - cl * T, c = c0 + cl;
                     uint32_t thr[D];
 #pragma unroll
                     for (int k = 0; k < D; ++k) thr[k] = sThr[4 * q + k];
@@ -108,7 +116,7 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
             }
         }
         // ---- a5: Houdayer exchange
-        if (a.do_houdayer) {
+        if (a.do_houdayer && NCH == 2) {
             const uint32_t step = a.houd0 + (uint32_t)m;
             if constexpr (LANES) {
                 // one LANE per temperature: warp k takes temperatures [32k, 32k+32), then strides by the warps in use
@@ -161,14 +169,14 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
         if (a.do_exchange && T > 1) {
             const uint32_t step = a.exch0 + (uint32_t)m;
             if (wid == 0) {
-                for (int i = lane; i < 2 * (T - 1); i += 32) {
-                    const int c = i / (T - 1), t = i - c * (T - 1);
+                for (int i = lane; i < NCH * (T - 1); i += 32) {
+                    const int c = i / (T - 1), t = i - c * (T - 1);        // c: chain index within the CTA
                     uint32_t u, o1, o2, o3;
-                    philox4x32_10((uint32_t)t, step, g, make_tag(DOM_SWAP, 0, c, 0), P.rk, u, o1, o2, o3);
+                    philox4x32_10((uint32_t)t, step, g, make_tag(DOM_SWAP, 0, c0 + c, 0), P.rk, u, o1, o2, o3);
                     sU[c * T + t] = u;
                 }
                 __syncwarp();
-                if (lane < 2) {
+                if (lane < NCH) {
                     const int c = lane;
                     int *so = sSot + c * T;
                     const int *Ec = sE + c * T;
@@ -211,12 +219,13 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
     if (T > 1)
         for (int i = tid; i < R; i += NT) {
             const int c = i / T, t = i - c * T;
-            if (t < T - 1 && sAcc[i]) P.d.accepts[((size_t)s * 2 + c) * (T - 1) + t] += (unsigned long long)sAcc[i];
+            if (t < T - 1 && sAcc[i]) P.d.accepts[((size_t)s * 2 + c0 + c) * (T - 1) + t] += (unsigned long long)sAcc[i];
         }
-    for (int i = tid; i < T; i += NT) {
-        P.d.last[(size_t)s * T + i] = sLast[i];
-        P.d.cum[(size_t)s * T + i] += sCum[i];
-    }
+    if (NCH == 2)
+        for (int i = tid; i < T; i += NT) {
+            P.d.last[(size_t)s * T + i] = sLast[i];
+            P.d.cum[(size_t)s * T + i] += sCum[i];
+        }
 }
 
 }  // namespace ptg

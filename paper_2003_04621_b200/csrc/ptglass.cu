@@ -340,10 +340,14 @@ cudaError_t launch_measure(int32_t *Q, int32_t *QL)
 // sample's state fits in shared memory with at least 4 CTAs per SM (else the separate kernels are faster).
 constexpr int kMcsThreads = 128, kMcsMinBlocks = 7;
 
-bool mcs_fused_eligible(size_t *smem_out)
+// One CTA per (sample, chain) instead of per sample: legal when the call makes no Houdayer moves (sweeps and PT passes
+// never couple the two chains, R10) and worthwhile when a chain alone still fills the CTA (>= 4 work items per thread).
+bool mcs_split_chains(int do_houdayer) { return !do_houdayer && (long)G.P.T * G.P.W >= 4L * kMcsThreads; }
+
+bool mcs_fused_eligible(size_t *smem_out, int do_houdayer = 1)
 {
     if (!G.fast || G.fused_mode == 0) return false;
-    const McsSmem lay(G.P.D, G.P.W, G.P.T, kMcsThreads / 32, 2 * G.P.W <= 32);
+    const McsSmem lay(G.P.D, G.P.W, G.P.T, kMcsThreads / 32, 2 * G.P.W <= 32, mcs_split_chains(do_houdayer) ? 1 : 2);
     const size_t smem = (size_t)lay.words * 4;
     if (smem_out) *smem_out = smem;
     return (smem + 1024) * 4 <= 227 * 1024;
@@ -357,11 +361,12 @@ cudaError_t launch_mcs(const McsArgs &a)
         using LAT = decltype(lat);
         if constexpr (LAT::kFast) {
             size_t smem = 0;
-            mcs_fused_eligible(&smem);
+            mcs_fused_eligible(&smem, a.do_houdayer);
             auto kern = k_mcs<LAT, kMcsThreads, kMcsMinBlocks>;
             err = allow_smem(kern, smem);
             if (err != cudaSuccess) return;
-            kern<<<(unsigned)G.P.S, kMcsThreads, smem, G.stream>>>(lat, G.P, a);
+            const unsigned grid = (unsigned)G.P.S * (a.split_chains ? 2u : 1u);
+            kern<<<grid, kMcsThreads, smem, G.stream>>>(lat, G.P, a);
             ++G.launches;
             err = cudaGetLastError();
         } else {
@@ -558,8 +563,9 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
         (do_houdayer && (uint64_t)G.n_houdayer + M > 4294967295ull))
         return fail(PT_ERR_OVERFLOW, "a step counter would overflow");
     if (n_mcs == 0 || (n_metro == 0 && !do_houdayer && !do_exchange)) return PT_OK;
-    if (mcs_fused_eligible(nullptr)) {
-        const McsArgs a{n_mcs, n_metro, do_houdayer ? 1 : 0, do_exchange ? 1 : 0, G.n_sweep, G.n_houdayer, G.n_exchange};
+    if (mcs_fused_eligible(nullptr, do_houdayer)) {
+        const McsArgs a{n_mcs, n_metro, do_houdayer ? 1 : 0, do_exchange ? 1 : 0, mcs_split_chains(do_houdayer) ? 1 : 0,
+                        G.n_sweep, G.n_houdayer, G.n_exchange};
         CK(launch_mcs(a));
         G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
         if (do_houdayer) G.n_houdayer += (uint32_t)M;
