@@ -58,6 +58,8 @@ def lib():
             "ref_set_spins": [C.c_void_p, C.c_void_p],
             "ref_set_couplings": [C.c_void_p, C.c_void_p],
             "ref_recompute_energy": [C.c_void_p, C.c_void_p, C.c_void_p],
+            "ref_get_round_trips": [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p],
+            "ref_schedule_family": [C.c_double, C.c_double, C.c_int, C.c_double, C.c_void_p, C.c_void_p],
         }.items():
             fn = getattr(L, name)
             fn.restype = C.c_int
@@ -72,6 +74,15 @@ def philox(key, ctr) -> np.ndarray:
     out = np.zeros(4, dtype=np.uint32)
     lib().ref_philox4x32_10(k.ctypes.data, c.ctypes.data, out.ctypes.data)
     return out
+
+
+def schedule_family(T_min, T_max, n_temps, phi):
+    """(temps, betas) of Eq. (6)-(7)."""
+    t = np.zeros(n_temps, dtype=np.float64)
+    b = np.zeros(n_temps, dtype=np.float64)
+    if lib().ref_schedule_family(float(T_min), float(T_max), int(n_temps), float(phi), t.ctypes.data, b.ctypes.data) != 0:
+        raise ValueError("ref_schedule_family rejected the arguments")
+    return t, b
 
 
 def threshold(x: float) -> int:
@@ -180,6 +191,13 @@ class Oracle:
         j = np.ascontiguousarray(J, dtype=np.int8)
         assert j.shape == (self.S, self.d, self.N)
         self._ck(lib().ref_set_couplings(self._h, _p(j)))
+
+    def get_round_trips(self):
+        trips = np.zeros((self.S, 2, self.T), dtype=np.uint32)
+        tau_sum = np.zeros((self.S, 2, 32), dtype=np.uint64)
+        tau_cnt = np.zeros((self.S, 2, 32), dtype=np.uint64)
+        self._ck(lib().ref_get_round_trips(self._h, _p(trips), _p(tau_sum), _p(tau_cnt)))
+        return trips, tau_sum, tau_cnt
 
     def recompute_energy(self):
         E = np.zeros((self.S, 2, self.T), dtype=np.int32)

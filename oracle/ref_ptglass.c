@@ -33,6 +33,12 @@ struct ref_ctx {
     uint32_t *last_size;  /* [S][T] */
     uint64_t *cum_size;   /* [S][T] */
     uint32_t n_sweep, n_exchange, n_houdayer;
+    /* round-trip bookkeeping (readings R27-R29), per slot / per (sample, chain) */
+    uint32_t *rt_label;   /* [S][2][T] 0 = never at index 0 yet, 1 = last end visited is index 0, 2 = index T-1 */
+    uint32_t *rt_start;   /* [S][2][T] pass number at which the current trip started */
+    uint32_t *rt_trips;   /* [S][2][T] completed round trips 0 -> T-1 -> 0 */
+    uint64_t *rt_tau_sum; /* [S][2][32] sum of round-trip times completed at pass n, bin = floor(log2 n) */
+    uint64_t *rt_tau_cnt; /* [S][2][32] */
     int *nbr;             /* [N][2d]: nbr[i][2mu] = i+e_mu, nbr[i][2mu+1] = i-e_mu */
     int *queue;           /* [N] BFS queue */
     uint8_t *mark;        /* [N] */
@@ -165,6 +171,11 @@ ref_ctx *ref_create(int L, int d, int S, int T, const double *betas, uint64_t se
     c->accepts = (uint64_t *)calloc((size_t)S * 2 * T, sizeof(uint64_t));
     c->last_size = (uint32_t *)calloc((size_t)S * T, sizeof(uint32_t));
     c->cum_size = (uint64_t *)calloc((size_t)S * T, sizeof(uint64_t));
+    c->rt_label = (uint32_t *)calloc(R, sizeof(uint32_t));
+    c->rt_start = (uint32_t *)calloc(R, sizeof(uint32_t));
+    c->rt_trips = (uint32_t *)calloc(R, sizeof(uint32_t));
+    c->rt_tau_sum = (uint64_t *)calloc((size_t)S * 2 * 32, sizeof(uint64_t));
+    c->rt_tau_cnt = (uint64_t *)calloc((size_t)S * 2 * 32, sizeof(uint64_t));
     c->nbr = (int *)malloc(sizeof(int) * N * 2 * d);
     c->queue = (int *)malloc(sizeof(int) * N);
     c->mark = (uint8_t *)malloc(N);
@@ -185,6 +196,8 @@ ref_ctx *ref_create(int L, int d, int S, int T, const double *betas, uint64_t se
                 c->temp_of_slot[rep(c, s, ch, r)] = r;
                 c->slot_of_temp[rep(c, s, ch, r)] = r;
             }
+        /* the slot that starts at temperature index 0 starts its first trip at pass 0 (R28) */
+        for (int ch = 0; ch < 2; ++ch) c->rt_label[rep(c, s, ch, 0)] = 1;
     }
     /* 4. energies */
     recompute_all(c);
@@ -203,6 +216,7 @@ void ref_destroy(ref_ctx *c)
     if (!c) return;
     free(c->betas); free(c->J); free(c->spin); free(c->E); free(c->temp_of_slot); free(c->slot_of_temp);
     free(c->thrM); free(c->sgn); free(c->attempts); free(c->accepts); free(c->last_size); free(c->cum_size);
+    free(c->rt_label); free(c->rt_start); free(c->rt_trips); free(c->rt_tau_sum); free(c->rt_tau_cnt);
     free(c->nbr); free(c->queue); free(c->mark);
     free(c);
 }
@@ -269,9 +283,54 @@ int ref_exchange(ref_ctx *c)
                     c->accepts[k] += 1;
                 }
             }
+            /* round-trip bookkeeping after the pass (R27-R29): n = number of passes done, this one included.
+             * The replica now at index T-1 has reached the far end; the replica now at index 0 completes a
+             * round trip 0 -> T-1 -> 0 if it has been at the far end since its trip started. */
+            if (T > 1) {
+                uint32_t n = c->n_exchange + 1u;
+                size_t base = rep(c, s, ch, 0);
+                int r1 = sot[T - 1], r0 = sot[0];
+                if (c->rt_label[base + r1] == 1u) c->rt_label[base + r1] = 2u;
+                if (c->rt_label[base + r0] == 2u) {
+                    uint32_t tau = n - c->rt_start[base + r0];
+                    int b = 0;
+                    while ((n >> (b + 1)) != 0u) ++b;           /* b = floor(log2 n), n >= 1 */
+                    c->rt_trips[base + r0] += 1u;
+                    c->rt_tau_sum[((size_t)s * 2 + ch) * 32 + b] += tau;
+                    c->rt_tau_cnt[((size_t)s * 2 + ch) * 32 + b] += 1u;
+                    c->rt_label[base + r0] = 1u;
+                    c->rt_start[base + r0] = n;
+                } else if (c->rt_label[base + r0] == 0u) {
+                    c->rt_label[base + r0] = 1u;
+                    c->rt_start[base + r0] = n;
+                }
+            }
         }
     }
     c->n_exchange += 1;
+    return 0;
+}
+
+/* ---------------------------------------------------------------- temperature-schedule family, Eq. (6)-(7) */
+int ref_schedule_family(double T_min, double T_max, int n_temps, double phi, double *temps, double *betas)
+{
+    if (!(T_min > 0.0) || !(T_max >= T_min) || n_temps < 1 || !(phi > 0.0) || !isfinite(T_max) || !isfinite(phi)) return -1;
+    double T_norm = (n_temps > 1) ? (T_max - T_min) / pow((double)(n_temps - 1), phi) : 0.0;     /* Eq. (7) */
+    for (int i = 0; i < n_temps; ++i) {
+        double Ti = pow((double)i, phi) * T_norm + T_min;                                        /* Eq. (6) */
+        if (temps) temps[i] = Ti;
+        if (betas) betas[i] = 1.0 / Ti;
+    }
+    return 0;
+}
+
+int ref_get_round_trips(const ref_ctx *c, uint32_t *trips, uint64_t *tau_sum, uint64_t *tau_cnt)
+{
+    if (!c) return -1;
+    size_t R = (size_t)c->S * 2 * c->T, B = (size_t)c->S * 2 * 32;
+    if (trips) memcpy(trips, c->rt_trips, R * sizeof(uint32_t));
+    if (tau_sum) memcpy(tau_sum, c->rt_tau_sum, B * sizeof(uint64_t));
+    if (tau_cnt) memcpy(tau_cnt, c->rt_tau_cnt, B * sizeof(uint64_t));
     return 0;
 }
 

@@ -53,6 +53,16 @@ int ref_get_swap_counts(const ref_ctx *c, uint64_t *attempts, uint64_t *accepts 
 int ref_get_cluster_sizes(const ref_ctx *c, uint32_t *last, uint64_t *cumulative /* [S][T], may be NULL */);
 int ref_get_perm(const ref_ctx *c, int32_t *temp_of_slot, int32_t *slot_of_temp /* [S][2][T] */);
 
+/* Temperature-schedule family of Eq. (6)-(7): T_i = i^phi * T_norm + T_min,
+ * T_norm = (T_max - T_min) / (N_T - 1)^phi, in double with C pow(); betas[i] = 1 / T_i.  temps / betas may be NULL. */
+int ref_schedule_family(double T_min, double T_max, int n_temps, double phi, double *temps, double *betas);
+
+/* Round trips in temperature space (tunnelling time; readings R27-R29): per slot the number of
+ * completed trips index 0 -> index T-1 -> index 0 (slot order); per (sample, chain) the sum and the number of
+ * round-trip times (in exchange passes) completed at pass n, binned by floor(log2 n) (logarithmic binning, Fig. 4). */
+int ref_get_round_trips(const ref_ctx *c, uint32_t *trips /* [S][2][T] */, uint64_t *tau_sum /* [S][2][32] */,
+                        uint64_t *tau_cnt /* [S][2][32] */);
+
 /* State in SLOT order. */
 int ref_get_spins(const ref_ctx *c, int8_t *spins /* [S][2][T][N] */);
 int ref_get_couplings(const ref_ctx *c, int8_t *J /* [S][d][N] */);
