@@ -98,6 +98,27 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange);
 int pt_set_fused(int mode);
 int pt_get_fused(int *fused);
 
+/* ---- NEXT-1: temperature-schedule family and tunnelling times --------------------------------- */
+
+/* Temperature-schedule family of Eq. (6)-(7) (R30): T_i = i^phi * T_norm + T_min with
+ * T_norm = (T_max - T_min) / (n_temps - 1)^phi, in double with pow(); betas_out[i] = 1 / T_i.  Index 0 is T_min (the
+ * paper's numbering T_0 < T_1 < ...); phi = 1 is the linear ladder.  HOST arrays [n_temps], either may be NULL.
+ * Pure host function: needs no device and no context.  PT_ERR_ARG unless 0 < T_min <= T_max < inf, n_temps >= 1,
+ * 0 < phi < inf.  Pass betas_out to pt_init like any ladder. */
+int pt_schedule_family(double T_min, double T_max, int n_temps, double phi, double *temps_out, double *betas_out);
+
+/* Round trips in temperature space, the paper's tunnelling time tau_tunnel (R27-R29): "the expected time
+ * it takes for a replica to move from the lowest to the highest temperature and back".  When tracking is on, after
+ * every PT pass n (1-based count of passes since pt_init) of every (sample, chain): the slot now at index T-1 is
+ * marked as having reached the far end; the slot now at index 0 completes a round trip if it was so marked since its
+ * trip began (tau = n - start; start <- n), or begins its first trip.  The slot that starts at index 0 begins at
+ * pass 0.  pt_set_round_trip_tracking must be called after pt_bind and BEFORE pt_init (PT_ERR_STATE otherwise);
+ * default off.  pt_get_round_trips: trips[S][2][T] completed trips per SLOT; tau_sum / tau_cnt [S][2][32]: sum and
+ * number of the round-trip times completed at pass n, in bin floor(log2 n) (logarithmic binning, Fig. 4); any pointer
+ * may be NULL; PT_ERR_STATE if tracking is off.  Time is counted in PT passes (= MCS in pt_mcs). */
+int pt_set_round_trip_tracking(int on);
+int pt_get_round_trips(uint32_t *trips, uint64_t *tau_sum, uint64_t *tau_cnt);
+
 /* ---- observables: all integer, indexed by TEMPERATURE index t ------------------------------------------- */
 
 int pt_get_energy(int32_t *E /* [S][2][T]: E of the configuration currently at temperature t (Eq. (3) x N) */);

@@ -31,6 +31,9 @@ SYMBOLS = {
     "pt_mcs": (_i, [_i, _i, _i, _i]),
     "pt_set_fused": (_i, [_i]),
     "pt_get_fused": (_i, [_vp]),
+    "pt_schedule_family": (_i, [C.c_double, C.c_double, _i, C.c_double, _vp, _vp]),
+    "pt_set_round_trip_tracking": (_i, [_i]),
+    "pt_get_round_trips": (_i, [_vp, _vp, _vp]),
     "pt_get_energy": (_i, [_vp]),
     "pt_measure_overlap": (_i, [_vp, _vp]),
     "pt_get_swap_counts": (_i, [_vp, _vp]),
@@ -136,7 +139,8 @@ def pt_free():
     _workspace = None
 
 
-def pt_open(L, d, n_samples, n_temps, betas, seed, sample_offset=0, device="cuda:0", stream=None, general=False):
+def pt_open(L, d, n_samples, n_temps, betas, seed, sample_offset=0, device="cuda:0", stream=None, general=False,
+            track_round_trips=False):
     """Convenience: allocate the workspace with torch, bind it and initialise.  Returns the workspace tensor."""
     import torch
 
@@ -145,8 +149,30 @@ def pt_open(L, d, n_samples, n_temps, betas, seed, sample_offset=0, device="cuda
         pt_bind(ws, stream)
         if general:
             pt_force_general_path(0)
+        if track_round_trips:
+            pt_set_round_trip_tracking(1)
         pt_init(L, d, n_samples, n_temps, betas, seed, sample_offset)
     return ws
+
+
+def pt_schedule_family(T_min, T_max, n_temps, phi):
+    """(temps, betas) of Eq. (6)-(7); host only."""
+    t = np.zeros(max(n_temps, 0), dtype=np.float64)
+    b = np.zeros(max(n_temps, 0), dtype=np.float64)
+    _ck(lib().pt_schedule_family(float(T_min), float(T_max), int(n_temps), float(phi), _p(t), _p(b)))
+    return t, b
+
+
+def pt_set_round_trip_tracking(on):
+    _ck(lib().pt_set_round_trip_tracking(int(on)))
+
+
+def pt_get_round_trips():
+    trips = np.zeros((_shape["S"], 2, _shape["T"]), dtype=np.uint32)
+    tau_sum = np.zeros((_shape["S"], 2, 32), dtype=np.uint64)
+    tau_cnt = np.zeros((_shape["S"], 2, 32), dtype=np.uint64)
+    _ck(lib().pt_get_round_trips(_p(trips), _p(tau_sum), _p(tau_cnt)))
+    return trips, tau_sum, tau_cnt
 
 
 def pt_sweep(n=1):

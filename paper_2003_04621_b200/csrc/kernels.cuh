@@ -28,12 +28,16 @@ struct DevPtrs {
     int32_t *outQ, *outQL;      // [S][T]
     int *mismatch;              // [1]
     int8_t *stage;              // int8 staging for get/set: max(S*2*T*N, S*D*N) bytes
+    // round-trip bookkeeping (NEXT-1, R27-R29)
+    uint32_t *rtLabel, *rtStart, *rtTrips;      // [S][2][T] per slot
+    unsigned long long *rtSum, *rtCnt;          // [S][2][32] per (sample, chain), bin = floor(log2 pass)
 };
 
 struct Params {
     int L, D, S, T, N, NH, W;
     uint32_t g0;                // sample_offset: global sample index = g0 + s
     uint32_t strideX;
+    int track;                  // 1: round-trip bookkeeping after every PT pass
     RoundKeys rk;
     DevPtrs d;
 };
@@ -165,6 +169,9 @@ __global__ void k_identity_perm(Params P)
     for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
         P.d.tos[id] = (int32_t)(id % P.T);
         P.d.sot[id] = (int32_t)(id % P.T);
+        P.d.rtLabel[id] = (id % P.T == 0) ? 1u : 0u;        // the slot that starts at index 0 starts its first trip (R28)
+        P.d.rtStart[id] = 0u;
+        P.d.rtTrips[id] = 0u;
     }
 }
 
@@ -388,6 +395,26 @@ __global__ void __launch_bounds__(128, 7) k_sweep(LAT lat, Params P, int R, uint
 // the lanes draw the T-1 Philox words in parallel, lane 0 walks the ladder sequentially on a temperature-ordered
 // copy of the energies in shared memory.  Only the two index arrays change.
 // =========================================================================================================
+// Round-trip bookkeeping after PT pass number n (1-based) of chain `chain` = s*2 + c (R27-R29): r0 / r1 = the slots now
+// at temperature index 0 / T-1.  Called by one thread per chain.
+__device__ __forceinline__ void round_trip_update(const Params &P, size_t chain, int r0, int r1, uint32_t n)
+{
+    uint32_t *lab = P.d.rtLabel + chain * P.T, *st = P.d.rtStart + chain * P.T;
+    if (lab[r1] == 1u) lab[r1] = 2u;
+    const uint32_t l0 = lab[r0];
+    if (l0 == 2u) {
+        const int b = 31 - __clz(n);
+        P.d.rtTrips[chain * P.T + r0] += 1u;
+        P.d.rtSum[chain * 32 + b] += (unsigned long long)(n - st[r0]);
+        P.d.rtCnt[chain * 32 + b] += 1ull;
+        lab[r0] = 1u;
+        st[r0] = n;
+    } else if (l0 == 0u) {
+        lab[r0] = 1u;
+        st[r0] = n;
+    }
+}
+
 __device__ __forceinline__ uint32_t thrX_lookup(const Params &P, int t, uint32_t m)
 {
     return (m < P.strideX) ? __ldg(P.d.thrX + (size_t)t * P.strideX + m) : 0u;
@@ -440,7 +467,10 @@ __global__ void k_exchange(Params P, uint32_t step)
             }
         }
     }
-    if (lane == 0) { Et[T - 1] = ea; so[T - 1] = ra; }
+    if (lane == 0) {
+        Et[T - 1] = ea; so[T - 1] = ra;
+        if (P.track && T > 1) round_trip_update(P, (size_t)chain, so[0], ra, step + 1u);
+    }
     __syncwarp();
     for (int t = lane; t < T; t += 32) {
         const int r = so[t];

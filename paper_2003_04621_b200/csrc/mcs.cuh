@@ -193,6 +193,7 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                         rb = rbn; eb = ebn;
                     }
                     so[T - 1] = ra;
+                    if (P.track) round_trip_update(P, (size_t)s * 2 + c0 + c, so[0], ra, step + 1u);
                 }
                 __syncwarp();
                 for (int i = lane; i < R; i += 32) {

@@ -26,6 +26,7 @@ struct Context {
     bool bound = false, inited = false;
     int force_general = -1;
     int fused_mode = -1;        // -1: fused pt_mcs where eligible, 0: always separate launches
+    int track = 0;              // round-trip bookkeeping (NEXT-1), chosen before pt_init
     bool fast = false;
     Params P{};
     std::vector<double> betas;
@@ -184,6 +185,11 @@ size_t carve(void *base, int L, int d, int S, int T, uint32_t strideX, DevPtrs *
     p.outQ = c.take<int32_t>(base, (size_t)S * T);
     p.outQL = c.take<int32_t>(base, (size_t)S * T);
     p.mismatch = c.take<int>(base, 64);
+    p.rtLabel = c.take<uint32_t>(base, R);
+    p.rtStart = c.take<uint32_t>(base, R);
+    p.rtTrips = c.take<uint32_t>(base, R);
+    p.rtSum = c.take<unsigned long long>(base, (size_t)S * 2 * 32);
+    p.rtCnt = c.take<unsigned long long>(base, (size_t)S * 2 * 32);
     const size_t sb = std::max(R * N, (size_t)S * d * N);
     p.stage = c.take<int8_t>(base, sb);
     if (out) *out = p;
@@ -468,6 +474,7 @@ int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas,
     P.g0 = sample_offset;
     P.rk = make_round_keys((uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32));
     P.strideX = swap_stride(G.betas, d, P.N);
+    P.track = G.track;
     const size_t need = carve(G.ws, L, d, n_samples, n_temps, P.strideX, &P.d, &G.stage_bytes);
     if (need > G.ws_bytes)
         return fail(PT_ERR_STATE, "workspace too small: %zu bytes bound, %zu needed", G.ws_bytes, need);
@@ -492,6 +499,8 @@ int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas,
     CK(cudaMemsetAsync(P.d.last, 0, (size_t)P.S * P.T * 4, G.stream));
     CK(cudaMemsetAsync(P.d.cum, 0, (size_t)P.S * P.T * 8, G.stream));
     CK(cudaMemsetAsync(P.d.mismatch, 0, 64 * sizeof(int), G.stream));
+    CK(cudaMemsetAsync(P.d.rtSum, 0, (size_t)P.S * 2 * 32 * 8, G.stream));
+    CK(cudaMemsetAsync(P.d.rtCnt, 0, (size_t)P.S * 2 * 32 * 8, G.stream));
 
     // couplings, spins (Philox domains 1, 2), identity permutations, energies
     k_draw_couplings<<<grid_for((long)P.S * P.D * (P.N / 4), 256), 256, 0, G.stream>>>(P);
@@ -592,6 +601,40 @@ int pt_get_fused(int *fused)
     NEED_INIT();
     if (fused) *fused = mcs_fused_eligible(nullptr) ? 1 : 0;
     return PT_OK;
+}
+
+// ---- NEXT-1: temperature-schedule family and round trips ---------------------------------------------------
+
+int pt_schedule_family(double T_min, double T_max, int n_temps, double phi, double *temps_out, double *betas_out)
+{
+    if (!(T_min > 0.0) || !(T_max >= T_min) || !std::isfinite(T_max) || n_temps < 1 || !(phi > 0.0) || !std::isfinite(phi))
+        return fail(PT_ERR_ARG, "pt_schedule_family: need 0 < T_min <= T_max < inf, n_temps >= 1, 0 < phi < inf");
+    const double T_norm = (n_temps > 1) ? (T_max - T_min) / std::pow((double)(n_temps - 1), phi) : 0.0;     // Eq. (7)
+    for (int i = 0; i < n_temps; ++i) {
+        const double Ti = std::pow((double)i, phi) * T_norm + T_min;                                        // Eq. (6)
+        if (temps_out) temps_out[i] = Ti;
+        if (betas_out) betas_out[i] = 1.0 / Ti;
+    }
+    return PT_OK;
+}
+
+int pt_set_round_trip_tracking(int on)
+{
+    if (!G.bound) return fail(PT_ERR_STATE, "pt_set_round_trip_tracking: no workspace bound");
+    if (G.inited) return fail(PT_ERR_STATE, "pt_set_round_trip_tracking must precede pt_init (the bookkeeping starts at pass 0)");
+    G.track = on ? 1 : 0;
+    return PT_OK;
+}
+
+int pt_get_round_trips(uint32_t *trips, uint64_t *tau_sum, uint64_t *tau_cnt)
+{
+    NEED_INIT();
+    if (!G.P.track) return fail(PT_ERR_STATE, "round-trip tracking is off (pt_set_round_trip_tracking before pt_init)");
+    int rc = PT_OK;
+    if (trips) rc = d2h(trips, G.P.d.rtTrips, (size_t)G.P.S * 2 * G.P.T * 4);
+    if (!rc && tau_sum) rc = d2h(tau_sum, G.P.d.rtSum, (size_t)G.P.S * 2 * 32 * 8);
+    if (!rc && tau_cnt) rc = d2h(tau_cnt, G.P.d.rtCnt, (size_t)G.P.S * 2 * 32 * 8);
+    return rc;
 }
 
 // ---- observables -----------------------------------------------------------------------------------------

@@ -52,3 +52,22 @@ def test_calls_before_init_are_state_errors(lib):
     with pytest.raises(B.PTError) as e:
         B._ck(lib.pt_init(8, 2, 1, 2, b.ctypes.data, 1))
     assert e.value.code == B.PT_ERR_STATE      # nothing bound
+
+
+def test_schedule_family_host_call_matches_oracle_and_closed_forms(lib):
+    """pt_schedule_family is a pure host function (Eq. (6)-(7)): no device needed.  Floating point:
+    both sides evaluate the same two pow() calls in double, so the tolerance is 1 ulp (derived: one rounding each in
+    pow, the product, the sum and the reciprocal; identical operation order on the same libm gives equality)."""
+    from oracle import ref
+
+    for (tmin, tmax, nt, phi) in [(0.2, 1.5, 32, 1.0), (0.2, 1.5, 32, 0.6), (0.2, 1.5, 32, 2.5), (0.1, 3.0, 7, 1.7), (0.5, 0.5, 1, 1.0)]:
+        t, b = B.pt_schedule_family(tmin, tmax, nt, phi)
+        to, bo = ref.schedule_family(tmin, tmax, nt, phi)
+        assert np.all(np.abs(t - to) <= np.spacing(to)) and np.all(np.abs(b - bo) <= np.spacing(bo))
+        assert t[0] == tmin and abs(t[-1] - tmax) <= 2 * np.spacing(tmax)
+    t, _ = B.pt_schedule_family(0.2, 1.5, 32, 1.0)
+    assert np.allclose(t, 0.2 + 1.3 * np.arange(32) / 31, rtol=4e-16, atol=0)        # phi = 1: linear
+    for bad in [(0.0, 1.0, 4, 1.0), (1.0, 0.5, 4, 1.0), (0.2, 1.5, 0, 1.0), (0.2, 1.5, 4, 0.0), (0.2, float("inf"), 4, 1.0)]:
+        with pytest.raises(B.PTError) as e:
+            B.pt_schedule_family(*bad)
+        assert e.value.code == B.PT_ERR_ARG
