@@ -49,6 +49,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--track-round-trips", action="store_true", help="NEXT-1: tunnelling-time bookkeeping in every PT pass")
     return ap.parse_args()
 
 
@@ -157,7 +158,7 @@ def config_of(a, w, n_gpus, sample=None):
              w.name, w.d, w.L, w.S, w.T, w.ladder, w.b_min, w.b_max),
          "mcs_per_step": a.mcs_per_step, "mcs_order": "sweep" + (", houdayer" if w.houdayer else "") + ", exchange",
          "measure_every": w.measure_every, "seed": wl.SEED, "parallelism": "samples sharded x%d" % n_gpus,
-         "l2": "flushed between steps (512 MiB write, untimed)"}
+         "l2": "flushed between steps (512 MiB write, untimed)", "round_trip_tracking": bool(a.track_round_trips)}
     if sample:
         c["sample"] = sample
     return c
@@ -191,7 +192,8 @@ def main():
     dev = torch.device("cuda", local)
 
     # weak scaling: every rank holds the full per-GPU workload on its own range of global sample indices
-    B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED, sample_offset=rank * w.S, device=dev)
+    B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED, sample_offset=rank * w.S, device=dev,
+              track_round_trips=a.track_round_trips)
     flush = torch.empty(512 * 2 ** 20, dtype=torch.uint8, device=dev)
     Qd = torch.empty((w.S, w.T), dtype=torch.int32, device=dev)
     QLd = torch.empty((w.S, w.T), dtype=torch.int32, device=dev)

@@ -49,6 +49,7 @@ def lib():
             "ref_get_energy": [C.c_void_p, C.c_void_p],
             "ref_measure_overlap": [C.c_void_p, C.c_void_p, C.c_void_p],
             "ref_get_swap_counts": [C.c_void_p, C.c_void_p, C.c_void_p],
+            "ref_measure_overlap_profile": [C.c_void_p, C.c_void_p],
             "ref_get_cluster_sizes": [C.c_void_p, C.c_void_p, C.c_void_p],
             "ref_get_perm": [C.c_void_p, C.c_void_p, C.c_void_p],
             "ref_get_spins": [C.c_void_p, C.c_void_p],
@@ -142,6 +143,11 @@ class Oracle:
         QL = np.zeros((self.S, self.T), dtype=np.int32)
         self._ck(lib().ref_measure_overlap(self._h, _p(Q), _p(QL)))
         return Q, QL
+
+    def measure_overlap_profile(self):
+        prof = np.zeros((self.S, self.T, self.d, self.L), dtype=np.int32)
+        self._ck(lib().ref_measure_overlap_profile(self._h, _p(prof)))
+        return prof
 
     def get_swap_counts(self):
         a = np.zeros((self.S, 2, max(self.T - 1, 0)), dtype=np.uint64)

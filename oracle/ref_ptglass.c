@@ -435,6 +435,27 @@ int ref_measure_overlap(const ref_ctx *c, int32_t *Q, int32_t *QL)
     return 0;
 }
 
+/* Overlap profiles (NEXT-2; "the modes for the correlation length"; reading R31): for every axis mu and every
+ * coordinate x along it, the sum of q_i = A_i B_i over the lattice plane x_mu = x.  The Fourier modes of the overlap
+ * field with wave vector along an axis, q(k e_mu) = sum_x prof[mu][x] exp(i k x), are a length-L transform of this. */
+int ref_measure_overlap_profile(const ref_ctx *c, int32_t *prof)
+{
+    if (!c || !prof) return -1;
+    int L = c->L, d = c->d;
+    for (int s = 0; s < c->S; ++s)
+        for (int t = 0; t < c->T; ++t) {
+            const int8_t *A = spins_of(c, s, 0, c->slot_of_temp[rep(c, s, 0, t)]);
+            const int8_t *B = spins_of(c, s, 1, c->slot_of_temp[rep(c, s, 1, t)]);
+            int32_t *out = prof + ((size_t)s * c->T + t) * d * L;
+            for (int k = 0; k < d * L; ++k) out[k] = 0;
+            for (int i = 0; i < c->N; ++i) {
+                int coord[3] = { i % L, (i / L) % L, i / (L * L) };
+                for (int mu = 0; mu < d; ++mu) out[mu * L + coord[mu]] += A[i] * B[i];
+            }
+        }
+    return 0;
+}
+
 int ref_get_swap_counts(const ref_ctx *c, uint64_t *attempts, uint64_t *accepts)
 {
     if (!c) return -1;

@@ -49,6 +49,8 @@ int ref_mcs(ref_ctx *c, int n_mcs, int n_metro, int do_houdayer, int do_exchange
 /* Observables, indexed by TEMPERATURE t. */
 int ref_get_energy(const ref_ctx *c, int32_t *E /* [S][2][T] */);
 int ref_measure_overlap(const ref_ctx *c, int32_t *Q /* [S][T] */, int32_t *QL /* [S][T] or NULL */);
+/* NEXT-2 (reading R31): prof[s][t][mu][x] = sum of q_i over the plane x_mu = x. */
+int ref_measure_overlap_profile(const ref_ctx *c, int32_t *prof /* [S][T][d][L] */);
 int ref_get_swap_counts(const ref_ctx *c, uint64_t *attempts, uint64_t *accepts /* [S][2][T-1] */);
 int ref_get_cluster_sizes(const ref_ctx *c, uint32_t *last, uint64_t *cumulative /* [S][T], may be NULL */);
 int ref_get_perm(const ref_ctx *c, int32_t *temp_of_slot, int32_t *slot_of_temp /* [S][2][T] */);
