@@ -125,6 +125,14 @@ int pt_get_energy(int32_t *E /* [S][2][T]: E of the configuration currently at t
 /* Q = sum_i s1_i s2_i (Eq. (4) x N), QL = sum_{mu,i} q_i q_{i+e_mu} (R14); [S][T] each; QL may be NULL.
  * Consumes no random numbers and advances no counter (R26). */
 int pt_measure_overlap(int32_t *Q, int32_t *QL);
+/* NEXT-2 ("the modes for the correlation length"; R31): overlap profiles
+ * prof[s][t][mu][x] = sum of q_i = s1_i s2_i over the lattice plane x_mu = x, for the two configurations at temperature
+ * t; shape [S][T][d][L], int32.  Every axis sums to Q.  The Fourier modes of the overlap field with wave vector along
+ * an axis, q(k e_mu) = sum_x prof[mu][x] exp(i k x) (k = 2 pi / L for the second-moment correlation length), are a
+ * length-L transform left to the caller; chi_SG = <Q^2>/N from pt_measure_overlap.  Integer only; consumes no random
+ * numbers, advances no counter.  The _device variant takes a DEVICE pointer and does not synchronise. */
+int pt_measure_overlap_profile(int32_t *prof);
+int pt_measure_overlap_profile_device(int32_t *prof_dev);
 int pt_get_swap_counts(uint64_t *attempts, uint64_t *accepts /* [S][2][T-1] since init; either may be NULL */);
 int pt_get_cluster_sizes(uint32_t *last, uint64_t *cumulative /* [S][T]; either may be NULL */);
 int pt_get_perm(int32_t *temp_of_slot, int32_t *slot_of_temp /* [S][2][T] each; either may be NULL */);

@@ -36,6 +36,8 @@ SYMBOLS = {
     "pt_get_round_trips": (_i, [_vp, _vp, _vp]),
     "pt_get_energy": (_i, [_vp]),
     "pt_measure_overlap": (_i, [_vp, _vp]),
+    "pt_measure_overlap_profile": (_i, [_vp]),
+    "pt_measure_overlap_profile_device": (_i, [_vp]),
     "pt_get_swap_counts": (_i, [_vp, _vp]),
     "pt_get_cluster_sizes": (_i, [_vp, _vp]),
     "pt_get_perm": (_i, [_vp, _vp]),
@@ -220,6 +222,16 @@ def pt_get_energy_device(E_dev):
 
 def pt_measure_overlap_device(Q_dev, QL_dev=None):
     _ck(lib().pt_measure_overlap_device(Q_dev.data_ptr(), None if QL_dev is None else QL_dev.data_ptr()))
+
+
+def pt_measure_overlap_profile():
+    prof = np.empty((_shape["S"], _shape["T"], _shape["d"], _shape["L"]), dtype=np.int32)
+    _ck(lib().pt_measure_overlap_profile(_p(prof)))
+    return prof
+
+
+def pt_measure_overlap_profile_device(prof_dev):
+    _ck(lib().pt_measure_overlap_profile_device(prof_dev.data_ptr()))
 
 
 def pt_get_swap_counts():

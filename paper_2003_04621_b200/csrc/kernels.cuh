@@ -26,6 +26,7 @@ struct DevPtrs {
     unsigned long long *cum;    // [S][T]
     int32_t *outE;              // [S][2][T] scratch for observables
     int32_t *outQ, *outQL;      // [S][T]
+    int32_t *outProf;           // [S][T][D][L] overlap profiles (NEXT-2)
     int *mismatch;              // [1]
     int8_t *stage;              // int8 staging for get/set: max(S*2*T*N, S*D*N) bytes
     // round-trip bookkeeping (NEXT-1, R27-R29)
@@ -680,6 +681,41 @@ __global__ void __launch_bounds__(128) k_measure(LAT lat, Params P, int32_t *out
         outQ[(size_t)s * P.T + t] = P.N - 2 * red[0];
         if (outQL) outQL[(size_t)s * P.T + t] = P.D * P.N - 2 * red[1];
     }
+}
+
+// =========================================================================================================
+// NEXT-2  overlap profiles (R31): prof[s][t][mu][x] = sum of q_i over the plane x_mu = x
+//         = L^(D-1) - 2 #(q_i = -1 in that plane).  One CTA per (sample, t); any even L (coordinates from the
+// half-index); only the q = -1 sites touch the shared counters.  dynamic smem: D*L counters.
+// =========================================================================================================
+__global__ void __launch_bounds__(128) k_profile(Params P, int32_t *out)
+{
+    extern __shared__ int pneg[];
+    const int t = blockIdx.x, s = blockIdx.y, tid = threadIdx.x;
+    const int DL = P.D * P.L;
+    for (int i = tid; i < DL; i += blockDim.x) pneg[i] = 0;
+    __syncthreads();
+    const size_t repA = rep_index(P, s, 0, P.d.sot[rep_index(P, s, 0, t)]);
+    const size_t repB = rep_index(P, s, 1, P.d.sot[rep_index(P, s, 1, t)]);
+    for (int id = tid; id < 2 * P.W; id += blockDim.x) {
+        const int p = id / P.W, w = id - p * P.W;
+        uint32_t x = spin_words(P, repA, p)[w] ^ spin_words(P, repB, p)[w];
+        const int left = P.NH - 32 * w;
+        if (left < 32) x &= (1u << left) - 1u;
+        while (x) {
+            const int b = __ffs(x) - 1;
+            x &= x - 1;
+            Coord c;
+            site_of(32 * w + b, p, P.L, P.D, &c);
+            atomicAdd(pneg + c.x, 1);
+            atomicAdd(pneg + P.L + c.y, 1);
+            if (P.D == 3) atomicAdd(pneg + 2 * P.L + c.z, 1);
+        }
+    }
+    __syncthreads();
+    const int plane = P.N / P.L;
+    int32_t *o = out + ((size_t)s * P.T + t) * DL;
+    for (int i = tid; i < DL; i += blockDim.x) o[i] = plane - 2 * pneg[i];
 }
 
 }  // namespace ptg

@@ -185,6 +185,7 @@ size_t carve(void *base, int L, int d, int S, int T, uint32_t strideX, DevPtrs *
     p.outQ = c.take<int32_t>(base, (size_t)S * T);
     p.outQL = c.take<int32_t>(base, (size_t)S * T);
     p.mismatch = c.take<int>(base, 64);
+    p.outProf = c.take<int32_t>(base, (size_t)S * T * d * L);
     p.rtLabel = c.take<uint32_t>(base, R);
     p.rtStart = c.take<uint32_t>(base, R);
     p.rtTrips = c.take<uint32_t>(base, R);
@@ -675,6 +676,27 @@ int pt_measure_overlap(int32_t *Q, int32_t *QL)
     if (rc) return rc;
     if (QL) rc = d2h(QL, G.P.d.outQL, (size_t)G.P.S * G.P.T * 4);
     return rc;
+}
+
+int pt_measure_overlap_profile_device(int32_t *prof_dev)
+{
+    NEED_INIT();
+    if (!prof_dev) return fail(PT_ERR_ARG, "prof is NULL");
+    ProfScope prof(3);
+    dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
+    k_profile<<<grid, 128, (size_t)G.P.D * G.P.L * sizeof(int), G.stream>>>(G.P, prof_dev);
+    ++G.launches;
+    CK(cudaGetLastError());
+    return PT_OK;
+}
+
+int pt_measure_overlap_profile(int32_t *prof)
+{
+    NEED_INIT();
+    if (!prof) return fail(PT_ERR_ARG, "prof is NULL");
+    const int rc = pt_measure_overlap_profile_device(G.P.d.outProf);
+    if (rc) return rc;
+    return d2h(prof, G.P.d.outProf, (size_t)G.P.S * G.P.T * G.P.D * G.P.L * 4);
 }
 
 int pt_get_swap_counts(uint64_t *attempts, uint64_t *accepts)
