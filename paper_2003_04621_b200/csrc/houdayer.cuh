@@ -154,87 +154,20 @@ struct NatLat {
 };
 
 // One pair, one warp.  A0/A1 and B0/B1: the colour-0 / colour-1 words of the two configurations (global or shared
-// memory); Jb: the sample's colour-0 couplings [2D][W]; scratch: 4W words of this warp's shared memory; u: the
+// memory); Jb: the sample's colour-0 couplings [2D][W]; scratch: kPairScratchWords<LAT> words of this warp's shared memory; u: the
 // pair's Philox word (domain 5).  Returns the cluster size; delta = change of E_A (E_B changes by -delta).
 // All lanes return the same values.
-template <class LAT>
-__device__ __forceinline__ int houdayer_pair(const LAT &lat, uint32_t *A0, uint32_t *A1, uint32_t *B0, uint32_t *B1,
-                                             const uint32_t *Jb, uint32_t *scratch, uint32_t u, int lane, int &delta)
+// Common tail of the warp-per-pair paths: the lane holds the cluster bits of its colour words [w_lo, w_hi) in c0 / c1
+// (colour 0 / 1) and its share of the size.  Publishes the cluster in the colour layout to CC (2W words of the warp's
+// shared memory), computes delta = 2 * sum over boundary bonds of J A_i A_j (old spins; each bond seen from its black
+// endpoint) = 2 * (#boundary - 2 #(boundary & unsatisfied)), then negates the cluster in both configurations.
+template <class LAT, int CPT>
+__device__ __forceinline__ int houdayer_apply(const LAT &lat, uint32_t *A0, uint32_t *A1, uint32_t *B0, uint32_t *B1,
+                                              const uint32_t *Jb, uint32_t *CC, const uint32_t (&c0)[CPT],
+                                              const uint32_t (&c1)[CPT], int w_lo, int w_hi, int size, int lane, int &delta)
 {
-    constexpr int D = LAT::D;
-    using NL = NatLat<D, LAT::kLog2L>;
-    constexpr int W = NL::W, NW = NL::NW;
-    constexpr int CPT = (W + 31) / 32;                 // colour words per lane (contiguous chunk)
-    uint32_t *Neg = scratch, *Cl = scratch + NW;
+    constexpr int D = LAT::D, W = LAT::W;
     const unsigned FULL = 0xFFFFFFFFu;
-
-    // q = -1 map in natural order; lane's chunk = colour words [w_lo, w_hi) = natural words [2 w_lo, 2 w_hi)
-    const int w_lo = min(W, lane * CPT), w_hi = min(W, w_lo + CPT);
-    int local = 0;
-    for (int w = w_lo; w < w_hi; ++w) {
-        const uint32_t x0 = A0[w] ^ B0[w], x1 = A1[w] ^ B1[w];
-        const uint32_t n0 = NL::interleave(2 * w, x0, x1), n1 = NL::interleave(2 * w + 1, x0 >> 16, x1 >> 16);
-        Neg[2 * w] = n0; Neg[2 * w + 1] = n1;
-        Cl[2 * w] = 0; Cl[2 * w + 1] = 0;
-        local += __popc(n0) + __popc(n1);
-    }
-    int incl = local;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int v = __shfl_up_sync(FULL, incl, o);
-        if (lane >= o) incl += v;
-    }
-    const int n_neg = __shfl_sync(FULL, incl, 31);
-    delta = 0;
-    if (n_neg == 0) return 0;
-    const int kth = (int)(((unsigned long long)u * (unsigned long long)n_neg) >> 32);
-    const int excl = incl - local;
-    if (kth >= excl && kth < incl) {
-        int rem = kth - excl;
-        for (int n = 2 * w_lo; n < 2 * w_hi; ++n) {
-            const uint32_t x = Neg[n];
-            const int c = __popc(x);
-            if (rem < c) { Cl[n] = 1u << select_bit(x, rem); break; }
-            rem -= c;
-        }
-    }
-    __syncwarp();
-
-    // grow to the fixed point
-    for (;;) {
-        bool changed = false;
-        for (int n = lane; n < NW; n += 32) {
-            const uint32_t neg = Neg[n], cur = Cl[n];
-            if (neg & ~cur) {
-                const uint32_t seeds = (cur | NL::neighbour_union(Cl, n, cur)) & neg;
-                if (seeds) {
-                    const uint32_t nw = NL::fill_runs(neg, seeds);
-                    if (nw != cur) { Cl[n] = nw; changed = true; }
-                }
-            }
-        }
-        __syncwarp();
-        if (!__any_sync(FULL, changed)) break;
-    }
-
-    // cluster in the colour layout, over the (no longer needed) q map: CC[p][w]
-    uint32_t *CC = Neg;
-    int size = 0;
-    uint32_t c0[CPT], c1[CPT];
-#pragma unroll
-    for (int i = 0; i < CPT; ++i) {
-        const int w = w_lo + i;
-        c0[i] = 0; c1[i] = 0;
-        if (w < w_hi) {
-            const uint32_t a = Cl[2 * w], b = Cl[2 * w + 1];
-            size += __popc(a) + __popc(b);
-            uint32_t a0, a1, b0, b1;
-            NL::deinterleave(2 * w, a, a0, a1);
-            NL::deinterleave(2 * w + 1, b, b0, b1);
-            c0[i] = a0 | (b0 << 16);
-            c1[i] = a1 | (b1 << 16);
-        }
-    }
     __syncwarp();
 #pragma unroll
     for (int i = 0; i < CPT; ++i) {
@@ -242,9 +175,6 @@ __device__ __forceinline__ int houdayer_pair(const LAT &lat, uint32_t *A0, uint3
         if (w < w_hi) { CC[w] = c0[i]; CC[W + w] = c1[i]; }
     }
     __syncwarp();
-
-    // delta = 2 * sum over boundary bonds of J A_i A_j = 2 * (#boundary - 2 #(boundary & unsatisfied)), old spins,
-    // each bond seen from its black endpoint
     int dl = 0;
     for (int w = lane; w < W; w += 32) {
         uint32_t nbC[2 * D];
@@ -278,6 +208,102 @@ __device__ __forceinline__ int houdayer_pair(const LAT &lat, uint32_t *A0, uint3
     __syncwarp();
     delta = 2 * dl;
     return size;
+}
+
+// scratch words per warp of houdayer_pair: two padded natural bit maps (NW + one pad word per lane chunk, each)
+template <class LAT>
+constexpr int kPairScratchWords = 2 * (4 * LAT::W / 2 + 32);      // 2 * (NW + NW / CHN) <= 2 * (2W + 32)
+
+template <class LAT>
+__device__ __forceinline__ int houdayer_pair(const LAT &lat, uint32_t *A0, uint32_t *A1, uint32_t *B0, uint32_t *B1,
+                                             const uint32_t *Jb, uint32_t *scratch, uint32_t u, int lane, int &delta)
+{
+    constexpr int D = LAT::D;
+    using NL = NatLat<D, LAT::kLog2L>;
+    constexpr int W = NL::W, NW = NL::NW;
+    constexpr int CPT = (W + 31) / 32;                 // colour words per lane (contiguous chunk)
+    constexpr int CHN = 2 * CPT;                       // natural words per lane
+    // Neg / Cl: natural word n lives at pos(n) = n + n / CHN: one pad word per lane chunk makes the chunk stride odd,
+    // so the 32 lanes walking their chunks in step hit 32 different banks.
+    constexpr int PADDED = NW + NW / CHN;
+    auto pos = [](int n) { return n + n / CHN; };
+    uint32_t *Neg = scratch, *Cl = scratch + PADDED;
+    const unsigned FULL = 0xFFFFFFFFu;
+
+    // q = -1 map in natural order; lane's chunk = colour words [w_lo, w_hi) = natural words [2 w_lo, 2 w_hi)
+    const int w_lo = min(W, lane * CPT), w_hi = min(W, w_lo + CPT);
+    int local = 0;
+    for (int w = w_lo; w < w_hi; ++w) {
+        const uint32_t x0 = A0[w] ^ B0[w], x1 = A1[w] ^ B1[w];
+        const uint32_t n0 = NL::interleave(2 * w, x0, x1), n1 = NL::interleave(2 * w + 1, x0 >> 16, x1 >> 16);
+        Neg[pos(2 * w)] = n0; Neg[pos(2 * w + 1)] = n1;
+        Cl[pos(2 * w)] = 0; Cl[pos(2 * w + 1)] = 0;
+        local += __popc(n0) + __popc(n1);
+    }
+    int incl = local;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(FULL, incl, o);
+        if (lane >= o) incl += v;
+    }
+    const int n_neg = __shfl_sync(FULL, incl, 31);
+    delta = 0;
+    if (n_neg == 0) return 0;
+    const int kth = (int)(((unsigned long long)u * (unsigned long long)n_neg) >> 32);
+    const int excl = incl - local;
+    if (kth >= excl && kth < incl) {
+        int rem = kth - excl;
+        for (int n = 2 * w_lo; n < 2 * w_hi; ++n) {
+            const uint32_t x = Neg[pos(n)];
+            const int c = __popc(x);
+            if (rem < c) { Cl[pos(n)] = 1u << select_bit(x, rem); break; }
+            rem -= c;
+        }
+    }
+    __syncwarp();
+
+    // grow to the fixed point.  Every lane owns a contiguous strip of natural words (whole rows where a row spans
+    // several words) and sweeps it down, then up, in place (Gauss-Seidel inside the strip: membership crosses the whole
+    // strip, and along x the whole row, in one round), reading its neighbours' strips as they are (Jacobi across
+    // strips; chaotic relaxation of a monotone map reaches the same least fixed point in any order).
+    const int n_lo = 2 * w_lo, n_hi = 2 * w_hi;
+    auto ldCl = [Cl](int i) { return Cl[i + i / CHN]; };
+    for (;;) {
+        bool changed = false;
+        for (int k = 0; k < 2 * (n_hi - n_lo) - 1; ++k) {
+            const int n = (k < n_hi - n_lo) ? n_lo + k : n_hi - 2 - (k - (n_hi - n_lo));
+            const uint32_t neg = Neg[pos(n)], cur = Cl[pos(n)];
+            if (neg & ~cur) {
+                const uint32_t seeds = (cur | NL::neighbour_union_f(ldCl, n, cur)) & neg;
+                if (seeds & ~cur) {
+                    Cl[pos(n)] = NL::fill_runs(neg, seeds);
+                    changed = true;
+                }
+            }
+        }
+        __syncwarp();
+        if (!__any_sync(FULL, changed)) break;
+    }
+
+    // cluster in the colour layout, over the (no longer needed) q map: CC[p][w]
+    uint32_t *CC = Neg;
+    int size = 0;
+    uint32_t c0[CPT], c1[CPT];
+#pragma unroll
+    for (int i = 0; i < CPT; ++i) {
+        const int w = w_lo + i;
+        c0[i] = 0; c1[i] = 0;
+        if (w < w_hi) {
+            const uint32_t a = Cl[pos(2 * w)], b = Cl[pos(2 * w + 1)];
+            size += __popc(a) + __popc(b);
+            uint32_t a0, a1, b0, b1;
+            NL::deinterleave(2 * w, a, a0, a1);
+            NL::deinterleave(2 * w + 1, b, b0, b1);
+            c0[i] = a0 | (b0 << 16);
+            c1[i] = a1 | (b1 << 16);
+        }
+    }
+    return houdayer_apply<LAT, CPT>(lat, A0, A1, B0, B1, Jb, CC, c0, c1, w_lo, w_hi, size, lane, delta);
 }
 
 }  // namespace ptg

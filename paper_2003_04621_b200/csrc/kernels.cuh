@@ -7,7 +7,7 @@
 
 #include "lattice.cuh"
 #include "philox.cuh"
-#include "houdayer.cuh"
+#include "houdayer_rows.cuh"
 
 namespace ptg {
 
@@ -616,7 +616,7 @@ __global__ void __launch_bounds__(128) k_houdayer_gen(LAT lat, Params P, uint32_
 
 // =========================================================================================================
 // a5  Houdayer cluster exchange, FAST path: one warp per (sample, t) pair (houdayer.cuh).
-// grid: ceil(S*T / warps per CTA); dynamic smem: 4W words per warp.
+// grid: ceil(S*T / warps per CTA); dynamic smem: kPairScratchWords<LAT> words per warp.
 // =========================================================================================================
 template <class LAT>
 __global__ void __launch_bounds__(256) k_houdayer(LAT lat, Params P, uint32_t step)
@@ -631,8 +631,8 @@ __global__ void __launch_bounds__(256) k_houdayer(LAT lat, Params P, uint32_t st
     uint32_t u, o1, o2, o3;
     philox4x32_10(0u, step, P.g0 + (uint32_t)s, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
     int delta;
-    const int size = houdayer_pair(lat, spin_words(P, repA, 0), spin_words(P, repA, 1), spin_words(P, repB, 0),
-                                   spin_words(P, repB, 1), J_words(P, s, 0, 0), hsm + (size_t)wib * 4 * LAT::W, u, lane, delta);
+    const int size = houdayer_warp(lat, spin_words(P, repA, 0), spin_words(P, repA, 1), spin_words(P, repB, 0),
+                                   spin_words(P, repB, 1), J_words(P, s, 0, 0), hsm + (size_t)wib * kPairScratchWords<LAT>, u, lane, delta);
     if (lane == 0) {
         if (delta) { P.d.E[repA] += delta; P.d.E[repB] -= delta; }
         P.d.last[pair] = (uint32_t)size;

@@ -48,7 +48,7 @@ struct McsSmem {
             const int groups = (T + 31) / 32;
             o += (groups < nwarps ? groups : nwarps) * 2 * (2 * W) * kLaneStride;
         } else {
-            o += nwarps * 4 * W;
+            o += nwarps * (4 * W + 64);         // kPairScratchWords
         }
         words = o;
     }
@@ -146,13 +146,13 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                 }
             } else {
                 // one WARP per temperature
-                uint32_t *scratch = msm + L.oScr + wid * 4 * W;
+                uint32_t *scratch = msm + L.oScr + wid * kPairScratchWords<LAT>;
                 for (int t = wid; t < T; t += NWARPS) {
                     const int ra = sSot[t], rb = T + sSot[T + t];
                     uint32_t u, o1, o2, o3;
                     philox4x32_10(0u, step, g, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
                     int delta;
-                    const int size = houdayer_pair(lat, sS + ra * RS, sS + ra * RS + W, sS + rb * RS, sS + rb * RS + W, sJ,
+                    const int size = houdayer_warp(lat, sS + ra * RS, sS + ra * RS + W, sS + rb * RS, sS + rb * RS + W, sJ,
                                                    scratch, u, lane, delta);
                     if (lane == 0) {
                         sE[ra] += delta;

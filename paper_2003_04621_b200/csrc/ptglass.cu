@@ -306,10 +306,10 @@ cudaError_t launch_houdayer()
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
         if constexpr (LAT::kFast) {
-            // one warp per pair; 4W words of shared memory per warp
+            // one warp per pair; kPairScratchWords words of shared memory per warp
             int wpb = 8;
-            while (wpb > 1 && (size_t)wpb * 4 * G.P.W * 4 > 96 * 1024) wpb >>= 1;
-            const size_t smem = (size_t)wpb * 4 * G.P.W * 4;
+            while (wpb > 1 && (size_t)wpb * kPairScratchWords<LAT> * 4 > 96 * 1024) wpb >>= 1;
+            const size_t smem = (size_t)wpb * kPairScratchWords<LAT> * 4;
             err = allow_smem(k_houdayer<LAT>, smem);
             if (err != cudaSuccess) return;
             const long pairs = (long)G.P.S * G.P.T;
