@@ -619,7 +619,7 @@ __global__ void __launch_bounds__(128) k_houdayer_gen(LAT lat, Params P, uint32_
 // grid: ceil(S*T / warps per CTA); dynamic smem: kPairScratchWords<LAT> words per warp.
 // =========================================================================================================
 template <class LAT>
-__global__ void __launch_bounds__(256) k_houdayer(LAT lat, Params P, uint32_t step)
+__global__ void __launch_bounds__(128, 6) k_houdayer(LAT lat, Params P, uint32_t step)
 {
     extern __shared__ uint32_t hsm[];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, wpb = blockDim.x >> 5;

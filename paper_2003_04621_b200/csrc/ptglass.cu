@@ -307,7 +307,7 @@ cudaError_t launch_houdayer()
         using LAT = decltype(lat);
         if constexpr (LAT::kFast) {
             // one warp per pair; kPairScratchWords words of shared memory per warp
-            int wpb = 8;
+            int wpb = 4;
             while (wpb > 1 && (size_t)wpb * kPairScratchWords<LAT> * 4 > 96 * 1024) wpb >>= 1;
             const size_t smem = (size_t)wpb * kPairScratchWords<LAT> * 4;
             err = allow_smem(k_houdayer<LAT>, smem);
