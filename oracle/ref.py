@@ -35,6 +35,8 @@ def lib():
         L = C.CDLL(build())
         L.ref_create.restype = C.c_void_p
         L.ref_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_uint64, C.c_uint32]
+        L.ref_create_p.restype = C.c_void_p
+        L.ref_create_p.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_uint64, C.c_uint32, C.c_double]
         L.ref_destroy.argtypes = [C.c_void_p]
         L.ref_destroy.restype = None
         L.ref_threshold.restype = C.c_uint32
@@ -97,12 +99,15 @@ def _p(a):
 class Oracle:
     """One oracle simulation.  Mirrors the product's call names (pt_* -> methods) so one harness drives both."""
 
-    def __init__(self, L, d, n_samples, n_temps, betas, seed, sample_offset=0):
+    def __init__(self, L, d, n_samples, n_temps, betas, seed, sample_offset=0, p_ferro=None):
         b = np.ascontiguousarray(betas, dtype=np.float64)
         assert b.shape == (n_temps,)
         self.L, self.d, self.S, self.T = L, d, n_samples, n_temps
         self.N = L ** d
-        self._h = lib().ref_create(L, d, n_samples, n_temps, b.ctypes.data, seed, sample_offset)
+        if p_ferro is None:
+            self._h = lib().ref_create(L, d, n_samples, n_temps, b.ctypes.data, seed, sample_offset)
+        else:
+            self._h = lib().ref_create_p(L, d, n_samples, n_temps, b.ctypes.data, seed, sample_offset, float(p_ferro))
         if not self._h:
             raise ValueError("ref_create rejected the arguments")
 

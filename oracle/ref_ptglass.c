@@ -145,6 +145,14 @@ static void recompute_all(ref_ctx *c)
 
 ref_ctx *ref_create(int L, int d, int S, int T, const double *betas, uint64_t seed, uint32_t sample_offset)
 {
+    return ref_create_p(L, d, S, T, betas, seed, sample_offset, 0.5);
+}
+
+/* Eq. (2) with general p (reading R32): J = +1 iff w < floor(p * 2^32) for the bond's Philox word w. */
+ref_ctx *ref_create_p(int L, int d, int S, int T, const double *betas, uint64_t seed, uint32_t sample_offset, double p_ferro)
+{
+    if (!(p_ferro >= 0.0) || !(p_ferro <= 1.0)) return NULL;
+    const uint64_t thrJ = (uint64_t)floor(ldexp(p_ferro, 32));
     if (d != 2 && d != 3) return NULL;
     if (L < 2 || (L & 1)) return NULL;
     if (S < 1 || T < 1 || T > 65535 || betas == NULL) return NULL;
@@ -186,7 +194,8 @@ ref_ctx *ref_create(int L, int d, int S, int T, const double *betas, uint64_t se
         /* 1. couplings: domain 1, p = 1/2 exactly (Eq. (2)) */
         for (int mu = 0; mu < d; ++mu)
             for (int i = 0; i < c->N; ++i)
-                c->J[((size_t)s * d + mu) * N + i] = sign_of(draw(c, (uint32_t)i >> 2, 0, g, 1, mu, 0, 0, i & 3));
+                c->J[((size_t)s * d + mu) * N + i] =
+                    ((uint64_t)draw(c, (uint32_t)i >> 2, 0, g, 1, mu, 0, 0, i & 3) < thrJ) ? (int8_t)1 : (int8_t)-1;
         /* 2. spins: domain 2 (R17);  3. identity permutations */
         for (int ch = 0; ch < 2; ++ch)
             for (int r = 0; r < T; ++r) {

@@ -37,6 +37,10 @@ uint32_t ref_threshold(double x);
  * (d not in {2,3}, L odd or < 2, S < 1, T < 1 or > 65535, betas NULL / negative / non-finite). */
 ref_ctx *ref_create(int L, int d, int n_samples, int n_temps, const double *betas, uint64_t seed,
                     uint32_t sample_offset);
+/* Same with the bimodal distribution of Eq. (2) for general p = P(J = +1) (NEXT-4, reading R32):
+ * J = +1 iff the bond's Philox word w < floor(p * 2^32); p = 1/2 is ref_create exactly.  NULL unless 0 <= p <= 1. */
+ref_ctx *ref_create_p(int L, int d, int n_samples, int n_temps, const double *betas, uint64_t seed,
+                      uint32_t sample_offset, double p_ferro);
 void ref_destroy(ref_ctx *c);
 
 /* Updates: Metropolis sweeps, PT pass (Eq. (5)),
