@@ -68,6 +68,10 @@ int pt_init(int L, int d, int n_samples, int n_temps, const double *betas, uint6
 int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas, uint64_t seed,
                   uint32_t sample_offset);
 int pt_free(void);
+/* NEXT-4: the bimodal distribution of Eq. (2) for general p = P(J = +1) (R32).  J[s][mu][i] = +1
+ * iff the bond's Philox word (domain 1) w < floor(p * 2^32); the default p = 1/2 is the sign-bit rule above, bit for bit.
+ * Call after pt_bind and BEFORE pt_init (PT_ERR_STATE otherwise); PT_ERR_ARG unless 0 <= p <= 1. */
+int pt_set_coupling_probability(double p_ferro);
 
 /* ---- updates -------------------------------------------------------------------------------- */
 

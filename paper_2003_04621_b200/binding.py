@@ -33,6 +33,7 @@ SYMBOLS = {
     "pt_get_fused": (_i, [_vp]),
     "pt_schedule_family": (_i, [C.c_double, C.c_double, _i, C.c_double, _vp, _vp]),
     "pt_set_round_trip_tracking": (_i, [_i]),
+    "pt_set_coupling_probability": (_i, [C.c_double]),
     "pt_get_round_trips": (_i, [_vp, _vp, _vp]),
     "pt_get_energy": (_i, [_vp]),
     "pt_measure_overlap": (_i, [_vp, _vp]),
@@ -142,7 +143,7 @@ def pt_free():
 
 
 def pt_open(L, d, n_samples, n_temps, betas, seed, sample_offset=0, device="cuda:0", stream=None, general=False,
-            track_round_trips=False):
+            track_round_trips=False, p_ferro=None):
     """Convenience: allocate the workspace with torch, bind it and initialise.  Returns the workspace tensor."""
     import torch
 
@@ -153,6 +154,8 @@ def pt_open(L, d, n_samples, n_temps, betas, seed, sample_offset=0, device="cuda
             pt_force_general_path(0)
         if track_round_trips:
             pt_set_round_trip_tracking(1)
+        if p_ferro is not None:
+            pt_set_coupling_probability(p_ferro)
         pt_init(L, d, n_samples, n_temps, betas, seed, sample_offset)
     return ws
 
@@ -163,6 +166,10 @@ def pt_schedule_family(T_min, T_max, n_temps, phi):
     b = np.zeros(max(n_temps, 0), dtype=np.float64)
     _ck(lib().pt_schedule_family(float(T_min), float(T_max), int(n_temps), float(phi), _p(t), _p(b)))
     return t, b
+
+
+def pt_set_coupling_probability(p_ferro):
+    _ck(lib().pt_set_coupling_probability(float(p_ferro)))
 
 
 def pt_set_round_trip_tracking(on):

@@ -39,6 +39,7 @@ struct Params {
     uint32_t g0;                // sample_offset: global sample index = g0 + s
     uint32_t strideX;
     int track;                  // 1: round-trip bookkeeping after every PT pass
+    unsigned long long thrJ;    // J = +1 iff Philox word < thrJ = floor(p * 2^32)  (Eq. (2), R32); 2^31 for p = 1/2
     RoundKeys rk;
     DevPtrs d;
 };
@@ -69,7 +70,7 @@ __global__ void k_draw_couplings(Params P)
         philox4x32_10((uint32_t)i4, 0u, P.g0 + (uint32_t)s, make_tag(DOM_J, mu, 0, 0), P.rk, w[0], w[1], w[2], w[3]);
         int8_t *dst = P.d.stage + ((size_t)s * P.D + mu) * P.N + 4 * (size_t)i4;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) dst[j] = (w[j] >> 31) ? -1 : 1;
+        for (int j = 0; j < 4; ++j) dst[j] = ((unsigned long long)w[j] < P.thrJ) ? 1 : -1;
     }
 }
 

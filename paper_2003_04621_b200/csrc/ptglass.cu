@@ -27,6 +27,7 @@ struct Context {
     int force_general = -1;
     int fused_mode = -1;        // -1: fused pt_mcs where eligible, 0: always separate launches
     int track = 0;              // round-trip bookkeeping (NEXT-1), chosen before pt_init
+    double p_ferro = 0.5;       // P(J = +1) of Eq. (2) (NEXT-4), chosen before pt_init
     bool fast = false;
     Params P{};
     std::vector<double> betas;
@@ -476,6 +477,7 @@ int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas,
     P.rk = make_round_keys((uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32));
     P.strideX = swap_stride(G.betas, d, P.N);
     P.track = G.track;
+    P.thrJ = (unsigned long long)std::floor(std::ldexp(G.p_ferro, 32));
     const size_t need = carve(G.ws, L, d, n_samples, n_temps, P.strideX, &P.d, &G.stage_bytes);
     if (need > G.ws_bytes)
         return fail(PT_ERR_STATE, "workspace too small: %zu bytes bound, %zu needed", G.ws_bytes, need);
@@ -616,6 +618,15 @@ int pt_schedule_family(double T_min, double T_max, int n_temps, double phi, doub
         if (temps_out) temps_out[i] = Ti;
         if (betas_out) betas_out[i] = 1.0 / Ti;
     }
+    return PT_OK;
+}
+
+int pt_set_coupling_probability(double p_ferro)
+{
+    if (!G.bound) return fail(PT_ERR_STATE, "pt_set_coupling_probability: no workspace bound");
+    if (G.inited) return fail(PT_ERR_STATE, "pt_set_coupling_probability must precede pt_init (couplings are drawn there)");
+    if (!(p_ferro >= 0.0) || !(p_ferro <= 1.0)) return fail(PT_ERR_ARG, "p must be in [0, 1]");
+    G.p_ferro = p_ferro;
     return PT_OK;
 }
 

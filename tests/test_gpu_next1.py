@@ -82,3 +82,35 @@ def test_full_size_C2_round_trips_sampled():
         o.mcs(150, 1, True, True)
         to, so, co = o.get_round_trips()
         assert np.array_equal(to[0], trips[g]) and np.array_equal(so[0], tau_sum[g]) and np.array_equal(co[0], tau_cnt[g])
+
+
+# ---- NEXT-4: general p in Eq. (2) ------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("p", [0.0, 0.3, 0.5, 0.85, 1.0])
+def test_general_p_couplings_and_dynamics_match_oracle(p):
+    L, d, S, T = 16, 2, 3, 4
+    betas = wl.betas_geometric(0.3, 1.2, T)
+    o = ref.Oracle(L, d, S, T, betas, wl.SEED, 1, p_ferro=p)
+    B.pt_open(L, d, S, T, betas, wl.SEED, 1, p_ferro=p)
+    assert np.array_equal(o.get_couplings(), B.pt_get_couplings())
+    o.mcs(12, 1, True, True); B.pt_mcs(12, 1, True, True)
+    a, b = o.state(), B.state()
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+    assert B.pt_recompute_energy()[1] == 0
+    if p == 0.5:
+        o2 = ref.Oracle(L, d, S, T, betas, wl.SEED, 1)
+        assert np.array_equal(o2.get_couplings(), B.pt_get_couplings())
+
+
+def test_general_p_argument_and_state_errors():
+    B.pt_open(8, 2, 1, 2, wl.betas_linear(0.2, 1.0, 2), wl.SEED)
+    with pytest.raises(B.PTError) as e:
+        B.pt_set_coupling_probability(0.3)                   # after pt_init
+    assert e.value.code == B.PT_ERR_STATE
+    import torch
+    ws = torch.empty(B.pt_workspace_bytes(8, 2, 1, 2), dtype=torch.uint8, device="cuda:0")
+    B.pt_bind(ws)
+    with pytest.raises(B.PTError) as e:
+        B.pt_set_coupling_probability(1.5)
+    assert e.value.code == B.PT_ERR_ARG
