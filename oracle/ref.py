@@ -61,6 +61,8 @@ def lib():
             "ref_set_spins": [C.c_void_p, C.c_void_p],
             "ref_set_couplings": [C.c_void_p, C.c_void_p],
             "ref_recompute_energy": [C.c_void_p, C.c_void_p, C.c_void_p],
+            "ref_set_couplings_fixed": [C.c_void_p, C.c_void_p, C.c_int],
+            "ref_get_couplings_fixed": [C.c_void_p, C.c_void_p, C.c_void_p],
             "ref_get_round_trips": [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p],
             "ref_schedule_family": [C.c_double, C.c_double, C.c_int, C.c_double, C.c_void_p, C.c_void_p],
         }.items():
@@ -209,6 +211,17 @@ class Oracle:
         tau_cnt = np.zeros((self.S, 2, 32), dtype=np.uint64)
         self._ck(lib().ref_get_round_trips(self._h, _p(trips), _p(tau_sum), _p(tau_cnt)))
         return trips, tau_sum, tau_cnt
+
+    def set_couplings_fixed(self, Jq, fbits):
+        j = np.ascontiguousarray(Jq, dtype=np.int32)
+        assert j.shape == (self.S, self.d, self.N)
+        self._ck(lib().ref_set_couplings_fixed(self._h, _p(j), int(fbits)))
+
+    def get_couplings_fixed(self):
+        j = np.zeros((self.S, self.d, self.N), dtype=np.int32)
+        f = C.c_int()
+        self._ck(lib().ref_get_couplings_fixed(self._h, _p(j), C.byref(f)))
+        return j, f.value
 
     def recompute_energy(self):
         E = np.zeros((self.S, 2, self.T), dtype=np.int32)

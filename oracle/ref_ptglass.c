@@ -23,6 +23,8 @@ struct ref_ctx {
     uint32_t sample_offset;
     double *betas;        /* [T] */
     int8_t *J;            /* [S][d][N]       J[mu][i] = bond i -> i+e_mu */
+    int32_t *Jq;          /* [S][d][N]       fixed-point couplings J = Jq * 2^-fbits (NEXT-3, R33), or NULL */
+    int fbits;            /* fractional bits of Jq; -1 in the +-J model */
     int8_t *spin;         /* [S][2][T][N]    slot order */
     int32_t *E;           /* [S][2][T]       slot order */
     int32_t *temp_of_slot;/* [S][2][T] */
@@ -94,6 +96,28 @@ static uint32_t thrX_of(const ref_ctx *c, int t, long m)
     return ref_threshold(-(fabs(c->betas[t + 1] - c->betas[t]) * (double)(4 * m)));
 }
 
+/* coupling of bond (mu, i) of sample s as an integer: +-1, or Jq in the fixed-point model (NEXT-3, R33) */
+static long jval(const ref_ctx *c, int s, int mu, int i)
+{
+    size_t k = ((size_t)s * c->d + mu) * c->N + i;
+    return c->Jq ? (long)c->Jq[k] : (long)c->J[k];
+}
+
+/* Metropolis threshold for a flip with a = s_i h_i > 0 (Delta E = 2a) at temperature index t:
+ * +-J: the table thrM[t][a/2];  fixed point (R34): THR(-(beta_t * ldexp((double)(2a), -fbits))), double exp. */
+static uint32_t thr_flip(const ref_ctx *c, int t, long a)
+{
+    if (!c->Jq) return c->thrM[t * c->d + (a / 2 - 1)];
+    return ref_threshold(-(c->betas[t] * ldexp((double)(2 * a), -c->fbits)));
+}
+
+/* swap threshold for |dE| at pair t: +-J: THR(-(|dbeta| * 4m)), m = |dE|/4;  fixed point (R34): THR(-(|dbeta| * ldexp(|dE|, -fbits))) */
+static uint32_t thr_swap(const ref_ctx *c, int t, long absdE)
+{
+    if (!c->Jq) return thrX_of(c, t, absdE / 4);
+    return ref_threshold(-(fabs(c->betas[t + 1] - c->betas[t]) * ldexp((double)absdE, -c->fbits)));
+}
+
 /* ---------------------------------------------------------------- lattice */
 
 static void build_neighbours(ref_ctx *c)
@@ -118,13 +142,13 @@ static int colour_of(const ref_ctx *c, int i)
 }
 
 /* E = -sum_{mu<d} sum_i J[mu][i] s_i s_{i+e_mu}   (Eq. (1) with H = 0; R3: both bonds counted at L=2) */
-static int32_t energy_of(const ref_ctx *c, const int8_t *J, const int8_t *s)
+static int32_t energy_of(const ref_ctx *c, int smp, const int8_t *s)
 {
-    int32_t e = 0;
+    long e = 0;
     for (int mu = 0; mu < c->d; ++mu)
         for (int i = 0; i < c->N; ++i)
-            e -= J[mu * c->N + i] * s[i] * s[c->nbr[i * 2 * c->d + 2 * mu]];
-    return e;
+            e -= jval(c, smp, mu, i) * s[i] * s[c->nbr[i * 2 * c->d + 2 * mu]];
+    return (int32_t)e;
 }
 
 static int8_t *spins_of(const ref_ctx *c, int s, int ch, int r)
@@ -138,7 +162,7 @@ static void recompute_all(ref_ctx *c)
     for (int s = 0; s < c->S; ++s)
         for (int ch = 0; ch < 2; ++ch)
             for (int r = 0; r < c->T; ++r)
-                c->E[rep(c, s, ch, r)] = energy_of(c, c->J + (size_t)s * c->d * c->N, spins_of(c, s, ch, r));
+                c->E[rep(c, s, ch, r)] = energy_of(c, s, spins_of(c, s, ch, r));
 }
 
 /* ---------------------------------------------------------------- init (8(c).2) */
@@ -165,6 +189,7 @@ ref_ctx *ref_create_p(int L, int d, int S, int T, const double *betas, uint64_t 
     ref_ctx *c = (ref_ctx *)calloc(1, sizeof(ref_ctx));
     c->L = L; c->d = d; c->S = S; c->T = T; c->seed = seed; c->sample_offset = sample_offset;
     c->N = (d == 2) ? L * L : L * L * L;
+    c->Jq = NULL; c->fbits = -1;
     size_t R = (size_t)S * 2 * T, N = (size_t)c->N;
     c->betas = (double *)malloc(sizeof(double) * T);
     memcpy(c->betas, betas, sizeof(double) * T);
@@ -223,6 +248,7 @@ ref_ctx *ref_create_p(int L, int d, int S, int T, const double *betas, uint64_t 
 void ref_destroy(ref_ctx *c)
 {
     if (!c) return;
+    free(c->Jq);
     free(c->betas); free(c->J); free(c->spin); free(c->E); free(c->temp_of_slot); free(c->slot_of_temp);
     free(c->thrM); free(c->sgn); free(c->attempts); free(c->accepts); free(c->last_size); free(c->cum_size);
     free(c->rt_label); free(c->rt_start); free(c->rt_trips); free(c->rt_tau_sum); free(c->rt_tau_cnt);
@@ -241,23 +267,22 @@ int ref_sweep(ref_ctx *c, int n)
         for (int p = 0; p < 2; ++p)                       /* black (x+y+z even) first, then white */
             for (int s = 0; s < c->S; ++s) {
                 uint32_t g = c->sample_offset + (uint32_t)s;
-                const int8_t *J = c->J + (size_t)s * d * N;
                 for (int ch = 0; ch < 2; ++ch)
                     for (int r = 0; r < c->T; ++r) {
                         int8_t *sp = spins_of(c, s, ch, r);
                         int t = c->temp_of_slot[rep(c, s, ch, r)];
                         for (int i = 0; i < N; ++i) {
                             if (colour_of(c, i) != p) continue;
-                            int h = 0;
+                            long h = 0;
                             for (int mu = 0; mu < d; ++mu) {
                                 int up = c->nbr[i * 2 * d + 2 * mu], dn = c->nbr[i * 2 * d + 2 * mu + 1];
-                                h += J[mu * N + i] * sp[up] + J[mu * N + dn] * sp[dn];
+                                h += jval(c, s, mu, i) * sp[up] + jval(c, s, mu, dn) * sp[dn];
                             }
-                            int a = sp[i] * h;            /* Delta E = 2a */
+                            long a = sp[i] * h;           /* Delta E = 2a */
                             uint32_t u = draw(c, (uint32_t)i >> 3, c->n_sweep, g, 3, p, ch, r, (i >> 1) & 3);
-                            if (a <= 0 || u < c->thrM[t * d + (a / 2 - 1)]) {
+                            if (a <= 0 || u < thr_flip(c, t, a)) {
                                 sp[i] = (int8_t)-sp[i];
-                                c->E[rep(c, s, ch, r)] += 2 * a;
+                                c->E[rep(c, s, ch, r)] += (int32_t)(2 * a);
                             }
                         }
                     }
@@ -283,11 +308,11 @@ int ref_exchange(ref_ctx *c)
             for (int t = 0; t + 1 < T; ++t) {
                 int ra = sot[t], rb = sot[t + 1];
                 long dE = (long)E[ra] - (long)E[rb];      /* multiple of 4 (R22b) */
-                if (dE % 4 != 0) abort();
+                if (!c->Jq && dE % 4 != 0) abort();
                 uint32_t u = draw(c, (uint32_t)t, c->n_exchange, g, 4, 0, ch, 0, 0);
                 size_t k = ((size_t)s * 2 + ch) * (T - 1) + t;
                 c->attempts[k] += 1;
-                if (c->sgn[t] * dE <= 0 || u < thrX_of(c, t, labs(dE) / 4)) {
+                if (c->sgn[t] * dE <= 0 || u < thr_swap(c, t, labs(dE))) {
                     sot[t] = rb; sot[t + 1] = ra; tos[ra] = t + 1; tos[rb] = t;
                     c->accepts[k] += 1;
                 }
@@ -352,7 +377,6 @@ int ref_houdayer(ref_ctx *c)
     int d = c->d, N = c->N, T = c->T;
     for (int s = 0; s < c->S; ++s) {
         uint32_t g = c->sample_offset + (uint32_t)s;
-        const int8_t *J = c->J + (size_t)s * d * N;
         for (int t = 0; t < T; ++t) {
             int ra = c->slot_of_temp[rep(c, s, 0, t)], rb = c->slot_of_temp[rep(c, s, 1, t)];
             int8_t *A = spins_of(c, s, 0, ra), *B = spins_of(c, s, 1, rb);
@@ -380,8 +404,8 @@ int ref_houdayer(ref_ctx *c)
                 if (!c->mark[i]) continue;
                 for (int mu = 0; mu < d; ++mu) {
                     int up = c->nbr[i * 2 * d + 2 * mu], dn = c->nbr[i * 2 * d + 2 * mu + 1];
-                    if (!c->mark[up]) delta += 2 * J[mu * N + i] * A[i] * A[up];
-                    if (!c->mark[dn]) delta += 2 * J[mu * N + dn] * A[i] * A[dn];
+                    if (!c->mark[up]) delta += (int32_t)(2 * jval(c, s, mu, i) * A[i] * A[up]);
+                    if (!c->mark[dn]) delta += (int32_t)(2 * jval(c, s, mu, dn) * A[i] * A[dn]);
                 }
             }
             for (int i = 0; i < N; ++i)
@@ -548,6 +572,35 @@ int ref_set_couplings(ref_ctx *c, const int8_t *J)
     return 0;
 }
 
+/* NEXT-3 (readings R33-R35): replace the couplings by fixed-point values J = Jq * 2^-fbits (e.g. a
+ * rounded standard normal sample, an INPUT of the run) and recompute the energies.  From here on the sweeps, the PT pass
+ * and the cluster move use integer fields / energy differences in units of 2^-fbits and evaluate the acceptance
+ * probabilities with double exp (thr_flip, thr_swap).  d * N * max|Jq| must stay below 2^31 (int32 energies). */
+int ref_set_couplings_fixed(ref_ctx *c, const int32_t *Jq, int fbits)
+{
+    if (!c || !Jq || fbits < 0 || fbits > 24) return -1;
+    size_t n = (size_t)c->S * c->d * c->N;
+    long maxabs = 0;
+    for (size_t k = 0; k < n; ++k) {
+        long v = Jq[k] < 0 ? -(long)Jq[k] : (long)Jq[k];
+        if (v > maxabs) maxabs = v;
+    }
+    if ((double)maxabs * (double)c->d * (double)c->N >= 2147483648.0) return -1;
+    if (!c->Jq) c->Jq = (int32_t *)malloc(n * sizeof(int32_t));
+    memcpy(c->Jq, Jq, n * sizeof(int32_t));
+    c->fbits = fbits;
+    recompute_all(c);
+    return 0;
+}
+
+int ref_get_couplings_fixed(const ref_ctx *c, int32_t *Jq, int *fbits)
+{
+    if (!c || !c->Jq) return -1;
+    if (Jq) memcpy(Jq, c->Jq, (size_t)c->S * c->d * c->N * sizeof(int32_t));
+    if (fbits) *fbits = c->fbits;
+    return 0;
+}
+
 int ref_recompute_energy(const ref_ctx *c, int32_t *E_slot_order, int *mismatch_count)
 {
     if (!c) return -1;
@@ -555,7 +608,7 @@ int ref_recompute_energy(const ref_ctx *c, int32_t *E_slot_order, int *mismatch_
     for (int s = 0; s < c->S; ++s)
         for (int ch = 0; ch < 2; ++ch)
             for (int r = 0; r < c->T; ++r) {
-                int32_t e = energy_of(c, c->J + (size_t)s * c->d * c->N, spins_of(c, s, ch, r));
+                int32_t e = energy_of(c, s, spins_of(c, s, ch, r));
                 if (E_slot_order) E_slot_order[rep(c, s, ch, r)] = e;
                 bad += (e != c->E[rep(c, s, ch, r)]);
             }

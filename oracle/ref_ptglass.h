@@ -77,6 +77,10 @@ int ref_get_thresholds(const ref_ctx *c, uint32_t *thrM /* [T][d], k = 1..d at [
 int ref_get_counters(const ref_ctx *c, uint32_t *n_sweep, uint32_t *n_exchange, uint32_t *n_houdayer);
 int ref_set_spins(ref_ctx *c, const int8_t *spins);
 int ref_set_couplings(ref_ctx *c, const int8_t *J);
+/* NEXT-3 (readings R33-R35): couplings as fixed-point numbers J = Jq * 2^-fbits, [S][d][N].
+ * -1 if fbits not in [0, 24] or d*N*max|Jq| >= 2^31. */
+int ref_set_couplings_fixed(ref_ctx *c, const int32_t *Jq, int fbits);
+int ref_get_couplings_fixed(const ref_ctx *c, int32_t *Jq, int *fbits);
 int ref_recompute_energy(const ref_ctx *c, int32_t *E_slot_order /* [S][2][T] or NULL */, int *mismatch_count);
 
 #ifdef __cplusplus

@@ -28,6 +28,17 @@ def betas_geometric(b_min: float, b_max: float, T: int) -> np.ndarray:
     return np.array([b_min * pow(b_max / b_min, t / (T - 1)) for t in range(T)], dtype=np.float64)
 
 
+def gaussian_couplings_fixed(seed: int, S: int, d: int, N: int, fbits: int = 16, sample_offset: int = 0) -> np.ndarray:
+    """Standard-normal couplings rounded to fixed point, int32 [S][d][N], J = Jq * 2^-fbits.  An INPUT of a
+    run (a disorder sample), drawn per global sample index with numpy's PCG64 so that shards agree; no arithmetic of the
+    method lives here."""
+    out = np.empty((S, d, N), dtype=np.int32)
+    for s in range(S):
+        rng = np.random.default_rng([seed, sample_offset + s, 7])
+        out[s] = np.rint(rng.standard_normal((d, N)) * (1 << fbits)).astype(np.int32)
+    return out
+
+
 @dataclass(frozen=True)
 class Workload:
     name: str

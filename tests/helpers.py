@@ -81,9 +81,11 @@ def _enumerate(J, betas, L, d):
     N = L ** d
     states = ((np.arange(1 << N)[:, None] >> np.arange(N)[None, :]) & 1).astype(np.int8) * 2 - 1
     nbr = neighbour_list(L, d)
-    E = np.zeros(1 << N, dtype=np.int64)
+    Jt = np.asarray(J)
+    acc = np.float64 if np.issubdtype(Jt.dtype, np.floating) else np.int64      # real couplings: NEXT-3
+    E = np.zeros(1 << N, dtype=acc)
     for mu in range(d):
-        E -= (J[mu][None, :].astype(np.int64) * states * states[:, nbr[:, 2 * mu]]).sum(axis=1)
+        E -= (Jt[mu][None, :].astype(acc) * states * states[:, nbr[:, 2 * mu]]).sum(axis=1)
     Em, q2 = [], []
     sf = states.astype(np.float64)
     for b in betas:
