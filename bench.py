@@ -49,6 +49,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--gaussian", action="store_true", help="NEXT-3: Gaussian couplings in fixed point (16 fractional bits), separate kernels")
     ap.add_argument("--track-round-trips", action="store_true", help="NEXT-1: tunnelling-time bookkeeping in every PT pass")
     return ap.parse_args()
 
@@ -102,11 +103,13 @@ def measured_peaks():
 
 
 # --------------------------------------------------------------------------------------------------------------
-def oracle_time(w, S, n_mcs, seed=wl.SEED):
+def oracle_time(w, S, n_mcs, seed=wl.SEED, gaussian=False):
     """Time the oracle as it stands on one host core; returns (flips/ns, seconds, flips)."""
     from oracle import ref
 
     o = ref.Oracle(w.L, w.d, S, w.T, w.betas(), seed)
+    if gaussian:
+        o.set_couplings_fixed(wl.gaussian_couplings_fixed(seed, S, w.d, w.N, 16), 16)
     t0 = time.perf_counter()
     for m in range(1, n_mcs + 1):
         o.mcs(1, 1, w.houdayer, True)
@@ -126,6 +129,8 @@ def run_reference(a, w, rank):
     from oracle import ref
 
     o = ref.Oracle(w.L, w.d, S_ref, w.T, w.betas(), wl.SEED)
+    if a.gaussian:
+        o.set_couplings_fixed(wl.gaussian_couplings_fixed(wl.SEED, S_ref, w.d, w.N, 16), 16)
 
     def step():
         o.mcs(a.mcs_per_step, 1, w.houdayer, True)
@@ -158,7 +163,8 @@ def config_of(a, w, n_gpus, sample=None):
              w.name, w.d, w.L, w.S, w.T, w.ladder, w.b_min, w.b_max),
          "mcs_per_step": a.mcs_per_step, "mcs_order": "sweep" + (", houdayer" if w.houdayer else "") + ", exchange",
          "measure_every": w.measure_every, "seed": wl.SEED, "parallelism": "samples sharded x%d" % n_gpus,
-         "l2": "flushed between steps (512 MiB write, untimed)", "round_trip_tracking": bool(a.track_round_trips)}
+         "l2": "flushed between steps (512 MiB write, untimed)", "round_trip_tracking": bool(a.track_round_trips),
+         "couplings": "gaussian, fixed point 2^-16 (NEXT-3)" if a.gaussian else "+-J, p = 1/2"}
     if sample:
         c["sample"] = sample
     return c
@@ -194,6 +200,8 @@ def main():
     # weak scaling: every rank holds the full per-GPU workload on its own range of global sample indices
     B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED, sample_offset=rank * w.S, device=dev,
               track_round_trips=a.track_round_trips)
+    if a.gaussian:
+        B.pt_set_couplings_fixed(wl.gaussian_couplings_fixed(wl.SEED, w.S, w.d, w.N, 16, sample_offset=rank * w.S), 16)
     flush = torch.empty(512 * 2 ** 20, dtype=torch.uint8, device=dev)
     Qd = torch.empty((w.S, w.T), dtype=torch.int32, device=dev)
     QLd = torch.empty((w.S, w.T), dtype=torch.int32, device=dev)
@@ -315,7 +323,7 @@ def main():
     cpu = None
     if not a.no_cpu_baseline:
         S_cpu, mcs_cpu = 4, max(1, int(3.0e8 / (w.flips_per_sweep(4))))
-        v, dt, flips = oracle_time(w, S_cpu, mcs_cpu)
+        v, dt, flips = oracle_time(w, S_cpu, mcs_cpu, gaussian=a.gaussian)
         cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
                "sample": "%s restricted to the first %d samples x %d MCS (%.2e flips), same MCS order" % (w.name, S_cpu, mcs_cpu, flips)}
 

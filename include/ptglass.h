@@ -155,6 +155,15 @@ int pt_get_thresholds(uint32_t *thrM /* [T][d], k=1..d at [t][k-1]; may be NULL 
 int pt_get_counters(uint32_t *n_sweep, uint32_t *n_exchange, uint32_t *n_houdayer);
 int pt_set_spins(const int8_t *spins);      /* values must be +1/-1 (PT_ERR_ARG otherwise); recomputes E */
 int pt_set_couplings(const int8_t *J);      /* values must be +1/-1; recomputes E */
+/* NEXT-3 (R33-R35): replace the couplings by fixed-point numbers J = Jq * 2^-frac_bits
+ * (HOST int32 [S][d][N], Jq[mu][i] = bond i -> i+e_mu; e.g. a rounded standard-normal sample -- the couplings are an input
+ * of the run) and recompute E.  From then on local fields, energies (in units of 2^-frac_bits, int32 as before) and energy
+ * differences are exact integers and the acceptance probabilities are evaluated per decision in double:
+ * flip with a = s_i h_i > 0: u < THR(-(beta_t * ldexp(2a, -frac_bits))); swap: u < THR(-(|dbeta| * ldexp(|dE|, -frac_bits))).
+ * Philox mapping, sweep order, PT pass and cluster move are unchanged; pt_mcs runs the separate kernels.
+ * PT_ERR_ARG: NULL, frac_bits outside [0, 24], or d*N*max|Jq| >= 2^31.  pt_set_couplings returns to the +-J model. */
+int pt_set_couplings_fixed(const int32_t *Jq, int frac_bits);
+int pt_get_couplings_fixed(int32_t *Jq /* [S][d][N] or NULL */, int *frac_bits /* or NULL */);   /* PT_ERR_STATE in the +-J model */
 /* Recompute every E from scratch and count slots whose tracked E differs (invariant check; must be 0). */
 int pt_recompute_energy(int32_t *E_slot_order /* [S][2][T] or NULL */, int *mismatch_count /* or NULL */);
 

@@ -51,6 +51,8 @@ SYMBOLS = {
     "pt_set_spins": (_i, [_vp]),
     "pt_set_couplings": (_i, [_vp]),
     "pt_recompute_energy": (_i, [_vp, _vp]),
+    "pt_set_couplings_fixed": (_i, [_vp, _i]),
+    "pt_get_couplings_fixed": (_i, [_vp, _vp]),
     "pt_synchronize": (_i, []),
     "pt_get_launch_count": (_i, [_vp]),
     "pt_set_profiling": (_i, [_i]),
@@ -299,6 +301,20 @@ def pt_set_couplings(J):
     if j.shape != (_shape["S"], _shape["d"], _shape["N"]):
         raise PTError(PT_ERR_ARG, "J must have shape [S][d][N]")
     _ck(lib().pt_set_couplings(_p(j)))
+
+
+def pt_set_couplings_fixed(Jq, frac_bits):
+    j = np.ascontiguousarray(Jq, dtype=np.int32)
+    if j.shape != (_shape["S"], _shape["d"], _shape["N"]):
+        raise PTError(PT_ERR_ARG, "Jq must have shape [S][d][N]")
+    _ck(lib().pt_set_couplings_fixed(_p(j), int(frac_bits)))
+
+
+def pt_get_couplings_fixed():
+    j = np.empty((_shape["S"], _shape["d"], _shape["N"]), dtype=np.int32)
+    f = C.c_int()
+    _ck(lib().pt_get_couplings_fixed(_p(j), C.byref(f)))
+    return j, f.value
 
 
 def pt_recompute_energy():

@@ -29,6 +29,11 @@ struct DevPtrs {
     int32_t *outProf;           // [S][T][D][L] overlap profiles (NEXT-2)
     int *mismatch;              // [1]
     int8_t *stage;              // int8 staging for get/set: max(S*2*T*N, S*D*N) bytes
+    // fixed-point couplings (NEXT-3, R33-R35)
+    int32_t *JqNat;             // [S][D][N] natural order (staging / read-back)
+    int32_t *Jdev;              // [S][2][2D][32 W] per colour and direction
+    double *betasD;             // [T]
+    double *absdb;              // [T-1] |beta_{t+1} - beta_t|
     // round-trip bookkeeping (NEXT-1, R27-R29)
     uint32_t *rtLabel, *rtStart, *rtTrips;      // [S][2][T] per slot
     unsigned long long *rtSum, *rtCnt;          // [S][2][32] per (sample, chain), bin = floor(log2 pass)
@@ -39,6 +44,7 @@ struct Params {
     uint32_t g0;                // sample_offset: global sample index = g0 + s
     uint32_t strideX;
     int track;                  // 1: round-trip bookkeeping after every PT pass
+    int gauss, fbits;           // 1: couplings are fixed-point numbers Jq * 2^-fbits (gauss.cuh)
     unsigned long long thrJ;    // J = +1 iff Philox word < thrJ = floor(p * 2^32)  (Eq. (2), R32); 2^31 for p = 1/2
     RoundKeys rk;
     DevPtrs d;
@@ -422,6 +428,17 @@ __device__ __forceinline__ uint32_t thrX_lookup(const Params &P, int t, uint32_t
     return (m < P.strideX) ? __ldg(P.d.thrX + (size_t)t * P.strideX + m) : 0u;
 }
 
+// swap threshold for |dE| = absdE at pair t: the +-J table entry m = |dE|/4, or, with fixed-point couplings (R34),
+// THR(-(|dbeta| * ldexp(|dE|, -fbits))) evaluated in double
+__device__ __forceinline__ uint32_t swap_threshold(const Params &P, int t, uint32_t absdE)
+{
+    if (!P.gauss) return thrX_lookup(P, t, absdE >> 2);
+    const double v = floor(ldexp(exp(-(P.d.absdb[t] * ldexp((double)absdE, -P.fbits))), 32));
+    if (v >= 4294967295.0) return 4294967295u;
+    if (v <= 0.0) return 0u;
+    return (uint32_t)v;
+}
+
 // dynamic smem: per warp [T] energies by temperature + [T] slot_of_temp.  GLOBAL_SCRATCH (very long ladders):
 // the same walk on outE / slot_of_temp in global memory.
 template <bool GLOBAL_SCRATCH>
@@ -457,8 +474,7 @@ __global__ void k_exchange(Params P, uint32_t step)
                 const int32_t eb = Et[t + 1], rb = so[t + 1];
                 const int32_t dE = ea - eb;
                 const int sg = P.d.sgn[t];
-                const uint32_t m = (uint32_t)(dE < 0 ? -dE : dE) >> 2;
-                const bool acc = ((long long)sg * dE <= 0) || (u < thrX_lookup(P, t, m));
+                const bool acc = ((long long)sg * dE <= 0) || (u < swap_threshold(P, t, (uint32_t)(dE < 0 ? -dE : dE)));
                 if (acc) {
                     Et[t] = eb; so[t] = rb;                 // position t is final; (ea, ra) moves up to t+1
                     P.d.accepts[(size_t)chain * (T - 1) + t] += 1ull;

@@ -14,6 +14,7 @@
 
 #include "kernels.cuh"
 #include "mcs.cuh"
+#include "gauss.cuh"
 
 using namespace ptg;
 
@@ -187,6 +188,10 @@ size_t carve(void *base, int L, int d, int S, int T, uint32_t strideX, DevPtrs *
     p.outQL = c.take<int32_t>(base, (size_t)S * T);
     p.mismatch = c.take<int>(base, 64);
     p.outProf = c.take<int32_t>(base, (size_t)S * T * d * L);
+    p.JqNat = c.take<int32_t>(base, (size_t)S * d * N);
+    p.Jdev = c.take<int32_t>(base, (size_t)S * 2 * 2 * d * 32 * W);
+    p.betasD = c.take<double>(base, (size_t)T);
+    p.absdb = c.take<double>(base, (size_t)T);
     p.rtLabel = c.take<uint32_t>(base, R);
     p.rtStart = c.take<uint32_t>(base, R);
     p.rtTrips = c.take<uint32_t>(base, R);
@@ -246,7 +251,8 @@ cudaError_t launch_energy(int mode)
     with_lattice([&](auto lat) {
         const long reps = (long)G.P.S * 2 * G.P.T;
         const int wpb = 4;
-        k_energy<<<(unsigned)((reps + wpb - 1) / wpb), wpb * 32, 0, G.stream>>>(lat, G.P, mode);
+        if (G.P.gauss) k_energy_q<<<(unsigned)((reps + wpb - 1) / wpb), wpb * 32, 0, G.stream>>>(lat, G.P, mode);
+        else k_energy<<<(unsigned)((reps + wpb - 1) / wpb), wpb * 32, 0, G.stream>>>(lat, G.P, mode);
         ++G.launches;
         err = cudaGetLastError();
     });
@@ -270,6 +276,16 @@ cudaError_t launch_sweep(int n)
         using LAT = decltype(lat);
         const int W = G.P.W, D = G.P.D;
         const int R = sweep_group(G.P.T, W);
+        if (G.P.gauss) {
+            const size_t smq = ((size_t)R * 2 * W + 2 * (size_t)R) * 4;
+            err = allow_smem(k_sweep_q<LAT>, smq);
+            if (err != cudaSuccess) return;
+            dim3 gq((unsigned)(2 * G.P.T / R), (unsigned)G.P.S);
+            k_sweep_q<LAT><<<gq, 128, smq, G.stream>>>(lat, G.P, R, G.n_sweep, n);
+            ++G.launches;
+            err = cudaGetLastError();
+            return;
+        }
         const size_t smem = ((size_t)2 * 2 * D * W + (size_t)R * 2 * W + (size_t)R * 4 + (size_t)R) * 4;
         err = allow_smem(k_sweep<LAT>, smem);
         if (err != cudaSuccess) return;
@@ -329,6 +345,15 @@ cudaError_t launch_houdayer()
     return err;
 }
 
+// The cluster kernels compute delta from the +-J bit couplings; with fixed-point couplings the cluster itself is the
+// same (it depends on q only) and the energies are simply recomputed from scratch, which for integers is the same number.
+cudaError_t launch_houdayer_any()
+{
+    cudaError_t err = launch_houdayer();
+    if (err == cudaSuccess && G.P.gauss) err = launch_energy(0);
+    return err;
+}
+
 cudaError_t launch_measure(int32_t *Q, int32_t *QL)
 {
     ProfScope prof(3);
@@ -354,7 +379,7 @@ bool mcs_split_chains(int do_houdayer) { return !do_houdayer && (long)G.P.T * G.
 
 bool mcs_fused_eligible(size_t *smem_out, int do_houdayer = 1)
 {
-    if (!G.fast || G.fused_mode == 0) return false;
+    if (!G.fast || G.fused_mode == 0 || G.P.gauss) return false;
     const McsSmem lay(G.P.D, G.P.W, G.P.T, kMcsThreads / 32, 2 * G.P.W <= 32, mcs_split_chains(do_houdayer) ? 1 : 2);
     const size_t smem = (size_t)lay.words * 4;
     if (smem_out) *smem_out = smem;
@@ -497,6 +522,10 @@ int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas,
     CK(cudaMemcpyAsync(P.d.thrM, thrM.data(), thrM.size() * 4, cudaMemcpyHostToDevice, G.stream));
     CK(cudaMemcpyAsync(P.d.thrX, thrX.data(), thrX.size() * 4, cudaMemcpyHostToDevice, G.stream));
     CK(cudaMemcpyAsync(P.d.sgn, sgn.data(), sgn.size() * 4, cudaMemcpyHostToDevice, G.stream));
+    std::vector<double> absdb((size_t)n_temps, 0.0);
+    for (int t = 0; t + 1 < n_temps; ++t) absdb[t] = std::fabs(betas[t + 1] - betas[t]);
+    CK(cudaMemcpyAsync(P.d.betasD, betas, (size_t)n_temps * 8, cudaMemcpyHostToDevice, G.stream));
+    CK(cudaMemcpyAsync(P.d.absdb, absdb.data(), (size_t)n_temps * 8, cudaMemcpyHostToDevice, G.stream));
     CK(cudaStreamSynchronize(G.stream));       // the host vectors go out of scope
     CK(cudaMemsetAsync(P.d.accepts, 0, (size_t)P.S * 2 * P.T * 8, G.stream));
     CK(cudaMemsetAsync(P.d.last, 0, (size_t)P.S * P.T * 4, G.stream));
@@ -560,7 +589,7 @@ int houdayer_step(void)
 {
     NEED_INIT();
     if (G.n_houdayer == 4294967295u) return fail(PT_ERR_OVERFLOW, "Houdayer counter would overflow");
-    CK(launch_houdayer());
+    CK(launch_houdayer_any());
     G.n_houdayer += 1;
     return PT_OK;
 }
@@ -586,7 +615,7 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
     }
     for (int m = 0; m < n_mcs; ++m) {
         if (n_metro > 0) { CK(launch_sweep(n_metro)); G.n_sweep += (uint32_t)n_metro; }
-        if (do_houdayer) { CK(launch_houdayer()); G.n_houdayer += 1; }
+        if (do_houdayer) { CK(launch_houdayer_any()); G.n_houdayer += 1; }
         if (do_exchange) { CK(launch_exchange()); G.n_exchange += 1; }
     }
     return PT_OK;
@@ -760,6 +789,7 @@ int pt_get_couplings(int8_t *J)
 {
     NEED_INIT();
     if (!J) return fail(PT_ERR_ARG, "J is NULL");
+    if (G.P.gauss) return fail(PT_ERR_STATE, "couplings are fixed-point numbers: use pt_get_couplings_fixed");
     const size_t n = (size_t)G.P.S * G.P.D * G.P.N;
     k_unpack_couplings<<<grid_for((long)n, 256), 256, 0, G.stream>>>(G.P);
     ++G.launches;
@@ -824,9 +854,40 @@ int pt_set_couplings(const int8_t *J)
     CK(cudaMemcpyAsync(G.P.d.stage, J, n, cudaMemcpyHostToDevice, G.stream));
     int rc = check_pm1_staged(n, "J");
     if (rc) return rc;
+    G.P.gauss = 0;
     if ((rc = pack_couplings())) return rc;
     CK(launch_energy(0));
     CK(cudaStreamSynchronize(G.stream));
+    return PT_OK;
+}
+
+int pt_set_couplings_fixed(const int32_t *Jq, int frac_bits)
+{
+    NEED_INIT();
+    if (!Jq) return fail(PT_ERR_ARG, "Jq is NULL");
+    if (frac_bits < 0 || frac_bits > 24) return fail(PT_ERR_ARG, "frac_bits must be in [0, 24]");
+    const size_t n = (size_t)G.P.S * G.P.D * G.P.N;
+    long long maxabs = 0;
+    for (size_t k = 0; k < n; ++k) maxabs = std::max<long long>(maxabs, Jq[k] < 0 ? -(long long)Jq[k] : (long long)Jq[k]);
+    if ((double)maxabs * (double)G.P.D * (double)G.P.N >= 2147483648.0)
+        return fail(PT_ERR_ARG, "d * N * max|Jq| must stay below 2^31 (int32 energies): use fewer fractional bits");
+    CK(cudaMemcpyAsync(G.P.d.JqNat, Jq, n * 4, cudaMemcpyHostToDevice, G.stream));
+    G.P.gauss = 1;
+    G.P.fbits = frac_bits;
+    k_pack_jq<<<grid_for((long)G.P.S * 2 * 2 * G.P.D * 32 * G.P.W, 256), 256, 0, G.stream>>>(G.P);
+    ++G.launches;
+    CK(cudaGetLastError());
+    CK(launch_energy(0));
+    CK(cudaStreamSynchronize(G.stream));
+    return PT_OK;
+}
+
+int pt_get_couplings_fixed(int32_t *Jq, int *frac_bits)
+{
+    NEED_INIT();
+    if (!G.P.gauss) return fail(PT_ERR_STATE, "couplings are +-1: use pt_get_couplings");
+    if (frac_bits) *frac_bits = G.P.fbits;
+    if (Jq) return d2h(Jq, G.P.d.JqNat, (size_t)G.P.S * G.P.D * G.P.N * 4);
     return PT_OK;
 }
 

@@ -1,0 +1,113 @@
+"""GPU parity of the NEXT-3 row: fixed-point (Gaussian) couplings with double-exp acceptance, through the
+C ABI, bit for bit against the oracle: spins, energies, permutations, swap counts, cluster sizes, overlaps.
+Run with `-m gpu`."""
+import numpy as np
+import pytest
+
+from oracle import ref
+from paper_2003_04621_b200 import binding as B
+from paper_2003_04621_b200 import build as build_mod
+from paper_2003_04621_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    build_mod.build()
+    yield
+    B.pt_free()
+
+
+def same_state(o, tag):
+    a, b = o.state(), B.state()
+    for k in a:
+        assert np.array_equal(a[k], b[k]), "%s: %s differs" % (tag, k)
+    Qo, QLo = o.measure_overlap(); Qg, QLg = B.pt_measure_overlap()
+    assert np.array_equal(Qo, Qg) and np.array_equal(QLo, QLg), tag
+    assert B.pt_recompute_energy()[1] == 0, tag
+
+
+@pytest.mark.parametrize("L,d,S,T,fbits,general", [
+    (8, 2, 3, 5, 16, False), (32, 2, 2, 6, 16, False), (64, 2, 1, 3, 12, False), (8, 3, 2, 4, 16, False), (16, 3, 1, 3, 14, False),
+    (4, 2, 2, 3, 16, False), (6, 3, 2, 3, 10, False), (10, 2, 1, 4, 16, False), (16, 2, 2, 4, 16, True)])
+def test_gaussian_couplings_match_oracle(L, d, S, T, fbits, general):
+    betas = wl.betas_geometric(0.2, 1.4, T)
+    Jq = wl.gaussian_couplings_fixed(wl.SEED, S, d, L ** d, fbits, sample_offset=2)
+    o = ref.Oracle(L, d, S, T, betas, wl.SEED, 2)
+    o.set_couplings_fixed(Jq, fbits)
+    B.pt_open(L, d, S, T, betas, wl.SEED, 2, general=general)
+    B.pt_set_couplings_fixed(Jq, fbits)
+    j2, f2 = B.pt_get_couplings_fixed()
+    assert np.array_equal(j2, Jq) and f2 == fbits
+    same_state(o, "after set")
+    for step in range(5):
+        o.sweep(1); B.pt_sweep(1)
+        same_state(o, "sweep %d" % step)
+        o.houdayer_step(); B.houdayer_step()
+        same_state(o, "houdayer %d" % step)
+        o.exchange(); B.pt_exchange()
+        same_state(o, "exchange %d" % step)
+    o.sweep(3); B.pt_sweep(3)
+    same_state(o, "sweep(3)")
+    o.mcs(20, 2, True, True); B.pt_mcs(20, 2, True, True)
+    same_state(o, "mcs")
+    assert B.pt_get_fused() == 0
+
+
+def test_pm_one_in_fixed_point_equals_the_pmJ_path_on_the_device():
+    L, d, S, T, fbits = 32, 2, 2, 5, 16
+    betas = wl.betas_geometric(0.3, 1.8, T)
+    B.pt_open(L, d, S, T, betas, wl.SEED)
+    J = B.pt_get_couplings()
+    B.pt_mcs(15, 1, True, True)
+    ref_state = B.state()
+    B.pt_open(L, d, S, T, betas, wl.SEED)
+    B.pt_set_couplings_fixed(J.astype(np.int32) << fbits, fbits)
+    B.pt_mcs(15, 1, True, True)
+    st = B.state()
+    for k in st:
+        if k == "energy":
+            assert np.array_equal(st[k], ref_state[k].astype(np.int64) << fbits)
+        else:
+            assert np.array_equal(st[k], ref_state[k]), k
+
+
+def test_errors_and_return_to_pmJ():
+    L, d, S, T = 8, 2, 1, 2
+    B.pt_open(L, d, S, T, wl.betas_linear(0.2, 1.0, T), wl.SEED)
+    with pytest.raises(B.PTError) as e:
+        B.pt_get_couplings_fixed()
+    assert e.value.code == B.PT_ERR_STATE
+    with pytest.raises(B.PTError) as e:
+        B.pt_set_couplings_fixed(np.full((S, d, L * L), 2 ** 25, dtype=np.int32), 16)
+    assert e.value.code == B.PT_ERR_ARG
+    with pytest.raises(B.PTError) as e:
+        B.pt_set_couplings_fixed(np.ones((S, d, L * L), dtype=np.int32), 25)
+    assert e.value.code == B.PT_ERR_ARG
+    J = B.pt_get_couplings()
+    B.pt_set_couplings_fixed(wl.gaussian_couplings_fixed(1, S, d, L * L, 16), 16)
+    with pytest.raises(B.PTError) as e:
+        B.pt_get_couplings()
+    assert e.value.code == B.PT_ERR_STATE
+    B.pt_set_couplings(J)                                   # back to +-J
+    assert np.array_equal(B.pt_get_couplings(), J) and B.pt_recompute_energy()[1] == 0
+
+
+def test_gaussian_C2_shape_sampled_samples():
+    """C2's lattice, ladder and chain count with Gaussian couplings on 64 samples; samples 0 and 63 against the oracle."""
+    w, S, fbits, n = wl.C2, 64, 16, 30
+    Jq = wl.gaussian_couplings_fixed(wl.SEED, S, w.d, w.N, fbits)
+    B.pt_open(w.L, w.d, S, w.T, w.betas(), wl.SEED)
+    B.pt_set_couplings_fixed(Jq, fbits)
+    B.pt_mcs(n, 1, True, True)
+    st = B.state()
+    assert B.pt_recompute_energy()[1] == 0
+    for g in (0, S - 1):
+        o = ref.Oracle(w.L, w.d, 1, w.T, w.betas(), wl.SEED, g)
+        o.set_couplings_fixed(Jq[g:g + 1], fbits)
+        o.mcs(n, 1, True, True)
+        a = o.state()
+        for k in a:
+            if k != "counters":
+                assert np.array_equal(a[k][0], st[k][g]), (g, k)
