@@ -439,7 +439,7 @@ __device__ __forceinline__ uint32_t swap_threshold(const Params &P, int t, uint3
     return (uint32_t)v;
 }
 
-// dynamic smem: per warp [T] energies by temperature + [T] slot_of_temp.  GLOBAL_SCRATCH (very long ladders):
+// dynamic smem: per warp [T] energies by temperature + [T] slot_of_temp + [T] draws + [T] signs / accept flags.  GLOBAL_SCRATCH (very long ladders):
 // the same walk on outE / slot_of_temp in global memory.
 template <bool GLOBAL_SCRATCH>
 __global__ void k_exchange(Params P, uint32_t step)
@@ -452,7 +452,7 @@ __global__ void k_exchange(Params P, uint32_t step)
     const uint32_t g = P.g0 + (uint32_t)s;
     const int T = P.T;
     const size_t base = (size_t)chain * T;
-    int32_t *Et = GLOBAL_SCRATCH ? P.d.outE + base : xsm + (size_t)wib * 2 * T;
+    int32_t *Et = GLOBAL_SCRATCH ? P.d.outE + base : xsm + (size_t)wib * 4 * T;
     int32_t *so = GLOBAL_SCRATCH ? P.d.sot + base : Et + T;
     for (int t = lane; t < T; t += 32) {
         const int r = P.d.sot[base + t];
@@ -461,6 +461,36 @@ __global__ void k_exchange(Params P, uint32_t step)
     }
     __syncwarp();
     int32_t ea = 0, ra = 0;
+    if constexpr (!GLOBAL_SCRATCH) {
+        // draws and signs staged in shared memory by all lanes; lane 0 walks with the next rung prefetched; accept
+        // flags are left in the sign array (value 2) and counted by all lanes afterwards
+        uint32_t *U = (uint32_t *)(so + T);
+        int32_t *SG = (int32_t *)(U + T);
+        for (int t = lane; t < T - 1; t += 32) {
+            uint32_t u, o1, o2, o3;
+            philox4x32_10((uint32_t)t, step, g, make_tag(DOM_SWAP, 0, c, 0), P.rk, u, o1, o2, o3);
+            U[t] = u;
+            SG[t] = P.d.sgn[t];
+        }
+        __syncwarp();
+        if (lane == 0 && T > 1) {
+            ea = Et[0]; ra = so[0];
+            int32_t eb = Et[1], rb = so[1];
+            for (int t = 0; t < T - 1; ++t) {
+                int32_t ebn = 0, rbn = 0;
+                if (t + 2 < T) { ebn = Et[t + 2]; rbn = so[t + 2]; }     // positions > t + 1 are not modified before they are read
+                const int32_t dE = ea - eb;
+                bool acc = (long long)SG[t] * dE <= 0;
+                if (!acc) acc = U[t] < swap_threshold(P, t, (uint32_t)(dE < 0 ? -dE : dE));
+                if (acc) { Et[t] = eb; so[t] = rb; SG[t] = 2; }          // position t is final; (ea, ra) moves up to t+1
+                else     { Et[t] = ea; so[t] = ra; ea = eb; ra = rb; }
+                eb = ebn; rb = rbn;
+            }
+        } else if (lane == 0) { ea = Et[0]; ra = so[0]; }
+        __syncwarp();
+        for (int t = lane; t < T - 1; t += 32)
+            if (SG[t] == 2) P.d.accepts[(size_t)chain * (T - 1) + t] += 1ull;
+    } else {
     if (lane == 0) { ea = Et[0]; ra = so[0]; }
     for (int tb = 0; tb < T - 1; tb += 32) {
         const int tl = tb + lane;
@@ -484,6 +514,7 @@ __global__ void k_exchange(Params P, uint32_t step)
                 }
             }
         }
+    }
     }
     if (lane == 0) {
         Et[T - 1] = ea; so[T - 1] = ra;

@@ -303,8 +303,8 @@ cudaError_t launch_exchange()
     const int T = G.P.T;
     const long chains = (long)G.P.S * 2;
     int wpb = 4;
-    while (wpb > 1 && (size_t)wpb * 2 * T * 4 > 64 * 1024) wpb >>= 1;
-    const size_t smem = (size_t)wpb * 2 * T * 4;
+    while (wpb > 1 && (size_t)wpb * 4 * T * 4 > 64 * 1024) wpb >>= 1;
+    const size_t smem = (size_t)wpb * 4 * T * 4;
     if (smem > 64 * 1024) {      // very long ladders: walk on global scratch instead of shared memory
         k_exchange<true><<<(unsigned)chains, 32, 0, G.stream>>>(G.P, G.n_exchange);
     } else {
