@@ -35,6 +35,10 @@ METRIC = "attempted_spin_flips_per_ns"
 UNIT = "flips/ns"
 SM_COUNT = 148
 INT32_LANES_PER_SM_CLK = 128       # 4 SMSPs x 1 warp-instruction/clk x 32 lanes (fma + alu pipes, 64 each)
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu --set full
+# capture of the same build (profiles/r1_v4_final.md): the packed state of C2 is read once per k_mcs launch (10.68 MB,
+# independent of the number of MCS per launch) and its write-back stays in L2 (0 B).  None where no capture exists.
+NCU_DRAM_BYTES_PER_LAUNCH = {("C2", "k_mcs"): 10.68e6}
 ALGO_OPS_PER_FLIP = {2: 20, 3: 22}  # Philox share 10 + 2d field terms + 6 decide/flip/accumulate
 
 
@@ -297,7 +301,8 @@ def main():
     philox_ops, _ = B.pt_microbench(4, 8, 1000, device=dev)     # measured live: Philox-only ceiling
     roofline = {
         "bound": "alu", "kernel": names[dom], "achieved": A * dom_flips_ns, "peak": peak_ops,
-        "unit": "Gop/s (INT32 thread-ops)", "frac": A * dom_flips_ns / peak_ops, "traffic": None,
+        "unit": "Gop/s (INT32 thread-ops)", "frac": A * dom_flips_ns / peak_ops,
+        "traffic": None if a.gaussian else NCU_DRAM_BYTES_PER_LAUNCH.get((w.name, names[dom])),
         "peak_how": "derived: 148 SMs x 128 INT32 lanes/clk (fma+alu pipes) x %.3f GHz max SM clock; A = %d algorithmic "
                     "ops/flip (Philox 10 + field 2d + decide 6); a %s launch = %d MCS = %d attempted flips" % (
                         peaks.get("sm_max_mhz", 1965.0) / 1e3, A, names[dom], mcs_per_launch, flips_per_launch),
