@@ -47,6 +47,8 @@ def lib():
             "ref_sweep": [C.c_void_p, C.c_int],
             "ref_exchange": [C.c_void_p],
             "ref_houdayer": [C.c_void_p],
+            "ref_houdayer_multi": [C.c_void_p],
+            "ref_set_cluster_moves": [C.c_void_p, C.c_void_p],
             "ref_mcs": [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int],
             "ref_get_energy": [C.c_void_p, C.c_void_p],
             "ref_measure_overlap": [C.c_void_p, C.c_void_p, C.c_void_p],
@@ -136,6 +138,17 @@ class Oracle:
 
     def houdayer_step(self):
         self._ck(lib().ref_houdayer(self._h))
+
+    def houdayer_multi_step(self):
+        self._ck(lib().ref_houdayer_multi(self._h))
+
+    def set_cluster_moves(self, n_clu):
+        if n_clu is None:
+            self._ck(lib().ref_set_cluster_moves(self._h, None))
+            return
+        a = np.ascontiguousarray(n_clu, dtype=np.int32)
+        assert a.shape == (self.T,)
+        self._ck(lib().ref_set_cluster_moves(self._h, _p(a)))
 
     def mcs(self, n_mcs, n_metro=1, do_houdayer=False, do_exchange=True):
         self._ck(lib().ref_mcs(self._h, n_mcs, n_metro, int(do_houdayer), int(do_exchange)))

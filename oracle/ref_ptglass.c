@@ -35,6 +35,7 @@ struct ref_ctx {
     uint32_t *last_size;  /* [S][T] */
     uint64_t *cum_size;   /* [S][T] */
     uint32_t n_sweep, n_exchange, n_houdayer;
+    int32_t *n_clu;       /* [T] single-cluster moves per ref_houdayer call (NEXT-4, R36), or NULL = 1 each */
     /* round-trip bookkeeping (readings R27-R29), per slot / per (sample, chain) */
     uint32_t *rt_label;   /* [S][2][T] 0 = never at index 0 yet, 1 = last end visited is index 0, 2 = index T-1 */
     uint32_t *rt_start;   /* [S][2][T] pass number at which the current trip started */
@@ -250,7 +251,7 @@ void ref_destroy(ref_ctx *c)
     if (!c) return;
     free(c->Jq);
     free(c->betas); free(c->J); free(c->spin); free(c->E); free(c->temp_of_slot); free(c->slot_of_temp);
-    free(c->thrM); free(c->sgn); free(c->attempts); free(c->accepts); free(c->last_size); free(c->cum_size);
+    free(c->thrM); free(c->sgn); free(c->attempts); free(c->accepts); free(c->last_size); free(c->cum_size); free(c->n_clu);
     free(c->rt_label); free(c->rt_start); free(c->rt_trips); free(c->rt_tau_sum); free(c->rt_tau_cnt);
     free(c->nbr); free(c->queue); free(c->mark);
     free(c);
@@ -370,52 +371,136 @@ int ref_get_round_trips(const ref_ctx *c, uint32_t *trips, uint64_t *tau_sum, ui
 
 /* ---------------------------------------------------------------- Houdayer cluster exchange (8(c).5; Eq. (10), R12, R13) */
 
+/* Exchange the sites with mark[i] = 1 between the two configurations at temperature t of sample s: since q_i = -1 there,
+ * both spins are negated; the marked set must be a union of q = -1 components.  Energies are updated by
+ * delta = 2 * sum over boundary bonds (i marked, j not) of J_ij A_i A_j, old spins. */
+static void exchange_marked(ref_ctx *c, int s, int t)
+{
+    int d = c->d, N = c->N;
+    int ra = c->slot_of_temp[rep(c, s, 0, t)], rb = c->slot_of_temp[rep(c, s, 1, t)];
+    int8_t *A = spins_of(c, s, 0, ra), *B = spins_of(c, s, 1, rb);
+    int32_t delta = 0;
+    for (int i = 0; i < N; ++i) {
+        if (!c->mark[i]) continue;
+        for (int mu = 0; mu < d; ++mu) {
+            int up = c->nbr[i * 2 * d + 2 * mu], dn = c->nbr[i * 2 * d + 2 * mu + 1];
+            if (!c->mark[up]) delta += (int32_t)(2 * jval(c, s, mu, i) * A[i] * A[up]);
+            if (!c->mark[dn]) delta += (int32_t)(2 * jval(c, s, mu, dn) * A[i] * A[dn]);
+        }
+    }
+    for (int i = 0; i < N; ++i)
+        if (c->mark[i]) { A[i] = (int8_t)-A[i]; B[i] = (int8_t)-B[i]; }
+    c->E[rep(c, s, 0, ra)] += delta;
+    c->E[rep(c, s, 1, rb)] -= delta;
+}
+
+/* One single-cluster move of pair (s, t): move number j of this step (j = 0 is the paper's one move per MCS, P:143;
+ * j > 0 only with ref_set_cluster_moves, R36).  Returns the cluster size (0 if no site has q = -1). */
+static uint32_t houdayer_move(ref_ctx *c, int s, int t, uint32_t j)
+{
+    int d = c->d, N = c->N;
+    uint32_t g = c->sample_offset + (uint32_t)s;
+    int ra = c->slot_of_temp[rep(c, s, 0, t)], rb = c->slot_of_temp[rep(c, s, 1, t)];
+    int8_t *A = spins_of(c, s, 0, ra), *B = spins_of(c, s, 1, rb);
+    int n_neg = 0;
+    for (int i = 0; i < N; ++i) n_neg += (A[i] * B[i] == -1);
+    uint32_t u = draw(c, j, c->n_houdayer, g, 5, 0, 0, t, 0);
+    if (n_neg == 0) return 0;
+    int k = (int)(((uint64_t)u * (uint64_t)n_neg) >> 32), i0 = -1;
+    for (int i = 0, seen = 0; i < N; ++i)
+        if (A[i] * B[i] == -1) { if (seen == k) { i0 = i; break; } ++seen; }
+    /* breadth-first search over q = -1 sites */
+    memset(c->mark, 0, (size_t)N);
+    int head = 0, tail = 0;
+    c->queue[tail++] = i0; c->mark[i0] = 1;
+    while (head < tail) {
+        int i = c->queue[head++];
+        for (int k2 = 0; k2 < 2 * d; ++k2) {
+            int jn = c->nbr[i * 2 * d + k2];
+            if (!c->mark[jn] && A[jn] * B[jn] == -1) { c->mark[jn] = 1; c->queue[tail++] = jn; }
+        }
+    }
+    exchange_marked(c, s, t);
+    return (uint32_t)tail;
+}
+
 int ref_houdayer(ref_ctx *c)
 {
     if (!c) return -1;
     if (c->n_houdayer == 4294967295u) return -3;
+    int T = c->T;
+    for (int s = 0; s < c->S; ++s)
+        for (int t = 0; t < T; ++t) {
+            int moves = c->n_clu ? c->n_clu[t] : 1;
+            uint32_t size = 0;
+            for (int j = 0; j < moves; ++j) {
+                size = houdayer_move(c, s, t, (uint32_t)j);
+                c->cum_size[(size_t)s * T + t] += (uint64_t)size;
+            }
+            c->last_size[(size_t)s * T + t] = size;        /* the last move's; 0 where n_clu[t] = 0 */
+        }
+    c->n_houdayer += 1;
+    return 0;
+}
+
+/* NEXT-4 ("perform several cluster updates in the high-temperature copies"; P:140 / ref. [39]: cluster moves
+ * only where they help; reading R36): n_clu[t] >= 0 single-cluster moves per ref_houdayer call at temperature index t;
+ * NULL restores one move everywhere. */
+int ref_set_cluster_moves(ref_ctx *c, const int32_t *n_clu)
+{
+    if (!c) return -1;
+    if (!n_clu) { free(c->n_clu); c->n_clu = NULL; return 0; }
+    for (int t = 0; t < c->T; ++t) if (n_clu[t] < 0 || n_clu[t] > 65535) return -1;
+    if (!c->n_clu) c->n_clu = (int32_t *)malloc((size_t)c->T * sizeof(int32_t));
+    if (!c->n_clu) return -2;
+    memcpy(c->n_clu, n_clu, (size_t)c->T * sizeof(int32_t));
+    return 0;
+}
+
+/* NEXT-4 ("a formal conversion to a multi-cluster variant"; reading R37): EVERY connected component of
+ * q = -1 sites is exchanged between the two configurations independently with probability 1/2.  The component whose
+ * smallest site index is i_min is exchanged iff the top bit of word (i_min & 3) of the Philox block
+ * ctr = (i_min >> 2, step, g, tag(5, aux = 1, 0, t)) is set.  Exchanging any union of q = -1 components leaves
+ * E1 + E2 unchanged (every boundary bond has a q = +1 end).  last_size = number of exchanged sites. */
+int ref_houdayer_multi(ref_ctx *c)
+{
+    if (!c) return -1;
+    if (c->n_houdayer == 4294967295u) return -3;
     int d = c->d, N = c->N, T = c->T;
+    uint8_t *seen = (uint8_t *)malloc((size_t)N);
+    if (!seen) return -2;
     for (int s = 0; s < c->S; ++s) {
         uint32_t g = c->sample_offset + (uint32_t)s;
         for (int t = 0; t < T; ++t) {
             int ra = c->slot_of_temp[rep(c, s, 0, t)], rb = c->slot_of_temp[rep(c, s, 1, t)];
             int8_t *A = spins_of(c, s, 0, ra), *B = spins_of(c, s, 1, rb);
-            int n_neg = 0;
-            for (int i = 0; i < N; ++i) n_neg += (A[i] * B[i] == -1);
-            uint32_t u = draw(c, 0, c->n_houdayer, g, 5, 0, 0, t, 0);
-            if (n_neg == 0) { c->last_size[(size_t)s * T + t] = 0; continue; }
-            int k = (int)(((uint64_t)u * (uint64_t)n_neg) >> 32), i0 = -1;
-            for (int i = 0, seen = 0; i < N; ++i)
-                if (A[i] * B[i] == -1) { if (seen == k) { i0 = i; break; } ++seen; }
-            /* breadth-first search over q = -1 sites */
+            memset(seen, 0, (size_t)N);
             memset(c->mark, 0, (size_t)N);
-            int head = 0, tail = 0;
-            c->queue[tail++] = i0; c->mark[i0] = 1;
-            while (head < tail) {
-                int i = c->queue[head++];
-                for (int k2 = 0; k2 < 2 * d; ++k2) {
-                    int j = c->nbr[i * 2 * d + k2];
-                    if (!c->mark[j] && A[j] * B[j] == -1) { c->mark[j] = 1; c->queue[tail++] = j; }
+            uint32_t total = 0;
+            for (int i0 = 0; i0 < N; ++i0) {
+                if (seen[i0] || A[i0] * B[i0] != -1) continue;
+                /* i0 is the smallest index of a component not seen yet: collect it by BFS */
+                int head = 0, tail = 0;
+                c->queue[tail++] = i0; seen[i0] = 1;
+                while (head < tail) {
+                    int i = c->queue[head++];
+                    for (int k2 = 0; k2 < 2 * d; ++k2) {
+                        int jn = c->nbr[i * 2 * d + k2];
+                        if (!seen[jn] && A[jn] * B[jn] == -1) { seen[jn] = 1; c->queue[tail++] = jn; }
+                    }
+                }
+                uint32_t w = draw(c, (uint32_t)(i0 >> 2), c->n_houdayer, g, 5, 1, 0, t, i0 & 3);
+                if (w >> 31) {
+                    for (int k = 0; k < tail; ++k) c->mark[c->queue[k]] = 1;
+                    total += (uint32_t)tail;
                 }
             }
-            /* delta = 2 * sum over boundary bonds (i in cluster, j not) of J_ij A_i A_j, old spins */
-            int32_t delta = 0;
-            for (int i = 0; i < N; ++i) {
-                if (!c->mark[i]) continue;
-                for (int mu = 0; mu < d; ++mu) {
-                    int up = c->nbr[i * 2 * d + 2 * mu], dn = c->nbr[i * 2 * d + 2 * mu + 1];
-                    if (!c->mark[up]) delta += (int32_t)(2 * jval(c, s, mu, i) * A[i] * A[up]);
-                    if (!c->mark[dn]) delta += (int32_t)(2 * jval(c, s, mu, dn) * A[i] * A[dn]);
-                }
-            }
-            for (int i = 0; i < N; ++i)
-                if (c->mark[i]) { A[i] = (int8_t)-A[i]; B[i] = (int8_t)-B[i]; }
-            c->E[rep(c, s, 0, ra)] += delta;
-            c->E[rep(c, s, 1, rb)] -= delta;
-            c->last_size[(size_t)s * T + t] = (uint32_t)tail;
-            c->cum_size[(size_t)s * T + t] += (uint64_t)tail;
+            if (total) exchange_marked(c, s, t);
+            c->last_size[(size_t)s * T + t] = total;
+            c->cum_size[(size_t)s * T + t] += (uint64_t)total;
         }
     }
+    free(seen);
     c->n_houdayer += 1;
     return 0;
 }
@@ -424,11 +509,12 @@ int ref_houdayer(ref_ctx *c)
 
 int ref_mcs(ref_ctx *c, int n_mcs, int n_metro, int do_houdayer, int do_exchange)
 {
-    if (!c || n_mcs < 0 || n_metro < 0) return -1;
+    if (!c || n_mcs < 0 || n_metro < 0 || do_houdayer < 0 || do_houdayer > 2) return -1;
     for (int m = 0; m < n_mcs; ++m) {
         int rc = ref_sweep(c, n_metro);
         if (rc) return rc;
-        if (do_houdayer && (rc = ref_houdayer(c))) return rc;
+        if (do_houdayer == 1 && (rc = ref_houdayer(c))) return rc;
+        if (do_houdayer == 2 && (rc = ref_houdayer_multi(c))) return rc;
         if (do_exchange && (rc = ref_exchange(c))) return rc;
     }
     return 0;

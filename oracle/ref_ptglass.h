@@ -48,7 +48,16 @@ void ref_destroy(ref_ctx *c);
 int ref_sweep(ref_ctx *c, int n);
 int ref_exchange(ref_ctx *c);
 int ref_houdayer(ref_ctx *c);
-int ref_mcs(ref_ctx *c, int n_mcs, int n_metro, int do_houdayer, int do_exchange);
+int ref_mcs(ref_ctx *c, int n_mcs, int n_metro, int do_houdayer /* 0 none, 1 single-cluster, 2 multi-cluster */,
+            int do_exchange);
+/* NEXT-4 cluster-move variants (readings R36, R37).
+ * ref_set_cluster_moves: n_clu[t] in [0, 65535] single-cluster moves per ref_houdayer call at temperature index t
+ * (move j draws its seed from Philox counter index j; n_clu = NULL restores one move everywhere; 0 switches the move
+ * off at that temperature -- the temperature window of ref. [39]).
+ * ref_houdayer_multi: every q = -1 component is exchanged with probability 1/2, decided by the Philox bit of its
+ * smallest site index; the cluster-size observables then count exchanged sites. */
+int ref_set_cluster_moves(ref_ctx *c, const int32_t *n_clu /* [T] or NULL */);
+int ref_houdayer_multi(ref_ctx *c);
 
 /* Observables, indexed by TEMPERATURE t. */
 int ref_get_energy(const ref_ctx *c, int32_t *E /* [S][2][T] */);
