@@ -92,8 +92,28 @@ int pt_exchange(void);
  * connected component among q = -1 sites is negated in both configurations; E1 += delta, E2 -= delta. */
 int houdayer_step(void);
 
+/* Cluster-move variants the paper proposes against idle threads and for three dimensions (P:140,
+ * ref. [39]), readings R36, R37.
+ *
+ * pt_set_cluster_moves: n_clu[t] in [0, 65535] single-cluster moves per houdayer_step (and per MCS of pt_mcs with
+ * do_houdayer = 1) at temperature index t -- "several cluster updates in the high-temperature copies"; 0 switches the
+ * move off at that temperature (a temperature window).  n_clu: host array [T], copied; NULL restores one move
+ * everywhere (the state after pt_init).  Move j at a temperature draws its seed from the domain-5 Philox block with
+ * counter index j, so the default (all ones) is bit-identical to the plain move.  last = size of the last move (0 where
+ * n_clu[t] = 0), cumulative adds every move.  PT_ERR_ARG on a count outside the range; call after pt_init.
+ *
+ * houdayer_multi_step: the multi-cluster variant -- EVERY connected component of q = -1 sites is exchanged with
+ * probability 1/2: the component whose smallest site index is i_min is exchanged iff the top bit of word (i_min & 3) of
+ * the Philox block ctr = (i_min >> 2, step, g, tag(5, aux 1, 0, t)) is set.  E1 + E2 is conserved for any such union
+ * (P:138).  last / cumulative count exchanged sites; the Houdayer step counter advances by one.  Components are found by
+ * label propagation in shared memory, one CTA per (sample, temperature): PT_ERR_ARG if 4 N bytes of labels do not fit
+ * (N <= ~56000 sites).  In pt_mcs it is do_houdayer = 2 (separate kernels, not fused). */
+int pt_set_cluster_moves(const int32_t *n_clu);
+int houdayer_multi_step(void);
+
 /* Fused Monte Carlo steps in the paper's order (R15): n_mcs x [ pt_sweep(n_metro);
- * houdayer_step() if do_houdayer; pt_exchange() if do_exchange ].  Bit-identical to the separate calls.
+ * houdayer_step() if do_houdayer = 1, houdayer_multi_step() if do_houdayer = 2; pt_exchange() if do_exchange ].
+ * Bit-identical to the separate calls.  PT_ERR_ARG if do_houdayer is not 0, 1 or 2.
  * Where a sample's whole state fits in shared memory this is ONE kernel launch that keeps each
  * sample resident in one CTA for all n_mcs steps; otherwise it issues the separate kernels in order. */
 int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange);

@@ -28,6 +28,8 @@ SYMBOLS = {
     "pt_sweep": (_i, [_i]),
     "pt_exchange": (_i, []),
     "houdayer_step": (_i, []),
+    "houdayer_multi_step": (_i, []),
+    "pt_set_cluster_moves": (_i, [_vp]),
     "pt_mcs": (_i, [_i, _i, _i, _i]),
     "pt_set_fused": (_i, [_i]),
     "pt_get_fused": (_i, [_vp]),
@@ -196,6 +198,19 @@ def pt_exchange():
 
 def houdayer_step():
     _ck(lib().houdayer_step())
+
+
+def houdayer_multi_step():
+    _ck(lib().houdayer_multi_step())
+
+
+def pt_set_cluster_moves(n_clu):
+    """n_clu: [T] int32 host array of single-cluster moves per temperature, or None for one move everywhere."""
+    if n_clu is None:
+        _ck(lib().pt_set_cluster_moves(None))
+        return
+    a = np.ascontiguousarray(n_clu, dtype=np.int32)
+    _ck(lib().pt_set_cluster_moves(a.ctypes.data))
 
 
 def pt_mcs(n_mcs, n_metro=1, do_houdayer=False, do_exchange=True):

@@ -37,6 +37,8 @@ struct DevPtrs {
     // round-trip bookkeeping (NEXT-1, R27-R29)
     uint32_t *rtLabel, *rtStart, *rtTrips;      // [S][2][T] per slot
     unsigned long long *rtSum, *rtCnt;          // [S][2][32] per (sample, chain), bin = floor(log2 pass)
+    // cluster-move variants (NEXT-4, R36): single-cluster moves per houdayer_step at temperature index t
+    int32_t *nclu;              // [T]
 };
 
 struct Params {
@@ -535,8 +537,58 @@ __global__ void k_exchange(Params P, uint32_t step)
 // colours until nothing changes -- the fixed point is exactly the connected component of the seed.
 // =========================================================================================================
 // dynamic smem: Neg[2][W] | Cl[2][W] | scan[blockDim/32 + 2]
+// Tail shared by the one-CTA-per-pair kernels: Cl[2][W] holds a union of q = -1 components in the colour layout.
+// size, delta = 2 * sum over boundary bonds of J A_i A_j = 2 * (#boundary - 2 #boundary&unsatisfied) (old spins), each
+// bond seen from its black endpoint; then the set is negated in both configurations and E, last, cum are updated.
+// red: 2 * nwarps ints of shared memory.  Every thread of the CTA must call.
 template <class LAT>
-__global__ void __launch_bounds__(128) k_houdayer_gen(LAT lat, Params P, uint32_t step)
+__device__ __forceinline__ void cta_exchange_set(const LAT &lat, const Params &P, int s, int t, size_t repA, size_t repB,
+                                                 uint32_t *const A[2], uint32_t *const B[2], const uint32_t *Cl, int *red)
+{
+    constexpr int D = LAT::D;
+    const int W = lat.words();
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nwarps = blockDim.x >> 5;
+    int size = 0, delta = 0;
+    for (int w = tid; w < W; w += blockDim.x) {
+        const uint32_t cb = Cl[w], cwh = Cl[W + w], v = lat.valid(w);
+        size += __popc(cb) + __popc(cwh);
+        uint32_t nbC[2 * D], nbA[2 * D];
+        lat.gather(Cl + W, w, 0, nbC);
+        lat.gather(A[1], w, 0, nbA);
+        const uint32_t ab = A[0][w];
+#pragma unroll
+        for (int k = 0; k < 2 * D; ++k) {
+            const uint32_t bnd = (cb ^ nbC[k]) & v;
+            const uint32_t uns = ab ^ nbA[k] ^ J_words(P, s, 0, k)[w];
+            delta += 2 * (__popc(bnd) - 2 * __popc(bnd & uns));
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        size += __shfl_xor_sync(0xFFFFFFFFu, size, o);
+        delta += __shfl_xor_sync(0xFFFFFFFFu, delta, o);
+    }
+    __syncthreads();                 // all reads of the old A done before anyone writes; red[] reusable
+    if (lane == 0) { red[wid] = size; red[nwarps + wid] = delta; }
+    __syncthreads();
+    for (int p = 0; p < 2; ++p)
+        for (int w = tid; w < W; w += blockDim.x) {
+            const uint32_t c = Cl[p * W + w];
+            if (c) { A[p][w] ^= c; B[p][w] ^= c; }
+        }
+    if (tid == 0) {
+        int sz = 0, dl = 0;
+        for (int i = 0; i < nwarps; ++i) { sz += red[i]; dl += red[nwarps + i]; }
+        P.d.E[repA] += dl;
+        P.d.E[repB] -= dl;
+        P.d.last[(size_t)s * P.T + t] = (uint32_t)sz;
+        P.d.cum[(size_t)s * P.T + t] += (unsigned long long)sz;
+    }
+}
+
+// move: number of this single-cluster move within the step (R36); pairs with nclu[t] <= move do nothing.
+template <class LAT>
+__global__ void __launch_bounds__(128) k_houdayer_gen(LAT lat, Params P, uint32_t step, uint32_t move)
 {
     constexpr int D = LAT::D;
     extern __shared__ uint32_t hsm[];
@@ -545,6 +597,10 @@ __global__ void __launch_bounds__(128) k_houdayer_gen(LAT lat, Params P, uint32_
     int *scan = (int *)(Cl + 2 * W);           // [0..nwarps): warp totals; [nwarps]: seed word; [nwarps+1]: seed colour|bit
     const int t = blockIdx.x, s = blockIdx.y;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nwarps = blockDim.x >> 5;
+    if (move >= (uint32_t)P.d.nclu[t]) {
+        if (move == 0 && tid == 0) P.d.last[(size_t)s * P.T + t] = 0;
+        return;
+    }
     const size_t repA = rep_index(P, s, 0, P.d.sot[rep_index(P, s, 0, t)]);
     const size_t repB = rep_index(P, s, 1, P.d.sot[rep_index(P, s, 1, t)]);
     uint32_t *A[2] = {spin_words(P, repA, 0), spin_words(P, repA, 1)};
@@ -580,7 +636,7 @@ __global__ void __launch_bounds__(128) k_houdayer_gen(LAT lat, Params P, uint32_
         return;
     }
     uint32_t u, o1, o2, o3;
-    philox4x32_10(0u, step, P.g0 + (uint32_t)s, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
+    philox4x32_10(move, step, P.g0 + (uint32_t)s, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
     const int kth = (int)(((unsigned long long)u * (unsigned long long)n_neg) >> 32);
     if (kth >= excl && kth < excl + local) {
         // this thread's chunk holds the seed: walk words, then the 32 half-indices of the word in site order
@@ -622,44 +678,7 @@ __global__ void __launch_bounds__(128) k_houdayer_gen(LAT lat, Params P, uint32_
         if (!__syncthreads_or(changed)) break;
     }
 
-    // size, delta = 2 * sum over boundary bonds of J A_i A_j = 2 * (#boundary - 2 #boundary&unsatisfied) (old spins),
-    // each bond seen from its black endpoint; then negate the cluster in both configurations
-    int size = 0, delta = 0;
-    for (int w = tid; w < W; w += blockDim.x) {
-        const uint32_t cb = Cl[w], cwh = Cl[W + w], v = lat.valid(w);
-        size += __popc(cb) + __popc(cwh);
-        uint32_t nbC[2 * D], nbA[2 * D];
-        lat.gather(Cl + W, w, 0, nbC);
-        lat.gather(A[1], w, 0, nbA);
-        const uint32_t ab = A[0][w];
-#pragma unroll
-        for (int k = 0; k < 2 * D; ++k) {
-            const uint32_t bnd = (cb ^ nbC[k]) & v;
-            const uint32_t uns = ab ^ nbA[k] ^ J_words(P, s, 0, k)[w];
-            delta += 2 * (__popc(bnd) - 2 * __popc(bnd & uns));
-        }
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        size += __shfl_xor_sync(0xFFFFFFFFu, size, o);
-        delta += __shfl_xor_sync(0xFFFFFFFFu, delta, o);
-    }
-    __syncthreads();                 // all reads of the old A done before anyone writes; scan[] reusable
-    if (lane == 0) { scan[wid] = size; scan[nwarps + wid] = delta; }
-    __syncthreads();
-    for (int p = 0; p < 2; ++p)
-        for (int w = tid; w < W; w += blockDim.x) {
-            const uint32_t c = Cl[p * W + w];
-            if (c) { A[p][w] ^= c; B[p][w] ^= c; }
-        }
-    if (tid == 0) {
-        int sz = 0, dl = 0;
-        for (int i = 0; i < nwarps; ++i) { sz += scan[i]; dl += scan[nwarps + i]; }
-        P.d.E[repA] += dl;
-        P.d.E[repB] -= dl;
-        P.d.last[(size_t)s * P.T + t] = (uint32_t)sz;
-        P.d.cum[(size_t)s * P.T + t] += (unsigned long long)sz;
-    }
+    cta_exchange_set(lat, P, s, t, repA, repB, A, B, Cl, scan);
 }
 
 // =========================================================================================================
@@ -667,17 +686,21 @@ __global__ void __launch_bounds__(128) k_houdayer_gen(LAT lat, Params P, uint32_
 // grid: ceil(S*T / warps per CTA); dynamic smem: kPairScratchWords<LAT> words per warp.
 // =========================================================================================================
 template <class LAT>
-__global__ void __launch_bounds__(128, 6) k_houdayer(LAT lat, Params P, uint32_t step)
+__global__ void __launch_bounds__(128, 6) k_houdayer(LAT lat, Params P, uint32_t step, uint32_t move)
 {
     extern __shared__ uint32_t hsm[];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
     const long pair = (long)blockIdx.x * wpb + wib;
     if (pair >= (long)P.S * P.T) return;
     const int s = (int)(pair / P.T), t = (int)(pair - (long)s * P.T);
+    if (move >= (uint32_t)P.d.nclu[t]) {                    // R36: this temperature makes no move number `move`
+        if (move == 0 && lane == 0) P.d.last[pair] = 0;
+        return;
+    }
     const size_t repA = rep_index(P, s, 0, P.d.sot[rep_index(P, s, 0, t)]);
     const size_t repB = rep_index(P, s, 1, P.d.sot[rep_index(P, s, 1, t)]);
     uint32_t u, o1, o2, o3;
-    philox4x32_10(0u, step, P.g0 + (uint32_t)s, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
+    philox4x32_10(move, step, P.g0 + (uint32_t)s, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
     int delta;
     const int size = houdayer_warp(lat, spin_words(P, repA, 0), spin_words(P, repA, 1), spin_words(P, repB, 0),
                                    spin_words(P, repB, 1), J_words(P, s, 0, 0), hsm + (size_t)wib * kPairScratchWords<LAT>, u, lane, delta);

@@ -15,6 +15,7 @@ namespace ptg {
 struct McsArgs {
     int n_mcs, n_metro, do_houdayer, do_exchange;
     int split_chains;                       // 1: one CTA per (sample, chain) -- only without Houdayer moves (the chains never meet)
+    int max_clu;                            // max over t of nclu[t] (R36); 1 in a default run
     uint32_t sweep0, houd0, exch0;          // counter values at the start of the call
 };
 
@@ -125,22 +126,26 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                     uint32_t *col = msm + L.oScr + wid * LaneHoudayer<LAT>::kScratchWords + lane;
                     for (int t0 = wid * 32; t0 < T; t0 += hw * 32) {
                         const int t = t0 + lane;
-                        const bool active = t < T;
-                        int ra = 0, rb = T;
-                        uint32_t u = 0, o1, o2, o3;
-                        if (active) {
-                            ra = sSot[t];
-                            rb = T + sSot[T + t];
-                            philox4x32_10(0u, step, g, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
-                        }
-                        int delta;
-                        const int size = houdayer_lane(lat, sS + ra * RS, sS + ra * RS + W, sS + rb * RS, sS + rb * RS + W,
-                                                       sJ, col, u, active, delta);
-                        if (active) {
-                            sE[ra] += delta;
-                            sE[rb] -= delta;
-                            sLast[t] = (uint32_t)size;
-                            sCum[t] += (unsigned long long)size;
+                        const int moves = (t < T) ? P.d.nclu[t] : 0;            // R36; 1 everywhere in a default run
+                        if (t < T && moves == 0) sLast[t] = 0u;
+                        for (int mv = 0; mv < a.max_clu; ++mv) {
+                            const bool active = mv < moves;
+                            int ra = 0, rb = T;
+                            uint32_t u = 0, o1, o2, o3;
+                            if (active) {
+                                ra = sSot[t];
+                                rb = T + sSot[T + t];
+                                philox4x32_10((uint32_t)mv, step, g, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
+                            }
+                            int delta;
+                            const int size = houdayer_lane(lat, sS + ra * RS, sS + ra * RS + W, sS + rb * RS, sS + rb * RS + W,
+                                                           sJ, col, u, active, delta);
+                            if (active) {
+                                sE[ra] += delta;
+                                sE[rb] -= delta;
+                                sLast[t] = (uint32_t)size;
+                                sCum[t] += (unsigned long long)size;
+                            }
                         }
                     }
                 }
@@ -149,16 +154,21 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                 uint32_t *scratch = msm + L.oScr + wid * kPairScratchWords<LAT>;
                 for (int t = wid; t < T; t += NWARPS) {
                     const int ra = sSot[t], rb = T + sSot[T + t];
-                    uint32_t u, o1, o2, o3;
-                    philox4x32_10(0u, step, g, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
-                    int delta;
-                    const int size = houdayer_warp(lat, sS + ra * RS, sS + ra * RS + W, sS + rb * RS, sS + rb * RS + W, sJ,
-                                                   scratch, u, lane, delta);
-                    if (lane == 0) {
-                        sE[ra] += delta;
-                        sE[rb] -= delta;
-                        sLast[t] = (uint32_t)size;
-                        sCum[t] += (unsigned long long)size;
+                    const int moves = P.d.nclu[t];                              // R36
+                    if (moves == 0 && lane == 0) sLast[t] = 0u;
+                    for (int mv = 0; mv < moves; ++mv) {
+                        uint32_t u, o1, o2, o3;
+                        philox4x32_10((uint32_t)mv, step, g, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
+                        int delta;
+                        const int size = houdayer_warp(lat, sS + ra * RS, sS + ra * RS + W, sS + rb * RS, sS + rb * RS + W, sJ,
+                                                       scratch, u, lane, delta);
+                        if (lane == 0) {
+                            sE[ra] += delta;
+                            sE[rb] -= delta;
+                            sLast[t] = (uint32_t)size;
+                            sCum[t] += (unsigned long long)size;
+                        }
+                        __syncwarp();
                     }
                 }
             }

@@ -15,6 +15,7 @@
 #include "kernels.cuh"
 #include "mcs.cuh"
 #include "gauss.cuh"
+#include "houdayer_multi.cuh"
 
 using namespace ptg;
 
@@ -34,6 +35,7 @@ struct Context {
     std::vector<double> betas;
     uint64_t seed = 0;
     uint32_t n_sweep = 0, n_exchange = 0, n_houdayer = 0;
+    int max_clu = 1;            // max over t of the per-temperature cluster-move counts (NEXT-4, R36)
     uint64_t launches = 0;
     size_t stage_bytes = 0;
 };
@@ -197,6 +199,7 @@ size_t carve(void *base, int L, int d, int S, int T, uint32_t strideX, DevPtrs *
     p.rtTrips = c.take<uint32_t>(base, R);
     p.rtSum = c.take<unsigned long long>(base, (size_t)S * 2 * 32);
     p.rtCnt = c.take<unsigned long long>(base, (size_t)S * 2 * 32);
+    p.nclu = c.take<int32_t>(base, (size_t)T);
     const size_t sb = std::max(R * N, (size_t)S * d * N);
     p.stage = c.take<int8_t>(base, sb);
     if (out) *out = p;
@@ -316,10 +319,12 @@ cudaError_t launch_exchange()
     return cudaGetLastError();
 }
 
+// One launch per move number (R36): move j touches the temperatures with nclu[t] > j; a default run makes one launch.
 cudaError_t launch_houdayer()
 {
     ProfScope prof(1);
     cudaError_t err = cudaSuccess;
+    for (uint32_t move = 0; move < (uint32_t)std::max(G.max_clu, 1) && err == cudaSuccess; ++move)
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
         if constexpr (LAT::kFast) {
@@ -330,14 +335,14 @@ cudaError_t launch_houdayer()
             err = allow_smem(k_houdayer<LAT>, smem);
             if (err != cudaSuccess) return;
             const long pairs = (long)G.P.S * G.P.T;
-            k_houdayer<LAT><<<(unsigned)((pairs + wpb - 1) / wpb), wpb * 32, smem, G.stream>>>(lat, G.P, G.n_houdayer);
+            k_houdayer<LAT><<<(unsigned)((pairs + wpb - 1) / wpb), wpb * 32, smem, G.stream>>>(lat, G.P, G.n_houdayer, move);
         } else {
             const int threads = 128;
             const size_t smem = ((size_t)4 * G.P.W + 2 * (threads / 32) + 2) * 4;
             err = allow_smem(k_houdayer_gen<LAT>, smem);
             if (err != cudaSuccess) return;
             dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
-            k_houdayer_gen<LAT><<<grid, threads, smem, G.stream>>>(lat, G.P, G.n_houdayer);
+            k_houdayer_gen<LAT><<<grid, threads, smem, G.stream>>>(lat, G.P, G.n_houdayer, move);
         }
         ++G.launches;
         err = cudaGetLastError();
@@ -347,9 +352,31 @@ cudaError_t launch_houdayer()
 
 // The cluster kernels compute delta from the +-J bit couplings; with fixed-point couplings the cluster itself is the
 // same (it depends on q only) and the energies are simply recomputed from scratch, which for integers is the same number.
-cudaError_t launch_houdayer_any()
+// multi-cluster variant (R37): one CTA per pair, labels in shared memory
+size_t multi_smem_bytes(int threads) { return ((size_t)4 * G.P.W + 2 * (threads / 32) + 2 + (size_t)G.P.N) * 4; }
+
+cudaError_t launch_houdayer_multi()
 {
-    cudaError_t err = launch_houdayer();
+    ProfScope prof(1);
+    cudaError_t err = cudaSuccess;
+    with_lattice([&](auto lat) {
+        using LAT = decltype(lat);
+        const int threads = 256;
+        const size_t smem = multi_smem_bytes(threads);
+        err = allow_smem(k_houdayer_multi<LAT>, smem);
+        if (err != cudaSuccess) return;
+        dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
+        k_houdayer_multi<LAT><<<grid, threads, smem, G.stream>>>(lat, G.P, G.n_houdayer);
+        ++G.launches;
+        err = cudaGetLastError();
+    });
+    return err;
+}
+
+// mode 1: single-cluster moves (R36 counts), mode 2: multi-cluster (R37)
+cudaError_t launch_houdayer_any(int mode = 1)
+{
+    cudaError_t err = (mode == 2) ? launch_houdayer_multi() : launch_houdayer();
     if (err == cudaSuccess && G.P.gauss) err = launch_energy(0);
     return err;
 }
@@ -508,6 +535,12 @@ int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas,
         return fail(PT_ERR_STATE, "workspace too small: %zu bytes bound, %zu needed", G.ws_bytes, need);
     G.fast = (G.force_general != 0) && fast_supported(L, d);
     G.n_sweep = G.n_exchange = G.n_houdayer = 0;
+    G.max_clu = 1;
+    {
+        const std::vector<int32_t> ones((size_t)n_temps, 1);
+        CK(cudaMemcpyAsync(P.d.nclu, ones.data(), ones.size() * 4, cudaMemcpyHostToDevice, G.stream));
+        CK(cudaStreamSynchronize(G.stream));
+    }
 
     // acceptance tables on the host, in double (R5, R6)
     std::vector<uint32_t> thrM((size_t)n_temps * 4, 0u);
@@ -594,19 +627,52 @@ int houdayer_step(void)
     return PT_OK;
 }
 
+int houdayer_multi_step(void)
+{
+    NEED_INIT();
+    if (G.n_houdayer == 4294967295u) return fail(PT_ERR_OVERFLOW, "Houdayer counter would overflow");
+    if (multi_smem_bytes(256) > 227 * 1024)
+        return fail(PT_ERR_ARG, "houdayer_multi_step: %d sites of labels do not fit in shared memory", G.P.N);
+    CK(launch_houdayer_any(2));
+    G.n_houdayer += 1;
+    return PT_OK;
+}
+
+int pt_set_cluster_moves(const int32_t *n_clu)
+{
+    NEED_INIT();
+    std::vector<int32_t> v((size_t)G.P.T, 1);
+    int mx = 1;
+    if (n_clu) {
+        mx = 0;
+        for (int t = 0; t < G.P.T; ++t) {
+            if (n_clu[t] < 0 || n_clu[t] > 65535) return fail(PT_ERR_ARG, "pt_set_cluster_moves: n_clu[%d] = %d not in [0, 65535]", t, n_clu[t]);
+            v[t] = n_clu[t];
+            mx = std::max(mx, (int)n_clu[t]);
+        }
+    }
+    CK(cudaMemcpyAsync(G.P.d.nclu, v.data(), v.size() * 4, cudaMemcpyHostToDevice, G.stream));
+    CK(cudaStreamSynchronize(G.stream));
+    G.max_clu = mx;
+    return PT_OK;
+}
+
 int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
 {
     NEED_INIT();
     if (n_mcs < 0 || n_metro < 0) return fail(PT_ERR_ARG, "pt_mcs: n_mcs and n_metro must be >= 0");
+    if (do_houdayer < 0 || do_houdayer > 2) return fail(PT_ERR_ARG, "pt_mcs: do_houdayer must be 0, 1 (single-cluster) or 2 (multi-cluster)");
+    if (do_houdayer == 2 && multi_smem_bytes(256) > 227 * 1024)
+        return fail(PT_ERR_ARG, "pt_mcs: %d sites of labels do not fit in shared memory (multi-cluster)", G.P.N);
     const uint64_t M = (uint64_t)n_mcs;
     if ((uint64_t)G.n_sweep + M * (uint64_t)n_metro > 4294967295ull ||
         (do_exchange && (uint64_t)G.n_exchange + M > 4294967295ull) ||
         (do_houdayer && (uint64_t)G.n_houdayer + M > 4294967295ull))
         return fail(PT_ERR_OVERFLOW, "a step counter would overflow");
     if (n_mcs == 0 || (n_metro == 0 && !do_houdayer && !do_exchange)) return PT_OK;
-    if (mcs_fused_eligible(nullptr, do_houdayer)) {
+    if (do_houdayer != 2 && mcs_fused_eligible(nullptr, do_houdayer)) {
         const McsArgs a{n_mcs, n_metro, do_houdayer ? 1 : 0, do_exchange ? 1 : 0, mcs_split_chains(do_houdayer) ? 1 : 0,
-                        G.n_sweep, G.n_houdayer, G.n_exchange};
+                        G.max_clu, G.n_sweep, G.n_houdayer, G.n_exchange};
         CK(launch_mcs(a));
         G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
         if (do_houdayer) G.n_houdayer += (uint32_t)M;
@@ -615,7 +681,7 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
     }
     for (int m = 0; m < n_mcs; ++m) {
         if (n_metro > 0) { CK(launch_sweep(n_metro)); G.n_sweep += (uint32_t)n_metro; }
-        if (do_houdayer) { CK(launch_houdayer_any()); G.n_houdayer += 1; }
+        if (do_houdayer) { CK(launch_houdayer_any(do_houdayer)); G.n_houdayer += 1; }
         if (do_exchange) { CK(launch_exchange()); G.n_exchange += 1; }
     }
     return PT_OK;

@@ -21,7 +21,7 @@ def lib():
 def test_header_symbols_all_exported(lib):
     hdr = open(os.path.join(ROOT, "include", "ptglass.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    names = set(re.findall(r"\b(pt_[a-z_]+|houdayer_step)\s*\(", hdr))
+    names = set(re.findall(r"\b(pt_[a-z_]+|houdayer_step|houdayer_multi_step)\s*\(", hdr))
     assert names == set(B.SYMBOLS), names ^ set(B.SYMBOLS)
     for n in names:
         assert hasattr(lib, n)
