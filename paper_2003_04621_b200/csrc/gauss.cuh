@@ -21,16 +21,52 @@ __device__ __forceinline__ uint32_t thr_double(double x)
     return (uint32_t)v;
 }
 
-// u < THR(x) decided exactly, cheaply: a float estimate of 2^32 e^x brackets the double threshold (the error of __expf
-// for |x| <= 23 is below 4e-6 relative, (float)x and (float)u add 2e-6; the bracket is 1e-4 wide), and only a draw that
-// falls inside the bracket (probability ~2e-4 p) pays for the double evaluation.  Same decision as thr_double(x) always.
-__device__ __forceinline__ bool accept_exp(uint32_t u, double x)
+// Uphill move with a = s_i h_i > 0 (units of 2^-fbits): accept iff u < THR(x), x = -(beta * ldexp(2a, -fbits)) (R34), decided
+// EXACTLY but cheaply.  Let Y = 2^32 e^x; u < floor(Y) <=> u + 1 <= Y.  A float estimate t9 of y9 = Y / 512 = 2^(23 + a c2),
+// c2 = (float)(-2 beta 2^-fbits log2 e), is off by at most 1e-5 relative: (float)a is exact below 2^23, the fma rounds once
+// (<= 2^-18 absolute in the exponent for |exponent| < 128), c2 carries 2^-24 relative of an exponent of magnitude < 150, and
+// ex2.approx is good to 2^-22.  With u9 = u >> 9 (512 u9 <= u < 512 (u9 + 1); 23 bits, exactly representable in float):
+//   u9 + 2 < 0.9999 t9   =>  u + 1 <= 512 (u9 + 1) < 512 (y9 - 1) < Y            => accept;
+//   u9 > 1.0001 t9 + 1   =>  u >= 512 u9 > Y                                      => reject
+// (the float products add < 2e-7 relative, far inside the 1e-4 bracket; the oracle's double exp is within 1e-16 of Y).
+// Only a draw inside the bracket (probability ~2e-4 of an uphill attempt) or a >= 2^23 pays for the double evaluation,
+// which is the oracle's formula.  Same decision as u < thr_double(x) always.
+__device__ __forceinline__ float ex2_approx(float x)
 {
-    const float t = __expf((float)x) * 4294967296.0f;
-    const float uf = (float)u;
-    if (uf < t * 0.9999f - 1.0f) return true;
-    if (uf > t * 1.0001f + 1.0f) return false;
-    return u < thr_double(x);
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// the rare exact evaluation, kept out of line so the 32 unrolled site decisions stay small
+__device__ __noinline__ bool accept_exact(uint32_t u, int a, const double *beta_ptr, int fbits)
+{
+    return u < thr_double(-(*beta_ptr * ldexp((double)(2LL * a), -fbits)));
+}
+
+// Decision for one site, branch-free except for the rare exact evaluation: a <= 0 always flips.
+// SMALL: the host has checked 2 D max|Jq| < 2^23, so every a is below 2^23 and the range test is dropped.
+template <bool SMALL>
+__device__ __forceinline__ bool accept_site(uint32_t u, int a, float c2, const double *beta_ptr, int fbits)
+{
+    const float af = __int_as_float(0x4B000000 + a) - 8388608.0f;              // exact for 0 <= a < 2^23 (unused otherwise)
+    const float t9 = ex2_approx(fmaf(af, c2, 23.0f));
+    const float uf9 = __uint_as_float(0x4B000000u | (u >> 9)) - 8388608.0f;    // exact: 23 bits fill the mantissa
+    const bool up = a > 0;
+    const bool small = SMALL || (uint32_t)a < (1u << 23);
+    const bool sure_acc = small && (uf9 + 2.0f < t9 * 0.9999f);
+    const bool sure_rej = small && (uf9 > fmaf(t9, 1.0001f, 1.0f));
+    bool acc = !up || sure_acc;
+    if (up && !sure_acc && !sure_rej) acc = accept_exact(u, a, beta_ptr, fbits);
+    return acc;
+}
+
+// s -= J if bit j of un is set: one LOP3 with predicate output + one predicated add
+template <int J>
+__device__ __forceinline__ void sub_if_bit(int &s, uint32_t un, int Jv)
+{
+    asm("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tand.b32 t, %1, %3;\n\tsetp.ne.u32 p, t, 0;\n\t@p sub.s32 %0, %0, %2;\n\t}"
+        : "+r"(s) : "r"(un), "r"(Jv), "n"(1u << J));
 }
 
 // natural-order int32 couplings JqNat[S][D][N] -> Jdev[S][2][2D][NHP]
@@ -103,11 +139,31 @@ __global__ void k_energy_q(LAT lat, Params P, int mode)
     }
 }
 
+template <int J> __device__ __forceinline__ int comp(const int4 &v) { return J == 0 ? v.x : J == 1 ? v.y : J == 2 ? v.z : v.w; }
+
+// Site J (0..3) of the current Philox block: un[k] has the block's four sign bits in bits 0..3.
+template <class LAT, bool SMALL, int J>
+__device__ __forceinline__ void sweep_site_q(const uint32_t (&un)[2 * LAT::D], const int4 (&Jv)[2 * LAT::D], uint32_t u, uint32_t vv,
+                                             float c2, const double *beta_ptr, int fbits, uint32_t &nib, int &dE)
+{
+    constexpr int D = LAT::D;
+    int tot = 0, lost = 0;                       // a = sum_k J_k - 2 sum_{k: s_i s_k = -1} J_k
+#pragma unroll
+    for (int k = 0; k < 2 * D; ++k) tot += comp<J>(Jv[k]);
+#pragma unroll
+    for (int k = 0; k < 2 * D; ++k) sub_if_bit<J>(lost, un[k], comp<J>(Jv[k]));
+    const int a = tot + 2 * lost;
+    bool acc = accept_site<SMALL>(u, a, c2, beta_ptr, fbits);
+    if constexpr (!LAT::kFast) acc = acc && (vv & (1u << J));
+    if (acc) { nib |= 1u << J; dE += 2 * a; }
+}
+
 // Metropolis sweeps with fixed-point couplings.  CTA = R replicas of one sample in shared memory; work item = one word =
-// 32 same-colour sites of one replica, walked site by site: h = sum_k J_k s_k (integer), a = s_i h, flip iff a <= 0 or
-// u < THR(-(beta * ldexp(2a, -fbits))).  Same Philox words as the +-J sweep (domain 3).
-// grid: (2T/R groups, S).  dynamic smem: [R][2][W] spins | [R] dE | [R] temperature index
-template <class LAT>
+// 32 same-colour sites of one replica, walked Philox block by Philox block (4 sites): a = s_i h_i = sum_k J_k (s_i s_k)
+// (integer) starts from sum_k J_k and loses 2 J_k for every unsatisfied-sign bit of un_k = s ^ nb_k; flip iff a <= 0 or
+// accept_uphill.  Same Philox words as the +-J sweep (domain 3).
+// grid: (2T/R groups, S).  dynamic smem: [R][2][W] spins | [R] dE | [R] temperature index | [R] c2 (float)
+template <class LAT, bool SMALL>
 __global__ void __launch_bounds__(128) k_sweep_q(LAT lat, Params P, int R, uint32_t step0, int n_sweeps)
 {
     constexpr int D = LAT::D;
@@ -116,12 +172,18 @@ __global__ void __launch_bounds__(128) k_sweep_q(LAT lat, Params P, int R, uint3
     uint32_t *sS = smem;                       // [R][2][W]
     int *sdE = (int *)(sS + R * 2 * W);        // [R]
     int *sT = sdE + R;                         // [R]
+    float *sC2 = (float *)(sT + R);            // [R]
     const int s = blockIdx.y;
     const int q0 = blockIdx.x * R;
     const size_t rep0 = (size_t)s * 2 * P.T + q0;
     const uint32_t g = P.g0 + (uint32_t)s;
     for (int i = threadIdx.x; i < R * 2 * W; i += blockDim.x) sS[i] = P.d.spin[rep0 * 2 * W + i];
-    for (int i = threadIdx.x; i < R; i += blockDim.x) { sdE[i] = 0; sT[i] = P.d.tos[rep0 + i]; }
+    for (int i = threadIdx.x; i < R; i += blockDim.x) {
+        const int t = P.d.tos[rep0 + i];
+        sdE[i] = 0;
+        sT[i] = t;
+        sC2[i] = (float)(-(2.0 * P.d.betasD[t]) * ldexp(1.4426950408889634, -P.fbits));
+    }
     __syncthreads();
 
     for (int it = 0; it < n_sweeps; ++it) {
@@ -131,37 +193,36 @@ __global__ void __launch_bounds__(128) k_sweep_q(LAT lat, Params P, int R, uint3
                 const int qi = item / W, w = item - qi * W;
                 const int q = q0 + qi;
                 const int c = (q >= P.T) ? 1 : 0, r = q - c * P.T;
-                const double beta = P.d.betasD[sT[qi]];
+                const float c2 = sC2[qi];
                 uint32_t *Sown = sS + (qi * 2 + p) * W;
-                uint32_t nb[2 * D];
-                lat.gather(sS + (qi * 2 + (1 - p)) * W, w, p, nb);
-                const uint32_t sw = Sown[w], valid = lat.valid(w);
+                uint32_t un[2 * D];
+                lat.gather(sS + (qi * 2 + (1 - p)) * W, w, p, un);
+                const uint32_t sw = Sown[w];
+                uint32_t vv = lat.valid(w);
+#pragma unroll
+                for (int k = 0; k < 2 * D; ++k) un[k] ^= sw;                   // bit = 1 <=> s_i s_k = -1
                 const Round0Shared r0 = philox_round0_shared(step0 + (uint32_t)it, g, make_tag(DOM_METRO, p, c, r), P.rk);
                 uint32_t flip = 0;
                 int dE = 0;
-#pragma unroll 1
+#pragma unroll 2
                 for (int B = 0; B < 8; ++B) {
-                    if (((valid >> (4 * B)) & 0xFu) == 0u) continue;
-                    uint32_t u[4];
-                    philox4x32_10_shared(8u * (uint32_t)w + (uint32_t)B, r0, P.rk, u[0], u[1], u[2], u[3]);
-                    int4 Jv[2 * D];
+                    if ((vv & 0xFu) != 0u) {
+                        uint32_t u[4];
+                        philox4x32_10_shared(8u * (uint32_t)w + (uint32_t)B, r0, P.rk, u[0], u[1], u[2], u[3]);
+                        int4 Jv[2 * D];
 #pragma unroll
-                    for (int k = 0; k < 2 * D; ++k) Jv[k] = *(const int4 *)(Jp + jdev_index(W, k, B, w));
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        const int b = 4 * B + j;
-                        if (!((valid >> b) & 1u)) continue;
-                        int h = 0;
-#pragma unroll
-                        for (int k = 0; k < 2 * D; ++k) {
-                            const int Jk = (j == 0) ? Jv[k].x : (j == 1) ? Jv[k].y : (j == 2) ? Jv[k].z : Jv[k].w;
-                            h += ((nb[k] >> b) & 1u) ? -Jk : Jk;
-                        }
-                        const int a = ((sw >> b) & 1u) ? -h : h;
-                        bool acc = a <= 0;
-                        if (!acc) acc = accept_exp(u[j], -(beta * ldexp((double)(2LL * a), -P.fbits)));
-                        if (acc) { flip |= 1u << b; dE += 2 * a; }
+                        for (int k = 0; k < 2 * D; ++k) Jv[k] = __ldg((const int4 *)(Jp + jdev_index(W, k, B, w)));
+                        uint32_t nib = 0;
+                        const double *bp = P.d.betasD + sT[qi];
+                        sweep_site_q<LAT, SMALL, 0>(un, Jv, u[0], vv, c2, bp, P.fbits, nib, dE);
+                        sweep_site_q<LAT, SMALL, 1>(un, Jv, u[1], vv, c2, bp, P.fbits, nib, dE);
+                        sweep_site_q<LAT, SMALL, 2>(un, Jv, u[2], vv, c2, bp, P.fbits, nib, dE);
+                        sweep_site_q<LAT, SMALL, 3>(un, Jv, u[3], vv, c2, bp, P.fbits, nib, dE);
+                        flip |= nib << (4 * B);
                     }
+#pragma unroll
+                    for (int k = 0; k < 2 * D; ++k) un[k] >>= 4;
+                    vv >>= 4;
                 }
                 Sown[w] = sw ^ flip;
                 if (dE != 0) atomicAdd(sdE + qi, dE);

@@ -35,6 +35,7 @@ struct Context {
     std::vector<double> betas;
     uint64_t seed = 0;
     uint32_t n_sweep = 0, n_exchange = 0, n_houdayer = 0;
+    bool q_small = false;       // fixed-point couplings with 2 D max|Jq| < 2^23 (gauss.cuh: accept_site<SMALL>)
     int max_clu = 1;            // max over t of the per-temperature cluster-move counts (NEXT-4, R36)
     uint64_t launches = 0;
     size_t stage_bytes = 0;
@@ -280,11 +281,12 @@ cudaError_t launch_sweep(int n)
         const int W = G.P.W, D = G.P.D;
         const int R = sweep_group(G.P.T, W);
         if (G.P.gauss) {
-            const size_t smq = ((size_t)R * 2 * W + 2 * (size_t)R) * 4;
-            err = allow_smem(k_sweep_q<LAT>, smq);
+            const size_t smq = ((size_t)R * 2 * W + 3 * (size_t)R) * 4;
+            auto kq = G.q_small ? k_sweep_q<LAT, true> : k_sweep_q<LAT, false>;
+            err = allow_smem(kq, smq);
             if (err != cudaSuccess) return;
             dim3 gq((unsigned)(2 * G.P.T / R), (unsigned)G.P.S);
-            k_sweep_q<LAT><<<gq, 128, smq, G.stream>>>(lat, G.P, R, G.n_sweep, n);
+            kq<<<gq, 128, smq, G.stream>>>(lat, G.P, R, G.n_sweep, n);
             ++G.launches;
             err = cudaGetLastError();
             return;
@@ -940,6 +942,7 @@ int pt_set_couplings_fixed(const int32_t *Jq, int frac_bits)
     CK(cudaMemcpyAsync(G.P.d.JqNat, Jq, n * 4, cudaMemcpyHostToDevice, G.stream));
     G.P.gauss = 1;
     G.P.fbits = frac_bits;
+    G.q_small = 2LL * G.P.D * maxabs < (1LL << 23);
     k_pack_jq<<<grid_for((long)G.P.S * 2 * 2 * G.P.D * 32 * G.P.W, 256), 256, 0, G.stream>>>(G.P);
     ++G.launches;
     CK(cudaGetLastError());
