@@ -4,12 +4,14 @@
 // index (domain 5, aux = 1: block i_min >> 2, word i_min & 3).
 //
 // One CTA per (sample, temperature); any lattice (coordinates in natural site order).  Components are found by
-// label propagation in shared memory -- the scheme north_star names for the cluster kernel: lab[i] starts as i on the
-// q = -1 sites, every pass takes the minimum over the q = -1 neighbours and then follows the label chain to its
-// current root (pointer jumping; a label is always the index of a site of the same component with a smaller or
-// equal index, so chains end at a site that is its own label).  Only the owner thread of site i writes lab[i] and
-// labels only decrease, so stale reads are harmless; at the fixed point every site of a component carries the
-// component's smallest index, which makes the decision independent of the thread mapping.
+// label equivalence in shared memory -- the scheme north_star names for the cluster kernel: lab[i] starts as i on the
+// q = -1 sites; a pass is (scan) every site takes the minimum label m over its q = -1 neighbours and, if m is smaller
+// than its own label l, lowers the label OF SITE l to m with an atomicMin (it merges the two trees at their roots,
+// not just the site), then (flatten) every site follows its label chain to the root (a label is always the index of
+// a site of the same component with a smaller or equal index, so chains end at a site that is its own label).
+// Merging at the roots converges in a handful of passes where plain neighbour propagation needs one per lattice
+// step.  At the fixed point every site of a component carries the component's smallest index, which makes the
+// decision independent of the thread mapping.
 #pragma once
 #include "kernels.cuh"
 
@@ -17,6 +19,53 @@ namespace ptg {
 
 constexpr uint32_t kNoLabel = 0x7FFFFFFFu;      // q = +1 site (never a valid site index: N*d < 2^31)
 constexpr uint32_t kFlagBit = 0x80000000u;      // set on a root's own label once its coin says "exchange"
+
+// natural-order neighbour / colour / site helpers: shifts and masks on the power-of-two lattices, coordinates otherwise
+template <class LAT, int K>
+__device__ __forceinline__ int nat_neighbour(int i, int L, int D)
+{
+    if constexpr (LAT::kFast) {
+        constexpr int LG = LAT::kLog2L, mu = K >> 1;
+        constexpr int st = 1 << (LG * mu), M = (LAT::L - 1) << (LG * mu);
+        return (i & ~M) | ((i + ((K & 1) ? -st : st)) & M);
+    } else {
+        return neighbour_site(i, K, L, D);
+    }
+}
+
+template <class LAT>
+__device__ __forceinline__ int nat_colour(int i, int L, int D)
+{
+    if constexpr (LAT::kFast) {
+        constexpr int LG = LAT::kLog2L;
+        return (i ^ (i >> LG) ^ (LAT::D == 3 ? (i >> (2 * LG)) : 0)) & 1;
+    } else {
+        return colour_of_site(i, L, D);
+    }
+}
+
+template <class LAT>
+__device__ __forceinline__ int nat_site_of(int h, int p, int L, int D)
+{
+    if constexpr (LAT::kFast) {
+        constexpr int LG = LAT::kLog2L;
+        const int i2 = 2 * h;
+        return i2 + ((p ^ (i2 >> LG) ^ (LAT::D == 3 ? (i2 >> (2 * LG)) : 0)) & 1);
+    } else {
+        return site_of(h, p, L, D);
+    }
+}
+
+template <class LAT, int K>
+__device__ __forceinline__ uint32_t min_neighbour_label(const uint32_t *lab, int i, int L, int D, uint32_t m)
+{
+    if constexpr (K < 2 * LAT::D) {
+        m = min(m, lab[nat_neighbour<LAT, K>(i, L, D)]);          // kNoLabel never wins
+        return min_neighbour_label<LAT, K + 1>(lab, i, L, D, m);
+    } else {
+        return m;
+    }
+}
 
 // dynamic smem: Neg[2][W] | Cl[2][W] | red[2 * nwarps + 2] | lab[N]
 template <class LAT>
@@ -43,23 +92,28 @@ __global__ void __launch_bounds__(256) k_houdayer_multi(LAT lat, Params P, uint3
     }
     __syncthreads();
     for (int i = tid; i < N; i += blockDim.x) {
-        const int p = colour_of_site(i, L, D), h = i >> 1;
+        const int p = nat_colour<LAT>(i, L, D), h = i >> 1;
         lab[i] = ((Neg[p * W + (h >> 5)] >> (h & 31)) & 1u) ? (uint32_t)i : kNoLabel;
     }
     __syncthreads();
 
-    // label propagation to the fixed point
+    // label equivalence to the fixed point
     for (;;) {
         int changed = 0;
-        for (int i = tid; i < N; i += blockDim.x) {
-            const uint32_t cur = lab[i];
-            if (cur == kNoLabel) continue;
-            uint32_t m = cur;
-            for (int k = 0; k < 2 * D; ++k) m = min(m, lab[neighbour_site(i, k, L, D)]);     // kNoLabel never wins
-            for (uint32_t up = lab[m]; up < m; up = lab[m]) m = up;                          // follow the chain to its root
-            if (m < cur) { lab[i] = m; changed = 1; }
+        for (int i = tid; i < N; i += blockDim.x) {                      // scan: merge trees at their roots
+            const uint32_t l = lab[i];
+            if (l == kNoLabel) continue;
+            const uint32_t m = min_neighbour_label<LAT, 0>(lab, i, L, D, l);
+            if (m < l) { atomicMin(lab + l, m); changed = 1; }
         }
         if (!__syncthreads_or(changed)) break;
+        for (int i = tid; i < N; i += blockDim.x) {                      // flatten: every site points at its root
+            uint32_t l = lab[i];
+            if (l == kNoLabel) continue;
+            for (uint32_t up = lab[l]; up != l; up = lab[l]) l = up;
+            lab[i] = l;
+        }
+        __syncthreads();
     }
 
     // one coin per component, thrown by its root (the site that is its own label)
@@ -79,7 +133,7 @@ __global__ void __launch_bounds__(256) k_houdayer_multi(LAT lat, Params P, uint3
         while (x) {
             const int b = __ffs(x) - 1;
             x &= x - 1;
-            const int i = site_of(32 * w + b, p, L, D);
+            const int i = nat_site_of<LAT>(32 * w + b, p, L, D);
             const uint32_t r = lab[i] & ~kFlagBit;
             if (lab[r] & kFlagBit) out |= 1u << b;
         }
