@@ -20,42 +20,6 @@ namespace ptg {
 constexpr uint32_t kNoLabel = 0x7FFFFFFFu;      // q = +1 site (never a valid site index: N*d < 2^31)
 constexpr uint32_t kFlagBit = 0x80000000u;      // set on a root's own label once its coin says "exchange"
 
-// natural-order neighbour / colour / site helpers: shifts and masks on the power-of-two lattices, coordinates otherwise
-template <class LAT, int K>
-__device__ __forceinline__ int nat_neighbour(int i, int L, int D)
-{
-    if constexpr (LAT::kFast) {
-        constexpr int LG = LAT::kLog2L, mu = K >> 1;
-        constexpr int st = 1 << (LG * mu), M = (LAT::L - 1) << (LG * mu);
-        return (i & ~M) | ((i + ((K & 1) ? -st : st)) & M);
-    } else {
-        return neighbour_site(i, K, L, D);
-    }
-}
-
-template <class LAT>
-__device__ __forceinline__ int nat_colour(int i, int L, int D)
-{
-    if constexpr (LAT::kFast) {
-        constexpr int LG = LAT::kLog2L;
-        return (i ^ (i >> LG) ^ (LAT::D == 3 ? (i >> (2 * LG)) : 0)) & 1;
-    } else {
-        return colour_of_site(i, L, D);
-    }
-}
-
-template <class LAT>
-__device__ __forceinline__ int nat_site_of(int h, int p, int L, int D)
-{
-    if constexpr (LAT::kFast) {
-        constexpr int LG = LAT::kLog2L;
-        const int i2 = 2 * h;
-        return i2 + ((p ^ (i2 >> LG) ^ (LAT::D == 3 ? (i2 >> (2 * LG)) : 0)) & 1);
-    } else {
-        return site_of(h, p, L, D);
-    }
-}
-
 template <class LAT, int K>
 __device__ __forceinline__ uint32_t min_neighbour_label(const uint32_t *lab, int i, int L, int D, uint32_t m)
 {

@@ -754,12 +754,54 @@ __global__ void __launch_bounds__(128) k_measure(LAT lat, Params P, int32_t *out
     }
 }
 
+// Same measurement with one WARP per (sample, t) pair and several pairs per CTA: on small lattices (W words per
+// colour <= 128) a CTA per pair is mostly launch overhead.  dynamic smem: W words per warp.
+template <class LAT>
+__global__ void __launch_bounds__(128) k_measure_warp(LAT lat, Params P, int32_t *outQ, int32_t *outQL)
+{
+    constexpr int D = LAT::D;
+    extern __shared__ uint32_t msm[];
+    const int W = lat.words();
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+    const long pair = (long)blockIdx.x * wpb + wib;
+    if (pair >= (long)P.S * P.T) return;
+    const int s = (int)(pair / P.T), t = (int)(pair - (long)s * P.T);
+    uint32_t *NegW = msm + (size_t)wib * W;
+    const size_t repA = rep_index(P, s, 0, P.d.sot[rep_index(P, s, 0, t)]);
+    const size_t repB = rep_index(P, s, 1, P.d.sot[rep_index(P, s, 1, t)]);
+    const uint32_t *Ab = spin_words(P, repA, 0), *Aw = spin_words(P, repA, 1);
+    const uint32_t *Bb = spin_words(P, repB, 0), *Bw = spin_words(P, repB, 1);
+    for (int w = lane; w < W; w += 32) NegW[w] = (Aw[w] ^ Bw[w]) & lat.valid(w);
+    __syncwarp();
+    int nneg = 0, ndiff = 0;
+    for (int w = lane; w < W; w += 32) {
+        const uint32_t v = lat.valid(w), nbk = (Ab[w] ^ Bb[w]) & v;
+        nneg += __popc(nbk) + __popc(NegW[w]);
+        if (outQL) {
+            uint32_t nb[2 * D];
+            lat.gather(NegW, w, 0, nb);
+#pragma unroll
+            for (int k = 0; k < 2 * D; ++k) ndiff += __popc((nbk ^ nb[k]) & v);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        nneg += __shfl_xor_sync(0xFFFFFFFFu, nneg, o);
+        ndiff += __shfl_xor_sync(0xFFFFFFFFu, ndiff, o);
+    }
+    if (lane == 0) {
+        outQ[pair] = P.N - 2 * nneg;
+        if (outQL) outQL[pair] = P.D * P.N - 2 * ndiff;
+    }
+}
+
 // =========================================================================================================
 // NEXT-2  overlap profiles (R31): prof[s][t][mu][x] = sum of q_i over the plane x_mu = x
 //         = L^(D-1) - 2 #(q_i = -1 in that plane).  One CTA per (sample, t); any even L (coordinates from the
 // half-index); only the q = -1 sites touch the shared counters.  dynamic smem: D*L counters.
 // =========================================================================================================
-__global__ void __launch_bounds__(128) k_profile(Params P, int32_t *out)
+template <class LAT>
+__global__ void __launch_bounds__(128) k_profile(LAT lat, Params P, int32_t *out)
 {
     extern __shared__ int pneg[];
     const int t = blockIdx.x, s = blockIdx.y, tid = threadIdx.x;
@@ -776,11 +818,11 @@ __global__ void __launch_bounds__(128) k_profile(Params P, int32_t *out)
         while (x) {
             const int b = __ffs(x) - 1;
             x &= x - 1;
-            Coord c;
-            site_of(32 * w + b, p, P.L, P.D, &c);
-            atomicAdd(pneg + c.x, 1);
-            atomicAdd(pneg + P.L + c.y, 1);
-            if (P.D == 3) atomicAdd(pneg + 2 * P.L + c.z, 1);
+            int cx, cy, cz;
+            nat_coords<LAT>(nat_site_of<LAT>(32 * w + b, p, P.L, P.D), P.L, P.D, cx, cy, cz);
+            atomicAdd(pneg + cx, 1);
+            atomicAdd(pneg + P.L + cy, 1);
+            if (LAT::D == 3) atomicAdd(pneg + 2 * P.L + cz, 1);
         }
     }
     __syncthreads();

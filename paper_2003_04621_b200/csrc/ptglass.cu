@@ -389,9 +389,14 @@ cudaError_t launch_measure(int32_t *Q, int32_t *QL)
     cudaError_t err = cudaSuccess;
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
-        const size_t smem = ((size_t)G.P.W + 2) * 4;
-        dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
-        k_measure<LAT><<<grid, 128, smem, G.stream>>>(lat, G.P, Q, QL);
+        if (G.P.W <= 128) {          // small lattices: one warp per pair, four pairs per CTA
+            const long pairs = (long)G.P.S * G.P.T;
+            k_measure_warp<LAT><<<(unsigned)((pairs + 3) / 4), 128, (size_t)4 * G.P.W * 4, G.stream>>>(lat, G.P, Q, QL);
+        } else {
+            const size_t smem = ((size_t)G.P.W + 2) * 4;
+            dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
+            k_measure<LAT><<<grid, 128, smem, G.stream>>>(lat, G.P, Q, QL);
+        }
         ++G.launches;
         err = cudaGetLastError();
     });
@@ -791,10 +796,15 @@ int pt_measure_overlap_profile_device(int32_t *prof_dev)
     NEED_INIT();
     if (!prof_dev) return fail(PT_ERR_ARG, "prof is NULL");
     ProfScope prof(3);
-    dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
-    k_profile<<<grid, 128, (size_t)G.P.D * G.P.L * sizeof(int), G.stream>>>(G.P, prof_dev);
-    ++G.launches;
-    CK(cudaGetLastError());
+    cudaError_t err = cudaSuccess;
+    with_lattice([&](auto lat) {
+        using LAT = decltype(lat);
+        dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
+        k_profile<LAT><<<grid, 128, (size_t)G.P.D * G.P.L * sizeof(int), G.stream>>>(lat, G.P, prof_dev);
+        ++G.launches;
+        err = cudaGetLastError();
+    });
+    CK(err);
     return PT_OK;
 }
 
