@@ -55,6 +55,9 @@ def parse():
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--gaussian", action="store_true", help="NEXT-3: Gaussian couplings in fixed point (16 fractional bits), separate kernels")
     ap.add_argument("--track-round-trips", action="store_true", help="NEXT-1: tunnelling-time bookkeeping in every PT pass")
+    ap.add_argument("--cluster", default="single", choices=["single", "counts", "multi"],
+                    help="NEXT-4 cluster-move variant of a Houdayer workload: one single-cluster move per temperature (the paper's "
+                         "MCS), per-temperature move counts 4..1 from the hot to the cold end, or the multi-cluster exchange")
     return ap.parse_args()
 
 
@@ -107,16 +110,19 @@ def measured_peaks():
 
 
 # --------------------------------------------------------------------------------------------------------------
-def oracle_time(w, S, n_mcs, seed=wl.SEED, gaussian=False):
+def oracle_time(w, S, n_mcs, seed=wl.SEED, gaussian=False, cluster="single"):
     """Time the oracle as it stands on one host core; returns (flips/ns, seconds, flips)."""
     from oracle import ref
 
     o = ref.Oracle(w.L, w.d, S, w.T, w.betas(), seed)
     if gaussian:
         o.set_couplings_fixed(wl.gaussian_couplings_fixed(seed, S, w.d, w.N, 16), 16)
+    hd = (2 if cluster == "multi" else 1) if w.houdayer else 0
+    if w.houdayer and cluster == "counts":
+        o.set_cluster_moves(np.array([1 + (3 * t) // max(w.T - 1, 1) for t in range(w.T)], dtype=np.int32)[::-1].copy())
     t0 = time.perf_counter()
     for m in range(1, n_mcs + 1):
-        o.mcs(1, 1, w.houdayer, True)
+        o.mcs(1, 1, hd, True)
         if w.measure_every and m % w.measure_every == 0:
             o.measure_overlap()
     dt = time.perf_counter() - t0
@@ -136,8 +142,12 @@ def run_reference(a, w, rank):
     if a.gaussian:
         o.set_couplings_fixed(wl.gaussian_couplings_fixed(wl.SEED, S_ref, w.d, w.N, 16), 16)
 
+    hd = (2 if a.cluster == "multi" else 1) if w.houdayer else 0
+    if w.houdayer and a.cluster == "counts":
+        o.set_cluster_moves(np.array([1 + (3 * t) // max(w.T - 1, 1) for t in range(w.T)], dtype=np.int32)[::-1].copy())
+
     def step():
-        o.mcs(a.mcs_per_step, 1, w.houdayer, True)
+        o.mcs(a.mcs_per_step, 1, hd, True)
         if w.measure_every:
             for _ in range(a.mcs_per_step // w.measure_every):
                 o.measure_overlap()
@@ -168,7 +178,9 @@ def config_of(a, w, n_gpus, sample=None):
          "mcs_per_step": a.mcs_per_step, "mcs_order": "sweep" + (", houdayer" if w.houdayer else "") + ", exchange",
          "measure_every": w.measure_every, "seed": wl.SEED, "parallelism": "samples sharded x%d" % n_gpus,
          "l2": "flushed between steps (512 MiB write, untimed)", "round_trip_tracking": bool(a.track_round_trips),
-         "couplings": "gaussian, fixed point 2^-16 (NEXT-3)" if a.gaussian else "+-J, p = 1/2"}
+         "couplings": "gaussian, fixed point 2^-16 (NEXT-3)" if a.gaussian else "+-J, p = 1/2",
+         "cluster_move": {"single": "one single-cluster move per temperature", "counts": "single-cluster moves, counts 4..1 hot to cold (NEXT-4)",
+                          "multi": "multi-cluster exchange (NEXT-4)"}[a.cluster] if w.houdayer else "none"}
     if sample:
         c["sample"] = sample
     return c
@@ -210,13 +222,16 @@ def main():
     Qd = torch.empty((w.S, w.T), dtype=torch.int32, device=dev)
     QLd = torch.empty((w.S, w.T), dtype=torch.int32, device=dev)
     n_meas = (a.mcs_per_step // w.measure_every) if w.measure_every else 0
+    hd = (2 if a.cluster == "multi" else 1) if w.houdayer else 0
+    if w.houdayer and a.cluster == "counts":       # index 0 is the lowest beta = the hot end
+        B.pt_set_cluster_moves(np.array([1 + (3 * t) // max(w.T - 1, 1) for t in range(w.T)], dtype=np.int32)[::-1].copy())
 
     def step():
         if n_meas == 0:
-            B.pt_mcs(a.mcs_per_step, 1, w.houdayer, True)
+            B.pt_mcs(a.mcs_per_step, 1, hd, True)
         else:
             for _ in range(n_meas):
-                B.pt_mcs(w.measure_every, 1, w.houdayer, True)
+                B.pt_mcs(w.measure_every, 1, hd, True)
                 B.pt_measure_overlap_device(Qd, QLd)
 
     def barrier():
@@ -328,7 +343,7 @@ def main():
     cpu = None
     if not a.no_cpu_baseline:
         S_cpu, mcs_cpu = 4, max(1, int(3.0e8 / (w.flips_per_sweep(4))))
-        v, dt, flips = oracle_time(w, S_cpu, mcs_cpu, gaussian=a.gaussian)
+        v, dt, flips = oracle_time(w, S_cpu, mcs_cpu, gaussian=a.gaussian, cluster=a.cluster)
         cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
                "sample": "%s restricted to the first %d samples x %d MCS (%.2e flips), same MCS order" % (w.name, S_cpu, mcs_cpu, flips)}
 
