@@ -142,6 +142,20 @@ def test_multi_cluster_special_cases_on_device():
     assert (B.pt_get_cluster_sizes()[0] == 0).all() and np.array_equal(B.pt_get_spins(), s4)
 
 
+def test_multi_cluster_label_array_must_fit_shared_memory():
+    B.pt_open(256, 2, 1, 2, [0.5, 0.9], wl.SEED)          # 65 536 sites: 256 KiB of labels per pair
+    st0 = B.state()
+    for fn in (B.houdayer_multi_step, lambda: B.pt_mcs(1, 1, 2, True)):
+        with pytest.raises(B.PTError) as e:
+            fn()
+        assert e.value.code == B.PT_ERR_ARG
+    st1 = B.state()
+    for k in st0:
+        assert np.array_equal(st0[k], st1[k]), k           # a refused call leaves the state and the counters alone
+    B.houdayer_step()                                      # the single-cluster move still runs at this size
+    assert B.pt_recompute_energy()[1] == 0
+
+
 @pytest.mark.parametrize("name,n_mcs", [("C2", 30), ("C5", 8)])
 def test_variants_full_size_sampled(name, n_mcs):
     """Full L, T, S of the config; samples {0, S/2, S-1} recomputed by the oracle through sample_offset."""

@@ -63,7 +63,9 @@ SHAPES = [(8, 2, 4, 8), (16, 2, 3, 5), (32, 2, 3, 6), (64, 2, 2, 3), (128, 2, 1,
           (2, 2, 2, 3), (4, 2, 3, 4), (6, 2, 2, 5), (10, 2, 2, 3), (12, 2, 1, 2), (20, 2, 1, 2),
           (2, 3, 3, 3), (4, 3, 2, 4), (6, 3, 2, 3), (10, 3, 1, 2),
           # long ladders: several 32-temperature groups in the lane-per-pair Houdayer phase of the fused kernel
-          (16, 2, 1, 70), (8, 2, 1, 130), (32, 2, 1, 48), (8, 3, 1, 33)]
+          (16, 2, 1, 70), (8, 2, 1, 130), (32, 2, 1, 48), (8, 3, 1, 33),
+          # the largest lattices of the word-parallel path
+          (256, 2, 1, 2), (32, 3, 1, 2)]
 
 
 @pytest.mark.parametrize("L,d,S,T", SHAPES)
