@@ -53,7 +53,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)
-    ap.add_argument("--gaussian", action="store_true", help="NEXT-3: Gaussian couplings in fixed point (16 fractional bits), separate kernels")
+    ap.add_argument("--gaussian", action="store_true", help="NEXT-3: Gaussian couplings in fixed point (16 fractional bits)")
     ap.add_argument("--track-round-trips", action="store_true", help="NEXT-1: tunnelling-time bookkeeping in every PT pass")
     ap.add_argument("--cluster", default="single", choices=["single", "counts", "multi"],
                     help="NEXT-4 cluster-move variant of a Houdayer workload: one single-cluster move per temperature (the paper's "

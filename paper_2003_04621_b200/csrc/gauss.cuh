@@ -158,10 +158,85 @@ __device__ __forceinline__ void sweep_site_q(const uint32_t (&un)[2 * LAT::D], c
     if (acc) { nib |= 1u << J; dE += 2 * a; }
 }
 
-// Metropolis sweeps with fixed-point couplings.  CTA = R replicas of one sample in shared memory; work item = one word =
-// 32 same-colour sites of one replica, walked Philox block by Philox block (4 sites): a = s_i h_i = sum_k J_k (s_i s_k)
-// (integer) starts from sum_k J_k and loses 2 J_k for every unsatisfied-sign bit of un_k = s ^ nb_k; flip iff a <= 0 or
-// accept_uphill.  Same Philox words as the +-J sweep (domain 3).
+// One work item of the fixed-point sweep = one word = 32 same-colour sites of one replica, walked Philox block by Philox
+// block (4 sites): a = s_i h_i = sum_k J_k (s_i s_k) (integer) starts from sum_k J_k and loses 2 J_k for every
+// unsatisfied-sign bit of un_k = s ^ nb_k; flip iff a <= 0 or the exact bracket test.  Same Philox words as the +-J sweep
+// (domain 3).  Sown / Soth: the replica's words of colour p / 1-p (shared memory); Jp: the sample's colour-p block of Jdev
+// (global, read through L1).  Returns the energy change of the replica.
+template <class LAT, bool SMALL>
+__device__ __forceinline__ int update_word_q(const LAT &lat, uint32_t *Sown, const uint32_t *Soth, const int32_t *Jp, int W,
+                                             int w, int p, float c2, const double *beta_ptr, int fbits, uint32_t step,
+                                             uint32_t g, uint32_t tag, const RoundKeys &rk)
+{
+    constexpr int D = LAT::D;
+    uint32_t un[2 * D];
+    lat.gather(Soth, w, p, un);
+    const uint32_t sw = Sown[w];
+    uint32_t vv = lat.valid(w);
+#pragma unroll
+    for (int k = 0; k < 2 * D; ++k) un[k] ^= sw;                   // bit = 1 <=> s_i s_k = -1
+    const Round0Shared r0 = philox_round0_shared(step, g, tag, rk);
+    uint32_t flip = 0;
+    int dE = 0;
+#pragma unroll 2
+    for (int B = 0; B < 8; ++B) {
+        if ((vv & 0xFu) != 0u) {
+            uint32_t u[4];
+            philox4x32_10_shared(8u * (uint32_t)w + (uint32_t)B, r0, rk, u[0], u[1], u[2], u[3]);
+            int4 Jv[2 * D];
+#pragma unroll
+            for (int k = 0; k < 2 * D; ++k) Jv[k] = __ldg((const int4 *)(Jp + jdev_index(W, k, B, w)));
+            uint32_t nib = 0;
+            sweep_site_q<LAT, SMALL, 0>(un, Jv, u[0], vv, c2, beta_ptr, fbits, nib, dE);
+            sweep_site_q<LAT, SMALL, 1>(un, Jv, u[1], vv, c2, beta_ptr, fbits, nib, dE);
+            sweep_site_q<LAT, SMALL, 2>(un, Jv, u[2], vv, c2, beta_ptr, fbits, nib, dE);
+            sweep_site_q<LAT, SMALL, 3>(un, Jv, u[3], vv, c2, beta_ptr, fbits, nib, dE);
+            flip |= nib << (4 * B);
+        }
+#pragma unroll
+        for (int k = 0; k < 2 * D; ++k) un[k] >>= 4;
+        vv >>= 4;
+    }
+    Sown[w] = sw ^ flip;
+    return dE;
+}
+
+// sum over the 32 black sites of word w of a_i = s_i h_i (every bond has exactly one black endpoint, so E = -sum over the
+// black sites of a_i).  Sb / Sw: the replica's black / white words; Jb: the sample's colour-0 block of Jdev.
+template <class LAT>
+__device__ __forceinline__ int field_sum_word_q(const LAT &lat, const uint32_t *Sb, const uint32_t *Sw, const int32_t *Jb, int W,
+                                                int w)
+{
+    constexpr int D = LAT::D;
+    uint32_t un[2 * D];
+    lat.gather(Sw, w, 0, un);
+    const uint32_t sb = Sb[w];
+    uint32_t vv = lat.valid(w);
+#pragma unroll
+    for (int k = 0; k < 2 * D; ++k) un[k] ^= sb;
+    int sum = 0;
+#pragma unroll 2
+    for (int B = 0; B < 8; ++B) {
+#pragma unroll
+        for (int k = 0; k < 2 * D; ++k) {
+            const int4 J4 = __ldg((const int4 *)(Jb + jdev_index(W, k, B, w)));
+            const uint32_t u4 = un[k], v4 = vv;
+            if (v4 & 1u) sum += (u4 & 1u) ? -J4.x : J4.x;
+            if (v4 & 2u) sum += (u4 & 2u) ? -J4.y : J4.y;
+            if (v4 & 4u) sum += (u4 & 4u) ? -J4.z : J4.z;
+            if (v4 & 8u) sum += (u4 & 8u) ? -J4.w : J4.w;
+        }
+#pragma unroll
+        for (int k = 0; k < 2 * D; ++k) un[k] >>= 4;
+        vv >>= 4;
+    }
+    return sum;
+}
+
+// c2 of accept_site for inverse temperature beta: (float)(-2 beta 2^-fbits log2 e)
+__device__ __forceinline__ float bracket_slope(double beta, int fbits) { return (float)(-(2.0 * beta) * ldexp(1.4426950408889634, -fbits)); }
+
+// Metropolis sweeps with fixed-point couplings, separate kernel.  CTA = R replicas of one sample in shared memory.
 // grid: (2T/R groups, S).  dynamic smem: [R][2][W] spins | [R] dE | [R] temperature index | [R] c2 (float)
 template <class LAT, bool SMALL>
 __global__ void __launch_bounds__(128) k_sweep_q(LAT lat, Params P, int R, uint32_t step0, int n_sweeps)
@@ -182,7 +257,7 @@ __global__ void __launch_bounds__(128) k_sweep_q(LAT lat, Params P, int R, uint3
         const int t = P.d.tos[rep0 + i];
         sdE[i] = 0;
         sT[i] = t;
-        sC2[i] = (float)(-(2.0 * P.d.betasD[t]) * ldexp(1.4426950408889634, -P.fbits));
+        sC2[i] = bracket_slope(P.d.betasD[t], P.fbits);
     }
     __syncthreads();
 
@@ -193,38 +268,9 @@ __global__ void __launch_bounds__(128) k_sweep_q(LAT lat, Params P, int R, uint3
                 const int qi = item / W, w = item - qi * W;
                 const int q = q0 + qi;
                 const int c = (q >= P.T) ? 1 : 0, r = q - c * P.T;
-                const float c2 = sC2[qi];
-                uint32_t *Sown = sS + (qi * 2 + p) * W;
-                uint32_t un[2 * D];
-                lat.gather(sS + (qi * 2 + (1 - p)) * W, w, p, un);
-                const uint32_t sw = Sown[w];
-                uint32_t vv = lat.valid(w);
-#pragma unroll
-                for (int k = 0; k < 2 * D; ++k) un[k] ^= sw;                   // bit = 1 <=> s_i s_k = -1
-                const Round0Shared r0 = philox_round0_shared(step0 + (uint32_t)it, g, make_tag(DOM_METRO, p, c, r), P.rk);
-                uint32_t flip = 0;
-                int dE = 0;
-#pragma unroll 2
-                for (int B = 0; B < 8; ++B) {
-                    if ((vv & 0xFu) != 0u) {
-                        uint32_t u[4];
-                        philox4x32_10_shared(8u * (uint32_t)w + (uint32_t)B, r0, P.rk, u[0], u[1], u[2], u[3]);
-                        int4 Jv[2 * D];
-#pragma unroll
-                        for (int k = 0; k < 2 * D; ++k) Jv[k] = __ldg((const int4 *)(Jp + jdev_index(W, k, B, w)));
-                        uint32_t nib = 0;
-                        const double *bp = P.d.betasD + sT[qi];
-                        sweep_site_q<LAT, SMALL, 0>(un, Jv, u[0], vv, c2, bp, P.fbits, nib, dE);
-                        sweep_site_q<LAT, SMALL, 1>(un, Jv, u[1], vv, c2, bp, P.fbits, nib, dE);
-                        sweep_site_q<LAT, SMALL, 2>(un, Jv, u[2], vv, c2, bp, P.fbits, nib, dE);
-                        sweep_site_q<LAT, SMALL, 3>(un, Jv, u[3], vv, c2, bp, P.fbits, nib, dE);
-                        flip |= nib << (4 * B);
-                    }
-#pragma unroll
-                    for (int k = 0; k < 2 * D; ++k) un[k] >>= 4;
-                    vv >>= 4;
-                }
-                Sown[w] = sw ^ flip;
+                const int dE = update_word_q<LAT, SMALL>(lat, sS + (qi * 2 + p) * W, sS + (qi * 2 + (1 - p)) * W, Jp, W, w, p, sC2[qi],
+                                                         P.d.betasD + sT[qi], P.fbits, step0 + (uint32_t)it, g,
+                                                         make_tag(DOM_METRO, p, c, r), P.rk);
                 if (dE != 0) atomicAdd(sdE + qi, dE);
             }
             __syncthreads();

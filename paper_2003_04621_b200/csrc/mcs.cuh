@@ -9,6 +9,7 @@
 #pragma once
 #include "kernels.cuh"
 #include "houdayer_lanes.cuh"
+#include "gauss.cuh"
 
 namespace ptg {
 
@@ -23,7 +24,7 @@ struct McsArgs {
 // A replica occupies RS = 2W + 1 words (colour 0 | colour 1 | pad): the odd stride lets 32 lanes that each own a
 // different replica (lane-per-pair Houdayer) hit 32 different banks.
 struct McsSmem {
-    int RS, oJ, oS, oE, oTos, oSot, oThr, oAcc, oLast, oCum, oU, oSgn, oScr, words;
+    int RS, oJ, oS, oE, oTos, oSot, oThr, oAcc, oLast, oCum, oU, oSgn, oC2, oScr, words;
     // nch: chains held by the CTA (2 = the whole sample, 1 = one chain)
     __host__ __device__ McsSmem(int D, int W, int T, int nwarps, bool lanes, int nch)
     {
@@ -42,6 +43,7 @@ struct McsSmem {
         oCum = o;  o += 2 * T;              // 64-bit
         oU = o;    o += 2 * T;              // PT draws of the current pass, [chain][pair]
         oSgn = o;  o += T;
+        oC2 = o;   o += 2 * T;              // fixed-point couplings: bracket slope per replica (float)
         oScr = o;
         if (nch < 2) {
             // no Houdayer phase, no scratch
@@ -55,7 +57,11 @@ struct McsSmem {
     }
 };
 
-template <class LAT, int NT, int MINB>
+// GAUSS: 0 = +-J bit couplings; 1 / 2 = fixed-point couplings (gauss.cuh) with / without the host's range guarantee
+// 2 D max|Jq| < 2^23.  With fixed-point couplings the sweep walks its word site by site (update_word_q), the energies are
+// recomputed from scratch after the cluster moves (field_sum_word_q; the cluster itself depends on q only) and the PT walk
+// evaluates its thresholds in double (swap_threshold).
+template <class LAT, int NT, int MINB, int GAUSS>
 __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
 {
     constexpr int D = LAT::D, W = LAT::W, NWARPS = NT / 32;
@@ -68,6 +74,7 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
     constexpr int RS = 2 * W + 1;
     uint32_t *sJ = msm + L.oJ, *sS = msm + L.oS, *sThr = msm + L.oThr, *sAcc = msm + L.oAcc, *sLast = msm + L.oLast;
     uint32_t *sU = msm + L.oU;
+    float *sC2 = (float *)(msm + L.oC2);
     int *sE = (int *)(msm + L.oE), *sTos = (int *)(msm + L.oTos), *sSot = (int *)(msm + L.oSot), *sSgn = (int *)(msm + L.oSgn);
     unsigned long long *sCum = (unsigned long long *)(msm + L.oCum);
     const int s = a.split_chains ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
@@ -89,6 +96,7 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
         sAcc[i] = 0;
 #pragma unroll
         for (int k = 0; k < 4; ++k) sThr[4 * i + k] = P.d.thrM[4 * t + k];
+        if constexpr (GAUSS != 0) sC2[i] = bracket_slope(P.d.betasD[t], P.fbits);
     }
     for (int i = tid; i < T; i += NT) {
         sLast[i] = P.d.last[(size_t)s * T + i];
@@ -106,11 +114,18 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                 for (int item = tid; item < R * W; item += NT) {
                     const int q = item / W, w = item - q * W;
                     const int cl = (q >= T) ? 1 : 0, r = q - cl * T, c = c0 + cl;
-                    uint32_t thr[D];
+                    int dE;
+                    if constexpr (GAUSS != 0) {
+                        dE = update_word_q<LAT, GAUSS == 1>(lat, sS + q * RS + p * W, sS + q * RS + (1 - p) * W,
+                                                            P.d.Jdev + ((size_t)s * 2 + p) * (2 * D) * (32 * W), W, w, p, sC2[q],
+                                                            P.d.betasD + sTos[q], P.fbits, step, g, make_tag(DOM_METRO, p, c, r), P.rk);
+                    } else {
+                        uint32_t thr[D];
 #pragma unroll
-                    for (int k = 0; k < D; ++k) thr[k] = sThr[4 * q + k];
-                    const int dE = update_word(lat, sS + q * RS + p * W, sS + q * RS + (1 - p) * W, sJ + p * 2 * D * W, W, w,
-                                               p, thr, step, g, make_tag(DOM_METRO, p, c, r), P.rk);
+                        for (int k = 0; k < D; ++k) thr[k] = sThr[4 * q + k];
+                        dE = update_word(lat, sS + q * RS + p * W, sS + q * RS + (1 - p) * W, sJ + p * 2 * D * W, W, w,
+                                         p, thr, step, g, make_tag(DOM_METRO, p, c, r), P.rk);
+                    }
                     if (dE != 0) atomicAdd(sE + q, dE);
                 }
                 __syncthreads();
@@ -173,6 +188,19 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                 }
             }
             __syncthreads();
+            if constexpr (GAUSS != 0) {
+                // the cluster kernels counted +-1 bonds: recompute every energy from the couplings' values
+                for (int i = tid; i < R; i += NT) sE[i] = 0;
+                __syncthreads();
+                const int32_t *Jb = P.d.Jdev + (size_t)s * 2 * (2 * D) * (32 * W);          // colour-0 block
+#pragma unroll 1
+                for (int item = tid; item < R * W; item += NT) {
+                    const int q = item / W, w = item - q * W;
+                    const int e = field_sum_word_q(lat, sS + q * RS, sS + q * RS + W, Jb, W, w);
+                    if (e != 0) atomicAdd(sE + q, -e);
+                }
+                __syncthreads();
+            }
         }
         // ---- a4: PT pass (R9: sequential walk, each step seeing the previous).  Warp 0: all lanes draw the Philox
         // words, then one lane per chain walks its ladder; only the two index maps change.
@@ -212,8 +240,10 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                 }
             }
             __syncthreads();
-            for (int i = tid; i < R; i += NT)
-                *(uint4 *)(sThr + 4 * i) = __ldg((const uint4 *)(P.d.thrM + 4 * sTos[i]));
+            for (int i = tid; i < R; i += NT) {
+                if constexpr (GAUSS != 0) sC2[i] = bracket_slope(P.d.betasD[sTos[i]], P.fbits);
+                else *(uint4 *)(sThr + 4 * i) = __ldg((const uint4 *)(P.d.thrM + 4 * sTos[i]));
+            }
             __syncthreads();
         }
     }

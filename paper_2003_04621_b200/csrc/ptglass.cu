@@ -413,7 +413,7 @@ bool mcs_split_chains(int do_houdayer) { return !do_houdayer && (long)G.P.T * G.
 
 bool mcs_fused_eligible(size_t *smem_out, int do_houdayer = 1)
 {
-    if (!G.fast || G.fused_mode == 0 || G.P.gauss) return false;
+    if (!G.fast || G.fused_mode == 0) return false;
     const McsSmem lay(G.P.D, G.P.W, G.P.T, kMcsThreads / 32, 2 * G.P.W <= 32, mcs_split_chains(do_houdayer) ? 1 : 2);
     const size_t smem = (size_t)lay.words * 4;
     if (smem_out) *smem_out = smem;
@@ -429,7 +429,8 @@ cudaError_t launch_mcs(const McsArgs &a)
         if constexpr (LAT::kFast) {
             size_t smem = 0;
             mcs_fused_eligible(&smem, a.do_houdayer);
-            auto kern = k_mcs<LAT, kMcsThreads, kMcsMinBlocks>;
+            auto kern = !G.P.gauss ? k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 0>
+                        : G.q_small ? k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 1> : k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 2>;
             err = allow_smem(kern, smem);
             if (err != cudaSuccess) return;
             const unsigned grid = (unsigned)G.P.S * (a.split_chains ? 2u : 1u);

@@ -30,7 +30,9 @@ def same_state(o, tag):
 
 @pytest.mark.parametrize("L,d,S,T,fbits,general", [
     (8, 2, 3, 5, 16, False), (32, 2, 2, 6, 16, False), (64, 2, 1, 3, 12, False), (8, 3, 2, 4, 16, False), (16, 3, 1, 3, 14, False),
-    (4, 2, 2, 3, 16, False), (6, 3, 2, 3, 10, False), (10, 2, 1, 4, 16, False), (16, 2, 2, 4, 16, True)])
+    (4, 2, 2, 3, 16, False), (6, 3, 2, 3, 10, False), (10, 2, 1, 4, 16, False), (16, 2, 2, 4, 16, True),
+    (8, 2, 3, 5, 21, False),            # 2 d max|Jq| >= 2^23: the kernels with the per-site range test
+    (32, 2, 1, 40, 16, False)])         # two 32-temperature groups in the fused kernel's cluster phase
 def test_gaussian_couplings_match_oracle(L, d, S, T, fbits, general):
     betas = wl.betas_geometric(0.2, 1.4, T)
     Jq = wl.gaussian_couplings_fixed(wl.SEED, S, d, L ** d, fbits, sample_offset=2)
@@ -50,9 +52,15 @@ def test_gaussian_couplings_match_oracle(L, d, S, T, fbits, general):
         same_state(o, "exchange %d" % step)
     o.sweep(3); B.pt_sweep(3)
     same_state(o, "sweep(3)")
-    o.mcs(20, 2, True, True); B.pt_mcs(20, 2, True, True)
+    o.mcs(20, 2, True, True); B.pt_mcs(20, 2, True, True)      # ONE fused launch on the word-parallel lattices
     same_state(o, "mcs")
-    assert B.pt_get_fused() == 0
+    assert B.pt_get_fused() == int(B.pt_get_path() == 1)
+    B.pt_set_fused(0)
+    o.mcs(4, 1, True, True); B.pt_mcs(4, 1, True, True)        # the separate kernels
+    same_state(o, "mcs, separate kernels")
+    B.pt_set_fused(-1)
+    o.mcs(3, 1, False, True); B.pt_mcs(3, 1, False, True)      # no cluster move: no energy recompute in the fused kernel
+    same_state(o, "mcs without the cluster move")
 
 
 def test_pm_one_in_fixed_point_equals_the_pmJ_path_on_the_device():
