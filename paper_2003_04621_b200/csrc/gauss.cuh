@@ -201,36 +201,56 @@ __device__ __forceinline__ int update_word_q(const LAT &lat, uint32_t *Sown, con
     return dE;
 }
 
-// sum over the 32 black sites of word w of a_i = s_i h_i (every bond has exactly one black endpoint, so E = -sum over the
-// black sites of a_i).  Sb / Sw: the replica's black / white words; Jb: the sample's colour-0 block of Jdev.
+// Energy of a replica from the couplings' values, every bond seen from its black endpoint:
+//   E = -sum_bonds J s_i s_j = -(sum_bonds J) + 2 * sum over the bonds with s_i s_j = -1 of J.
+// bond_sum_word_q: sum over the 32 black sites of word w and their 2D directions of J (a constant of the sample);
+// unsat_sum_word_q: the same sum restricted to the bonds with s_i s_j = -1 (one predicate-setting LOP3 and one predicated
+// subtract per bond; returns minus the sum).  Sb / Sw: the replica's black / white words; Jb: colour-0 block of Jdev.
 template <class LAT>
-__device__ __forceinline__ int field_sum_word_q(const LAT &lat, const uint32_t *Sb, const uint32_t *Sw, const int32_t *Jb, int W,
+__device__ __forceinline__ int bond_sum_word_q(const LAT &lat, const int32_t *Jb, int W, int w)
+{
+    constexpr int D = LAT::D;
+    uint32_t vv = lat.valid(w);
+    int sum = 0;
+    for (int B = 0; B < 8; ++B) {
+#pragma unroll
+        for (int k = 0; k < 2 * D; ++k) {
+            const int4 J4 = __ldg((const int4 *)(Jb + jdev_index(W, k, B, w)));
+            if (vv & 1u) sum += J4.x;
+            if (vv & 2u) sum += J4.y;
+            if (vv & 4u) sum += J4.z;
+            if (vv & 8u) sum += J4.w;
+        }
+        vv >>= 4;
+    }
+    return sum;
+}
+
+template <class LAT>
+__device__ __forceinline__ int unsat_sum_word_q(const LAT &lat, const uint32_t *Sb, const uint32_t *Sw, const int32_t *Jb, int W,
                                                 int w)
 {
     constexpr int D = LAT::D;
     uint32_t un[2 * D];
     lat.gather(Sw, w, 0, un);
-    const uint32_t sb = Sb[w];
-    uint32_t vv = lat.valid(w);
+    const uint32_t sb = Sb[w], v = lat.valid(w);
 #pragma unroll
-    for (int k = 0; k < 2 * D; ++k) un[k] ^= sb;
-    int sum = 0;
+    for (int k = 0; k < 2 * D; ++k) un[k] = (un[k] ^ sb) & v;
+    int lost = 0;                                   // = -(sum of J over the unsatisfied-sign bonds)
 #pragma unroll 2
     for (int B = 0; B < 8; ++B) {
 #pragma unroll
         for (int k = 0; k < 2 * D; ++k) {
             const int4 J4 = __ldg((const int4 *)(Jb + jdev_index(W, k, B, w)));
-            const uint32_t u4 = un[k], v4 = vv;
-            if (v4 & 1u) sum += (u4 & 1u) ? -J4.x : J4.x;
-            if (v4 & 2u) sum += (u4 & 2u) ? -J4.y : J4.y;
-            if (v4 & 4u) sum += (u4 & 4u) ? -J4.z : J4.z;
-            if (v4 & 8u) sum += (u4 & 8u) ? -J4.w : J4.w;
+            sub_if_bit<0>(lost, un[k], J4.x);
+            sub_if_bit<1>(lost, un[k], J4.y);
+            sub_if_bit<2>(lost, un[k], J4.z);
+            sub_if_bit<3>(lost, un[k], J4.w);
         }
 #pragma unroll
         for (int k = 0; k < 2 * D; ++k) un[k] >>= 4;
-        vv >>= 4;
     }
-    return sum;
+    return lost;
 }
 
 // c2 of accept_site for inverse temperature beta: (float)(-2 beta 2^-fbits log2 e)

@@ -24,7 +24,7 @@ struct McsArgs {
 // A replica occupies RS = 2W + 1 words (colour 0 | colour 1 | pad): the odd stride lets 32 lanes that each own a
 // different replica (lane-per-pair Houdayer) hit 32 different banks.
 struct McsSmem {
-    int RS, oJ, oS, oE, oTos, oSot, oThr, oAcc, oLast, oCum, oU, oSgn, oC2, oScr, words;
+    int RS, oJ, oS, oE, oTos, oSot, oThr, oAcc, oLast, oCum, oU, oSgn, oC2, oPair, oTot, oScr, words;
     // nch: chains held by the CTA (2 = the whole sample, 1 = one chain)
     __host__ __device__ McsSmem(int D, int W, int T, int nwarps, bool lanes, int nch)
     {
@@ -44,6 +44,8 @@ struct McsSmem {
         oU = o;    o += 2 * T;              // PT draws of the current pass, [chain][pair]
         oSgn = o;  o += T;
         oC2 = o;   o += 2 * T;              // fixed-point couplings: bracket slope per replica (float)
+        oPair = o; o += T;                  //   E_A + E_B of the pair at temperature t before the cluster moves
+        oTot = o;  o += 1;                  //   sum of all couplings of the sample
         oScr = o;
         if (nch < 2) {
             // no Houdayer phase, no scratch
@@ -75,6 +77,7 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
     uint32_t *sJ = msm + L.oJ, *sS = msm + L.oS, *sThr = msm + L.oThr, *sAcc = msm + L.oAcc, *sLast = msm + L.oLast;
     uint32_t *sU = msm + L.oU;
     float *sC2 = (float *)(msm + L.oC2);
+    int *sPair = (int *)(msm + L.oPair), *sTot = (int *)(msm + L.oTot);
     int *sE = (int *)(msm + L.oE), *sTos = (int *)(msm + L.oTos), *sSot = (int *)(msm + L.oSot), *sSgn = (int *)(msm + L.oSgn);
     unsigned long long *sCum = (unsigned long long *)(msm + L.oCum);
     const int s = a.split_chains ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
@@ -97,6 +100,15 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
 #pragma unroll
         for (int k = 0; k < 4; ++k) sThr[4 * i + k] = P.d.thrM[4 * t + k];
         if constexpr (GAUSS != 0) sC2[i] = bracket_slope(P.d.betasD[t], P.fbits);
+    }
+    if constexpr (GAUSS != 0) {
+        if (tid == 0) *sTot = 0;
+        __syncthreads();
+        if (a.do_houdayer && NCH == 2) {
+            int part = 0;
+            for (int w = tid; w < W; w += NT) part += bond_sum_word_q(lat, P.d.Jdev + (size_t)s * 2 * (2 * D) * (32 * W), W, w);
+            if (part != 0) atomicAdd(sTot, part);
+        }
     }
     for (int i = tid; i < T; i += NT) {
         sLast[i] = P.d.last[(size_t)s * T + i];
@@ -134,6 +146,10 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
         // ---- a5: Houdayer exchange
         if (a.do_houdayer && NCH == 2) {
             const uint32_t step = a.houd0 + (uint32_t)m;
+            if constexpr (GAUSS != 0) {
+                for (int t = tid; t < T; t += NT) sPair[t] = sE[sSot[t]] + sE[T + sSot[T + t]];
+                __syncthreads();
+            }
             if constexpr (LANES) {
                 // one LANE per temperature: warp k takes temperatures [32k, 32k+32), then strides by the warps in use
                 const int groups = (T + 31) / 32, hw = groups < NWARPS ? groups : NWARPS;
@@ -189,16 +205,20 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
             }
             __syncthreads();
             if constexpr (GAUSS != 0) {
-                // the cluster kernels counted +-1 bonds: recompute every energy from the couplings' values
-                for (int i = tid; i < R; i += NT) sE[i] = 0;
+                // the cluster phase counted +-1 bonds: recompute the energies of chain 0 from the couplings' values
+                // (E = -sum J + 2 sum_unsatisfied J, every bond seen from its black endpoint); the move conserves
+                // E_A + E_B of a pair exactly, which gives chain 1
+                for (int i = tid; i < T; i += NT) sE[i] = -*sTot;
                 __syncthreads();
                 const int32_t *Jb = P.d.Jdev + (size_t)s * 2 * (2 * D) * (32 * W);          // colour-0 block
 #pragma unroll 1
-                for (int item = tid; item < R * W; item += NT) {
+                for (int item = tid; item < T * W; item += NT) {
                     const int q = item / W, w = item - q * W;
-                    const int e = field_sum_word_q(lat, sS + q * RS, sS + q * RS + W, Jb, W, w);
-                    if (e != 0) atomicAdd(sE + q, -e);
+                    const int lost = unsat_sum_word_q(lat, sS + q * RS, sS + q * RS + W, Jb, W, w);
+                    if (lost != 0) atomicAdd(sE + q, -2 * lost);
                 }
+                __syncthreads();
+                for (int t = tid; t < T; t += NT) sE[T + sSot[T + t]] = sPair[t] - sE[sSot[t]];
                 __syncthreads();
             }
         }
