@@ -31,13 +31,6 @@ __device__ __forceinline__ uint32_t thr_double(double x)
 // (the float products add < 2e-7 relative, far inside the 1e-4 bracket; the oracle's double exp is within 1e-16 of Y).
 // Only a draw inside the bracket (probability ~2e-4 of an uphill attempt) or a >= 2^23 pays for the double evaluation,
 // which is the oracle's formula.  Same decision as u < thr_double(x) always.
-__device__ __forceinline__ float ex2_approx(float x)
-{
-    float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-
 // the rare exact evaluation, kept out of line so the 32 unrolled site decisions stay small
 __device__ __noinline__ bool accept_exact(uint32_t u, int a, const double *beta_ptr, int fbits)
 {

@@ -34,6 +34,7 @@ struct DevPtrs {
     int32_t *Jdev;              // [S][2][2D][32 W] per colour and direction
     double *betasD;             // [T]
     double *absdb;              // [T-1] |beta_{t+1} - beta_t|
+    float *swapSlope;           // [T-1] (float)(-|dbeta| 2^-fbits log2 e): slope of the swap test's float bracket
     // round-trip bookkeeping (NEXT-1, R27-R29)
     uint32_t *rtLabel, *rtStart, *rtTrips;      // [S][2][T] per slot
     unsigned long long *rtSum, *rtCnt;          // [S][2][32] per (sample, chain), bin = floor(log2 pass)
@@ -441,6 +442,27 @@ __device__ __forceinline__ uint32_t swap_threshold(const Params &P, int t, uint3
     return (uint32_t)v;
 }
 
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// PT decision for an unfavourable swap with |dE| = absdE at pair t: u < swap_threshold, decided exactly.  +-J: the table.
+// Fixed point: the float bracket of gauss.cuh (accept_site) around Y / 512 = 2^(23 + |dE| slope_t): (float)|dE| and the slope
+// carry 2^-24 relative each of an exponent below 150 in magnitude, the fma rounds once (2^-18), ex2.approx is good to 2^-22
+// -- under 2e-5 relative in all, against a bracket of 1e-4 -- and only a draw inside the bracket pays for the double exp.
+__device__ __forceinline__ bool swap_accept(const Params &P, int t, uint32_t u, uint32_t absdE)
+{
+    if (!P.gauss) return u < thrX_lookup(P, t, absdE >> 2);
+    const float t9 = ex2_approx(fmaf((float)absdE, __ldg(P.d.swapSlope + t), 23.0f));
+    const float uf9 = __uint_as_float(0x4B000000u | (u >> 9)) - 8388608.0f;    // exact: 23 bits fill the mantissa
+    if (uf9 + 2.0f < t9 * 0.9999f) return true;
+    if (uf9 > fmaf(t9, 1.0001f, 1.0f)) return false;
+    return u < swap_threshold(P, t, absdE);
+}
+
 // dynamic smem: per warp [T] energies by temperature + [T] slot_of_temp + [T] draws + [T] signs / accept flags.  GLOBAL_SCRATCH (very long ladders):
 // the same walk on outE / slot_of_temp in global memory.
 template <bool GLOBAL_SCRATCH>
@@ -483,7 +505,7 @@ __global__ void k_exchange(Params P, uint32_t step)
                 if (t + 2 < T) { ebn = Et[t + 2]; rbn = so[t + 2]; }     // positions > t + 1 are not modified before they are read
                 const int32_t dE = ea - eb;
                 bool acc = (long long)SG[t] * dE <= 0;
-                if (!acc) acc = U[t] < swap_threshold(P, t, (uint32_t)(dE < 0 ? -dE : dE));
+                if (!acc) acc = swap_accept(P, t, U[t], (uint32_t)(dE < 0 ? -dE : dE));
                 if (acc) { Et[t] = eb; so[t] = rb; SG[t] = 2; }          // position t is final; (ea, ra) moves up to t+1
                 else     { Et[t] = ea; so[t] = ra; ea = eb; ra = rb; }
                 eb = ebn; rb = rbn;
@@ -506,7 +528,7 @@ __global__ void k_exchange(Params P, uint32_t step)
                 const int32_t eb = Et[t + 1], rb = so[t + 1];
                 const int32_t dE = ea - eb;
                 const int sg = P.d.sgn[t];
-                const bool acc = ((long long)sg * dE <= 0) || (u < swap_threshold(P, t, (uint32_t)(dE < 0 ? -dE : dE)));
+                const bool acc = ((long long)sg * dE <= 0) || swap_accept(P, t, u, (uint32_t)(dE < 0 ? -dE : dE));
                 if (acc) {
                     Et[t] = eb; so[t] = rb;                 // position t is final; (ea, ra) moves up to t+1
                     P.d.accepts[(size_t)chain * (T - 1) + t] += 1ull;

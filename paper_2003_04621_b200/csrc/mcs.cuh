@@ -245,7 +245,11 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                         if (t + 2 < T) { rbn = so[t + 2]; ebn = Ec[rbn]; }     // positions > t are not modified before they are read
                         const int dE = ea - eb;
                         bool acc = sSgn[t] * dE <= 0;
-                        if (!acc) acc = sU[c * T + t] < swap_threshold(P, t, (uint32_t)(dE < 0 ? -dE : dE));
+                        if (!acc) {
+                            const uint32_t adE = (uint32_t)(dE < 0 ? -dE : dE);
+                            if constexpr (GAUSS != 0) acc = swap_accept(P, t, sU[c * T + t], adE);
+                            else acc = sU[c * T + t] < thrX_lookup(P, t, adE >> 2);
+                        }
                         if (acc) { so[t] = rb; sAcc[c * T + t] += 1u; }        // position t is final; (ea, ra) moves up
                         else     { so[t] = ra; ea = eb; ra = rb; }
                         rb = rbn; eb = ebn;

@@ -195,6 +195,7 @@ size_t carve(void *base, int L, int d, int S, int T, uint32_t strideX, DevPtrs *
     p.Jdev = c.take<int32_t>(base, (size_t)S * 2 * 2 * d * 32 * W);
     p.betasD = c.take<double>(base, (size_t)T);
     p.absdb = c.take<double>(base, (size_t)T);
+    p.swapSlope = c.take<float>(base, (size_t)T);
     p.rtLabel = c.take<uint32_t>(base, R);
     p.rtStart = c.take<uint32_t>(base, R);
     p.rtTrips = c.take<uint32_t>(base, R);
@@ -954,6 +955,13 @@ int pt_set_couplings_fixed(const int32_t *Jq, int frac_bits)
     G.P.gauss = 1;
     G.P.fbits = frac_bits;
     G.q_small = 2LL * G.P.D * maxabs < (1LL << 23);
+    {
+        std::vector<float> slope((size_t)G.P.T, 0.0f);
+        for (int t = 0; t + 1 < G.P.T; ++t)
+            slope[t] = (float)(-std::fabs(G.betas[t + 1] - G.betas[t]) * std::ldexp(1.4426950408889634, -frac_bits));
+        CK(cudaMemcpyAsync(G.P.d.swapSlope, slope.data(), slope.size() * 4, cudaMemcpyHostToDevice, G.stream));
+        CK(cudaStreamSynchronize(G.stream));
+    }
     k_pack_jq<<<grid_for((long)G.P.S * 2 * 2 * G.P.D * 32 * G.P.W, 256), 256, 0, G.stream>>>(G.P);
     ++G.launches;
     CK(cudaGetLastError());
