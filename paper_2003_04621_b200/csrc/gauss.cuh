@@ -37,21 +37,22 @@ __device__ __noinline__ bool accept_exact(uint32_t u, int a, const double *beta_
     return u < thr_double(-(*beta_ptr * ldexp((double)(2LL * a), -fbits)));
 }
 
-// Decision for one site, branch-free except for the rare exact evaluation: a <= 0 always flips.
+// Decision for one site, branch-free: returns the sure part of the decision (a <= 0 always flips; an uphill move
+// whose draw is below the bracket flips) and sets `need` when the draw fell inside the bracket (or a >= 2^23) and the exact
+// evaluation (accept_exact) has to decide.  u9 + 2 is formed directly by the magic subtraction (exact below 2^24).
 // SMALL: the host has checked 2 D max|Jq| < 2^23, so every a is below 2^23 and the range test is dropped.
 template <bool SMALL>
-__device__ __forceinline__ bool accept_site(uint32_t u, int a, float c2, const double *beta_ptr, int fbits)
+__device__ __forceinline__ bool accept_site(uint32_t u, int a, float c2, bool &need)
 {
     const float af = __int_as_float(0x4B000000 + a) - 8388608.0f;              // exact for 0 <= a < 2^23 (unused otherwise)
     const float t9 = ex2_approx(fmaf(af, c2, 23.0f));
-    const float uf9 = __uint_as_float(0x4B000000u | (u >> 9)) - 8388608.0f;    // exact: 23 bits fill the mantissa
+    const float uf9p2 = __uint_as_float(0x4B000000u | (u >> 9)) - 8388606.0f;  // u9 + 2, exact: 23 bits fill the mantissa
     const bool up = a > 0;
     const bool small = SMALL || (uint32_t)a < (1u << 23);
-    const bool sure_acc = small && (uf9 + 2.0f < t9 * 0.9999f);
-    const bool sure_rej = small && (uf9 > fmaf(t9, 1.0001f, 1.0f));
-    bool acc = !up || sure_acc;
-    if (up && !sure_acc && !sure_rej) acc = accept_exact(u, a, beta_ptr, fbits);
-    return acc;
+    const bool sure_acc = small && (uf9p2 < t9 * 0.9999f);
+    const bool sure_rej = small && (uf9p2 > fmaf(t9, 1.0001f, 3.0f));
+    need = up && !sure_acc && !sure_rej;
+    return !up || sure_acc;
 }
 
 // s -= J if bit j of un is set: one LOP3 with predicate output + one predicated add
@@ -134,10 +135,11 @@ __global__ void k_energy_q(LAT lat, Params P, int mode)
 
 template <int J> __device__ __forceinline__ int comp(const int4 &v) { return J == 0 ? v.x : J == 1 ? v.y : J == 2 ? v.z : v.w; }
 
-// Site J (0..3) of the current Philox block: un[k] has the block's four sign bits in bits 0..3.
+// Site J (0..3) of the current Philox block: un[k] has the block's four sign bits in bits 0..3.  The sure decisions go
+// into nib / dE at once; a site whose draw fell inside the bracket sets bit J of needmask and is settled by the caller.
 template <class LAT, bool SMALL, int J>
-__device__ __forceinline__ void sweep_site_q(const uint32_t (&un)[2 * LAT::D], const int4 (&Jv)[2 * LAT::D], uint32_t u, uint32_t vv,
-                                             float c2, const double *beta_ptr, int fbits, uint32_t &nib, int &dE)
+__device__ __forceinline__ int sweep_site_q(const uint32_t (&un)[2 * LAT::D], const int4 (&Jv)[2 * LAT::D], uint32_t u, uint32_t vv,
+                                            float c2, uint32_t &nib, int &dE, uint32_t &needmask)
 {
     constexpr int D = LAT::D;
     int tot = 0, lost = 0;                       // a = sum_k J_k - 2 sum_{k: s_i s_k = -1} J_k
@@ -146,9 +148,12 @@ __device__ __forceinline__ void sweep_site_q(const uint32_t (&un)[2 * LAT::D], c
 #pragma unroll
     for (int k = 0; k < 2 * D; ++k) sub_if_bit<J>(lost, un[k], comp<J>(Jv[k]));
     const int a = tot + 2 * lost;
-    bool acc = accept_site<SMALL>(u, a, c2, beta_ptr, fbits);
-    if constexpr (!LAT::kFast) acc = acc && (vv & (1u << J));
+    bool need;
+    bool acc = accept_site<SMALL>(u, a, c2, need);
+    if constexpr (!LAT::kFast) { const bool ok = vv & (1u << J); acc = acc && ok; need = need && ok; }
     if (acc) { nib |= 1u << J; dE += 2 * a; }
+    if (need) needmask |= 1u << J;
+    return a;
 }
 
 // One work item of the fixed-point sweep = one word = 32 same-colour sites of one replica, walked Philox block by Philox
@@ -179,11 +184,17 @@ __device__ __forceinline__ int update_word_q(const LAT &lat, uint32_t *Sown, con
             int4 Jv[2 * D];
 #pragma unroll
             for (int k = 0; k < 2 * D; ++k) Jv[k] = __ldg((const int4 *)(Jp + jdev_index(W, k, B, w)));
-            uint32_t nib = 0;
-            sweep_site_q<LAT, SMALL, 0>(un, Jv, u[0], vv, c2, beta_ptr, fbits, nib, dE);
-            sweep_site_q<LAT, SMALL, 1>(un, Jv, u[1], vv, c2, beta_ptr, fbits, nib, dE);
-            sweep_site_q<LAT, SMALL, 2>(un, Jv, u[2], vv, c2, beta_ptr, fbits, nib, dE);
-            sweep_site_q<LAT, SMALL, 3>(un, Jv, u[3], vv, c2, beta_ptr, fbits, nib, dE);
+            uint32_t nib = 0, needmask = 0;
+            int av[4];
+            av[0] = sweep_site_q<LAT, SMALL, 0>(un, Jv, u[0], vv, c2, nib, dE, needmask);
+            av[1] = sweep_site_q<LAT, SMALL, 1>(un, Jv, u[1], vv, c2, nib, dE, needmask);
+            av[2] = sweep_site_q<LAT, SMALL, 2>(un, Jv, u[2], vv, c2, nib, dE, needmask);
+            av[3] = sweep_site_q<LAT, SMALL, 3>(un, Jv, u[3], vv, c2, nib, dE, needmask);
+            if (needmask) {                      // rare (~1e-3 of the blocks): the oracle's double formula decides
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if (((needmask >> j) & 1u) && accept_exact(u[j], av[j], beta_ptr, fbits)) { nib |= 1u << j; dE += 2 * av[j]; }
+            }
             flip |= nib << (4 * B);
         }
 #pragma unroll
