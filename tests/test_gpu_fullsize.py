@@ -114,3 +114,34 @@ def test_fused_and_separate_launches_agree_at_full_size():
         B.pt_set_fused(-1)
     for k in fused:
         assert np.array_equal(fused[k], sep[k]), k
+
+
+@pytest.mark.parametrize("name,n_mcs,g", [("C2", 10000, 777), ("C3", 10000, 1301), ("C4", 2000, 77), ("C5", 500, 101)])
+def test_full_length_run_one_sample_against_the_oracle(name, n_mcs, g):
+    """The config's whole run of 10^4 MCS (C2, C3; a bounded prefix of it for C4, C5, whose single-core oracle needs
+    minutes per sample) at full S, L, T in bench.py's launch configuration (50 MCS per pt_mcs call, the overlap
+    measurement every k-th MCS where the config asks for it); global sample g is recomputed by the oracle through
+    sample_offset and compared bit for bit at MCS 10, 100, 1000 and at the end, with every overlap record in between."""
+    w = wl.CONFIGS[name]
+    B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED)
+    o = ref.Oracle(w.L, w.d, 1, w.T, w.betas(), wl.SEED, g)
+    chunk = w.measure_every if w.measure_every else 50
+    checkpoints = {10, 100, 1000, n_mcs}
+    done = 0
+    while done < n_mcs:
+        n = min(chunk, n_mcs - done, min(c for c in checkpoints if c > done) - done)
+        B.pt_mcs(n, 1, w.houdayer, True)
+        o.mcs(n, 1, w.houdayer, True)
+        done += n
+        if w.measure_every and done % w.measure_every == 0:
+            Qg, QLg = B.pt_measure_overlap()
+            Qo, QLo = o.measure_overlap()
+            assert np.array_equal(Qo[0], Qg[g]) and np.array_equal(QLo[0], QLg[g]), (name, done)
+        if done in checkpoints:
+            st, a = B.state(), o.state()
+            for k in a:
+                if k != "counters":
+                    assert np.array_equal(a[k][0], st[k][g]), "%s sample %d after %d MCS: %s differs" % (name, g, done, k)
+    assert B.pt_recompute_energy()[1] == 0
+    assert tuple(B.pt_get_counters()) == (n_mcs, n_mcs, n_mcs if w.houdayer else 0)
+    o.close()
