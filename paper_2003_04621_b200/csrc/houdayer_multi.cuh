@@ -33,7 +33,7 @@ __device__ __forceinline__ uint32_t min_neighbour_label(const uint32_t *lab, int
 
 // dynamic smem: Neg[2][W] | Cl[2][W] | red[2 * nwarps + 2] | lab[N]
 template <class LAT>
-__global__ void __launch_bounds__(256) k_houdayer_multi(LAT lat, Params P, uint32_t step)
+__global__ void __launch_bounds__(512) k_houdayer_multi(LAT lat, Params P, uint32_t step)
 {
     extern __shared__ uint32_t hsm[];
     const int W = lat.words();

@@ -356,6 +356,14 @@ cudaError_t launch_houdayer()
 // The cluster kernels compute delta from the +-J bit couplings; with fixed-point couplings the cluster itself is the
 // same (it depends on q only) and the energies are simply recomputed from scratch, which for integers is the same number.
 // multi-cluster variant (R37): one CTA per pair, labels in shared memory
+// CTA size of k_houdayer_multi: ~32 sites per thread, 64..512 threads (measured: C2 best at 64, C5 at 512)
+int multi_threads()
+{
+    int t = 64;
+    while (t < 512 && (long)t * 32 < (long)G.P.N) t <<= 1;
+    return t;
+}
+
 size_t multi_smem_bytes(int threads) { return ((size_t)4 * G.P.W + 2 * (threads / 32) + 2 + (size_t)G.P.N) * 4; }
 
 cudaError_t launch_houdayer_multi()
@@ -364,7 +372,7 @@ cudaError_t launch_houdayer_multi()
     cudaError_t err = cudaSuccess;
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
-        const int threads = 256;
+        const int threads = multi_threads();
         const size_t smem = multi_smem_bytes(threads);
         err = allow_smem(k_houdayer_multi<LAT>, smem);
         if (err != cudaSuccess) return;
@@ -640,7 +648,7 @@ int houdayer_multi_step(void)
 {
     NEED_INIT();
     if (G.n_houdayer == 4294967295u) return fail(PT_ERR_OVERFLOW, "Houdayer counter would overflow");
-    if (multi_smem_bytes(256) > 227 * 1024)
+    if (multi_smem_bytes(multi_threads()) > 227 * 1024)
         return fail(PT_ERR_ARG, "houdayer_multi_step: %d sites of labels do not fit in shared memory", G.P.N);
     CK(launch_houdayer_any(2));
     G.n_houdayer += 1;
@@ -671,7 +679,7 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
     NEED_INIT();
     if (n_mcs < 0 || n_metro < 0) return fail(PT_ERR_ARG, "pt_mcs: n_mcs and n_metro must be >= 0");
     if (do_houdayer < 0 || do_houdayer > 2) return fail(PT_ERR_ARG, "pt_mcs: do_houdayer must be 0, 1 (single-cluster) or 2 (multi-cluster)");
-    if (do_houdayer == 2 && multi_smem_bytes(256) > 227 * 1024)
+    if (do_houdayer == 2 && multi_smem_bytes(multi_threads()) > 227 * 1024)
         return fail(PT_ERR_ARG, "pt_mcs: %d sites of labels do not fit in shared memory (multi-cluster)", G.P.N);
     const uint64_t M = (uint64_t)n_mcs;
     if ((uint64_t)G.n_sweep + M * (uint64_t)n_metro > 4294967295ull ||
