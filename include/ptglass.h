@@ -180,6 +180,8 @@ int pt_set_couplings(const int8_t *J);      /* values must be +1/-1; recomputes 
  * of the run) and recompute E.  From then on local fields, energies (in units of 2^-frac_bits, int32 as before) and energy
  * differences are exact integers and the acceptance probabilities are evaluated per decision in double:
  * flip with a = s_i h_i > 0: u < THR(-(beta_t * ldexp(2a, -frac_bits))); swap: u < THR(-(|dbeta| * ldexp(|dE|, -frac_bits))).
+ * (the kernels settle a decision with a float bracket of 2^32 e^x that is provably on one side of the double threshold and
+ * evaluate the double exp only for a draw inside the bracket: the decision is the double one always).
  * Philox mapping, sweep order, PT pass and cluster move are unchanged; pt_mcs is fused where the +-J path is.
  * PT_ERR_ARG: NULL, frac_bits outside [0, 24], or d*N*max|Jq| >= 2^31.  pt_set_couplings returns to the +-J model. */
 int pt_set_couplings_fixed(const int32_t *Jq, int frac_bits);
