@@ -6,7 +6,7 @@
 A STEP is `--mcs-per-step` Monte Carlo steps (one Metropolis sweep of every replica, one
 Houdayer cluster exchange per equal-temperature pair where the config enables it, one parallel-tempering pass,
 plus the overlap measurement every k-th MCS where the config asks for it) of the whole workload, issued as one
-pt_mcs() call through the C ABI.  At N=1 the workload is BASELINE.json configs[1] (C2: 2D L=32, 1024 samples x
+pt_mcs() / pt_mcs_measure_device() call through the C ABI.  At N=1 the workload is BASELINE.json configs[1] (C2: 2D L=32, 1024 samples x
 32 temperatures x 2 chains, Houdayer + PT every sweep).  With the default K=200, 50 MCS per step the timed region is
 exactly the config's 10^4 MCS.  Inputs are synthetic (seeded +-J samples) and resident in HBM when the
 timed region starts; L2 is flushed between steps (untimed); each step is timed with CUDA events on the library's
@@ -219,20 +219,19 @@ def main():
     if a.gaussian:
         B.pt_set_couplings_fixed(wl.gaussian_couplings_fixed(wl.SEED, w.S, w.d, w.N, 16, sample_offset=rank * w.S), 16)
     flush = torch.empty(512 * 2 ** 20, dtype=torch.uint8, device=dev)
-    Qd = torch.empty((w.S, w.T), dtype=torch.int32, device=dev)
-    QLd = torch.empty((w.S, w.T), dtype=torch.int32, device=dev)
     n_meas = (a.mcs_per_step // w.measure_every) if w.measure_every else 0
     hd = (2 if a.cluster == "multi" else 1) if w.houdayer else 0
     if w.houdayer and a.cluster == "counts":       # index 0 is the lowest beta = the hot end
         B.pt_set_cluster_moves(np.array([1 + (3 * t) // max(w.T - 1, 1) for t in range(w.T)], dtype=np.int32)[::-1].copy())
 
+    Qrec = torch.empty((max(n_meas, 1), w.S, w.T), dtype=torch.int32, device=dev)
+    QLrec = torch.empty_like(Qrec)
+
     def step():
         if n_meas == 0:
             B.pt_mcs(a.mcs_per_step, 1, hd, True)
-        else:
-            for _ in range(n_meas):
-                B.pt_mcs(w.measure_every, 1, hd, True)
-                B.pt_measure_overlap_device(Qd, QLd)
+        else:                                    # the MCS with the overlap records fused in (one launch where eligible)
+            B.pt_mcs_measure_device(a.mcs_per_step, 1, hd, True, w.measure_every, Qrec, QLrec)
 
     def barrier():
         torch.cuda.synchronize()
@@ -307,7 +306,7 @@ def main():
     dom = int(np.argmax(kms))
     if dom not in (0, 4):          # the roofline is quoted for the kernel that does the Metropolis sweeps
         dom = 4 if kn[4] > 0 else 0
-    mcs_per_launch = 1 if dom == 0 else (w.measure_every if n_meas else a.mcs_per_step)
+    mcs_per_launch = 1 if dom == 0 else max(1, (a.mcs_per_step * a.steps) // max(int(kn[4]), 1))
     dom_ms = kms[dom] / max(int(kn[dom]), 1)
     flips_per_launch = w.flips_per_sweep() * mcs_per_launch
     dom_flips_ns = flips_per_launch / (dom_ms * 1e6) if dom_ms > 0 else 0.0

@@ -117,6 +117,15 @@ int houdayer_multi_step(void);
  * Where a sample's whole state fits in shared memory this is ONE kernel launch that keeps each
  * sample resident in one CTA for all n_mcs steps; otherwise it issues the separate kernels in order. */
 int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange);
+/* pt_mcs with the two-replica measurement of Eq. (4) fused in: n_mcs steps as pt_mcs, and after every measure_every-th
+ * step of the call the overlaps Q and (if QL_rec_dev is not NULL) link overlaps QL of all (sample, temperature) pairs are
+ * written to record r = 0, 1, ... of the DEVICE buffers Q_rec_dev / QL_rec_dev, [n_mcs / measure_every][S][T] int32 each,
+ * caller-owned -- exactly what pt_mcs(measure_every, ...) followed by pt_measure_overlap_device(record r) would leave
+ * there (BASELINE config 3: "overlap q and link overlap measured every 10 sweeps").  Where a CTA of the fused kernel
+ * holds both chains of a sample the whole call is ONE launch and the records come from the resident state; otherwise the
+ * library issues those calls.  PT_ERR_ARG: measure_every < 1, Q_rec_dev NULL, negative counts, bad do_houdayer. */
+int pt_mcs_measure_device(int n_mcs, int n_metro, int do_houdayer, int do_exchange, int measure_every, int32_t *Q_rec_dev,
+                          int32_t *QL_rec_dev);
 /* mode -1 (default): pt_mcs uses the fused kernel where eligible; 0: always the separate kernels (tests, profiling).
  * pt_get_fused: 1 if pt_mcs of the bound problem runs fused. */
 int pt_set_fused(int mode);

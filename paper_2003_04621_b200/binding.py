@@ -31,6 +31,7 @@ SYMBOLS = {
     "houdayer_multi_step": (_i, []),
     "pt_set_cluster_moves": (_i, [_vp]),
     "pt_mcs": (_i, [_i, _i, _i, _i]),
+    "pt_mcs_measure_device": (_i, [_i, _i, _i, _i, _i, _vp, _vp]),
     "pt_set_fused": (_i, [_i]),
     "pt_get_fused": (_i, [_vp]),
     "pt_schedule_family": (_i, [C.c_double, C.c_double, _i, C.c_double, _vp, _vp]),
@@ -215,6 +216,12 @@ def pt_set_cluster_moves(n_clu):
 
 def pt_mcs(n_mcs, n_metro=1, do_houdayer=False, do_exchange=True):
     _ck(lib().pt_mcs(n_mcs, n_metro, int(do_houdayer), int(do_exchange)))
+
+
+def pt_mcs_measure_device(n_mcs, n_metro, do_houdayer, do_exchange, measure_every, Q_rec_dev, QL_rec_dev=None):
+    """Q_rec_dev / QL_rec_dev: torch int32 CUDA tensors [n_mcs // measure_every][S][T] (QL optional)."""
+    _ck(lib().pt_mcs_measure_device(n_mcs, n_metro, int(do_houdayer), int(do_exchange), int(measure_every),
+                                    Q_rec_dev.data_ptr(), None if QL_rec_dev is None else QL_rec_dev.data_ptr()))
 
 
 def pt_set_fused(mode):

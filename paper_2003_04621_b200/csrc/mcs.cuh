@@ -18,15 +18,19 @@ struct McsArgs {
     int split_chains;                       // 1: one CTA per (sample, chain) -- only without Houdayer moves (the chains never meet)
     int max_clu;                            // max over t of nclu[t] (R36); 1 in a default run
     uint32_t sweep0, houd0, exch0;          // counter values at the start of the call
+    int measure_every;                      // > 0: overlap record after every measure_every-th MCS of the call (whole-sample CTAs only)
+    int32_t *recQ, *recQL;                  // device records [n_mcs / measure_every][S][T]; recQL may be null
 };
 
 // shared-memory carve-up, shared by host (size) and device (pointers); all offsets in 32-bit words.
 // A replica occupies RS = 2W + 1 words (colour 0 | colour 1 | pad): the odd stride lets 32 lanes that each own a
 // different replica (lane-per-pair Houdayer) hit 32 different banks.
 struct McsSmem {
-    int RS, oJ, oS, oE, oTos, oSot, oThr, oAcc, oLast, oCum, oU, oSgn, oC2, oPair, oTot, oScr, words;
+    int RS, oJ, oS, oE, oTos, oSot, oThr, oAcc, oLast, oCum, oU, oSgn, oC2, oPair, oTot, oMeas, oScr, words;
     // nch: chains held by the CTA (2 = the whole sample, 1 = one chain)
-    __host__ __device__ McsSmem(int D, int W, int T, int nwarps, bool lanes, int nch)
+    // extras: the arrays only the fixed-point (GAUSS) and fused-measurement (MEAS) variants use, placed after the scratch so
+    // that the plain +-J kernel keeps its layout
+    __host__ __device__ McsSmem(int D, int W, int T, int nwarps, bool lanes, int nch, bool extras)
     {
         RS = 2 * W + 1;
         int o = 0;
@@ -43,9 +47,6 @@ struct McsSmem {
         oCum = o;  o += 2 * T;              // 64-bit
         oU = o;    o += 2 * T;              // PT draws of the current pass, [chain][pair]
         oSgn = o;  o += T;
-        oC2 = o;   o += 2 * T;              // fixed-point couplings: bracket slope per replica (float)
-        oPair = o; o += T;                  //   E_A + E_B of the pair at temperature t before the cluster moves
-        oTot = o;  o += 1;                  //   sum of all couplings of the sample
         oScr = o;
         if (nch < 2) {
             // no Houdayer phase, no scratch
@@ -55,15 +56,59 @@ struct McsSmem {
         } else {
             o += nwarps * (4 * W + 64);         // kPairScratchWords
         }
+        oC2 = oPair = oTot = oMeas = o;
+        if (extras) {
+            oC2 = o;   o += 2 * T;          // fixed-point couplings: bracket slope per replica (float)
+            oPair = o; o += T;              //   E_A + E_B of the pair at temperature t before the cluster moves
+            oTot = o;  o += 1;              //   sum of all couplings of the sample
+            oMeas = o; o += 2 * T;          // overlap accumulators of a fused measurement: #(q = -1) | #(bonds with q_i != q_j)
+        }
         words = o;
     }
 };
+
+// a6 inside the fused kernel: overlap record (Eq. (4), link overlap R14) of the pairs now at equal temperature, from
+// the resident state: what pt_measure_overlap would return after this MCS.  gather() is a bit permutation, so the
+// neighbour bits of q = A ^ B are gather(A) ^ gather(B).  Kept out of line: inlined into the MCS loop it cost the sweep
+// loop 9 % on C3 (register allocation), although it runs once per measure_every steps.  Every thread of the CTA calls.
+template <class LAT, int NT>
+__device__ __noinline__ void mcs_overlap_record(LAT lat, const Params &P, const uint32_t *sS, const int *sSot, int *sQ, int s, size_t rec,
+                                                int32_t *recQ, int32_t *recQL)
+{
+    constexpr int D = LAT::D, W = LAT::W, RS = 2 * W + 1;
+    const int T = P.T, tid = threadIdx.x;
+    int *sQL = sQ + T;
+    for (int i = tid; i < 2 * T; i += NT) sQ[i] = 0;
+    __syncthreads();
+#pragma unroll 1
+    for (int item = tid; item < T * W; item += NT) {
+        const int t = item / W, w = item - t * W;
+        const uint32_t *A0 = sS + sSot[t] * RS, *B0 = sS + (T + sSot[T + t]) * RS;
+        const uint32_t nbk = A0[w] ^ B0[w];
+        atomicAdd(sQ + t, __popc(nbk) + __popc(A0[W + w] ^ B0[W + w]));
+        if (recQL) {
+            uint32_t nbA[2 * D], nbB[2 * D];
+            lat.gather(A0 + W, w, 0, nbA);
+            lat.gather(B0 + W, w, 0, nbB);
+            int nd = 0;
+#pragma unroll
+            for (int k = 0; k < 2 * D; ++k) nd += __popc(nbk ^ nbA[k] ^ nbB[k]);
+            atomicAdd(sQL + t, nd);
+        }
+    }
+    __syncthreads();
+    for (int t = tid; t < T; t += NT) {
+        recQ[(rec * P.S + s) * T + t] = P.N - 2 * sQ[t];
+        if (recQL) recQL[(rec * P.S + s) * T + t] = P.D * P.N - 2 * sQL[t];
+    }
+}
 
 // GAUSS: 0 = +-J bit couplings; 1 / 2 = fixed-point couplings (gauss.cuh) with / without the host's range guarantee
 // 2 D max|Jq| < 2^23.  With fixed-point couplings the sweep walks its word site by site (update_word_q), the energies are
 // recomputed from scratch after the cluster moves (field_sum_word_q; the cluster itself depends on q only) and the PT walk
 // evaluates its thresholds in double (swap_threshold).
-template <class LAT, int NT, int MINB, int GAUSS>
+// MEAS: overlap records after every a.measure_every-th MCS from the resident state (pt_mcs_measure_device).
+template <class LAT, int NT, int MINB, int GAUSS, bool MEAS>
 __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
 {
     constexpr int D = LAT::D, W = LAT::W, NWARPS = NT / 32;
@@ -72,7 +117,7 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
     const int T = P.T;
     const int NCH = a.split_chains ? 1 : 2;         // chains in this CTA
     const int R = NCH * T;                          // replicas in this CTA
-    const McsSmem L(D, W, T, NWARPS, LANES, NCH);
+    const McsSmem L(D, W, T, NWARPS, LANES, NCH, GAUSS != 0 || MEAS);
     constexpr int RS = 2 * W + 1;
     uint32_t *sJ = msm + L.oJ, *sS = msm + L.oS, *sThr = msm + L.oThr, *sAcc = msm + L.oAcc, *sLast = msm + L.oLast;
     uint32_t *sU = msm + L.oU;
@@ -270,6 +315,12 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
             }
             __syncthreads();
         }
+        // ---- a6: overlap record (Eq. (4), link overlap R14) of the pairs now at equal temperature, from the resident
+        // state: what pt_measure_overlap would return after this MCS.  gather() is a bit permutation, so the neighbour
+        // bits of q = A ^ B are gather(A) ^ gather(B).
+        if constexpr (MEAS)
+            if (a.measure_every > 0 && NCH == 2 && (m + 1) % a.measure_every == 0)
+                mcs_overlap_record<LAT, NT>(lat, P, sS, sSot, (int *)(msm + L.oMeas), s, (size_t)((m + 1) / a.measure_every - 1), a.recQ, a.recQL);
     }
 
     for (int i = tid; i < R * 2 * W; i += NT) {

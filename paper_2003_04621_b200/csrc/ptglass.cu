@@ -420,10 +420,11 @@ constexpr int kMcsThreads = 128, kMcsMinBlocks = 7;
 // never couple the two chains, R10) and worthwhile when a chain alone still fills the CTA (>= 4 work items per thread).
 bool mcs_split_chains(int do_houdayer) { return !do_houdayer && (long)G.P.T * G.P.W >= 4L * kMcsThreads; }
 
-bool mcs_fused_eligible(size_t *smem_out, int do_houdayer = 1)
+bool mcs_fused_eligible(size_t *smem_out, int do_houdayer = 1, bool measure = false)
 {
     if (!G.fast || G.fused_mode == 0) return false;
-    const McsSmem lay(G.P.D, G.P.W, G.P.T, kMcsThreads / 32, 2 * G.P.W <= 32, mcs_split_chains(do_houdayer) ? 1 : 2);
+    const McsSmem lay(G.P.D, G.P.W, G.P.T, kMcsThreads / 32, 2 * G.P.W <= 32, mcs_split_chains(do_houdayer) ? 1 : 2,
+                      G.P.gauss || measure);
     const size_t smem = (size_t)lay.words * 4;
     if (smem_out) *smem_out = smem;
     return (smem + 1024) * 4 <= 227 * 1024;
@@ -437,9 +438,11 @@ cudaError_t launch_mcs(const McsArgs &a)
         using LAT = decltype(lat);
         if constexpr (LAT::kFast) {
             size_t smem = 0;
-            mcs_fused_eligible(&smem, a.do_houdayer);
-            auto kern = !G.P.gauss ? k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 0>
-                        : G.q_small ? k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 1> : k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 2>;
+            const bool meas = a.measure_every > 0;
+            mcs_fused_eligible(&smem, a.do_houdayer, meas);
+            // the fused measurement is instantiated for the +-J model only (pt_mcs_measure_device falls back otherwise)
+            auto kern = !G.P.gauss ? (meas ? k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 0, true> : k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 0, false>)
+                        : G.q_small ? k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 1, false> : k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 2, false>;
             err = allow_smem(kern, smem);
             if (err != cudaSuccess) return;
             const unsigned grid = (unsigned)G.P.S * (a.split_chains ? 2u : 1u);
@@ -689,7 +692,7 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
     if (n_mcs == 0 || (n_metro == 0 && !do_houdayer && !do_exchange)) return PT_OK;
     if (do_houdayer != 2 && mcs_fused_eligible(nullptr, do_houdayer)) {
         const McsArgs a{n_mcs, n_metro, do_houdayer ? 1 : 0, do_exchange ? 1 : 0, mcs_split_chains(do_houdayer) ? 1 : 0,
-                        G.max_clu, G.n_sweep, G.n_houdayer, G.n_exchange};
+                        G.max_clu, G.n_sweep, G.n_houdayer, G.n_exchange, 0, nullptr, nullptr};
         CK(launch_mcs(a));
         G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
         if (do_houdayer) G.n_houdayer += (uint32_t)M;
@@ -702,6 +705,42 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
         if (do_exchange) { CK(launch_exchange()); G.n_exchange += 1; }
     }
     return PT_OK;
+}
+
+int pt_mcs_measure_device(int n_mcs, int n_metro, int do_houdayer, int do_exchange, int measure_every, int32_t *Q_rec_dev,
+                          int32_t *QL_rec_dev)
+{
+    NEED_INIT();
+    if (measure_every < 1) return fail(PT_ERR_ARG, "pt_mcs_measure_device: measure_every must be >= 1");
+    if (!Q_rec_dev) return fail(PT_ERR_ARG, "pt_mcs_measure_device: Q_rec_dev is NULL");
+    if (n_mcs < 0 || n_metro < 0) return fail(PT_ERR_ARG, "pt_mcs_measure_device: n_mcs and n_metro must be >= 0");
+    const size_t stride = (size_t)G.P.S * G.P.T;
+    // ONE launch for the whole call where a CTA holds both chains of a sample: the records come from the resident state
+    if (!G.P.gauss && n_mcs >= measure_every && (do_houdayer == 0 || do_houdayer == 1) && mcs_fused_eligible(nullptr, do_houdayer, true) &&
+        !mcs_split_chains(do_houdayer) && (n_metro > 0 || do_houdayer || do_exchange)) {
+        const uint64_t M = (uint64_t)n_mcs;
+        if ((uint64_t)G.n_sweep + M * (uint64_t)n_metro > 4294967295ull ||
+            (do_exchange && (uint64_t)G.n_exchange + M > 4294967295ull) ||
+            (do_houdayer && (uint64_t)G.n_houdayer + M > 4294967295ull))
+            return fail(PT_ERR_OVERFLOW, "a step counter would overflow");
+        const McsArgs a{n_mcs, n_metro, do_houdayer ? 1 : 0, do_exchange ? 1 : 0, 0, G.max_clu, G.n_sweep, G.n_houdayer,
+                        G.n_exchange, measure_every, Q_rec_dev, QL_rec_dev};
+        CK(launch_mcs(a));
+        G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
+        if (do_houdayer) G.n_houdayer += (uint32_t)M;
+        if (do_exchange) G.n_exchange += (uint32_t)M;
+        return PT_OK;
+    }
+    // otherwise exactly the calls it stands for
+    int done = 0, rec = 0;
+    while (n_mcs - done >= measure_every) {
+        int rc = pt_mcs(measure_every, n_metro, do_houdayer, do_exchange);
+        if (rc) return rc;
+        CK(launch_measure(Q_rec_dev + rec * stride, QL_rec_dev ? QL_rec_dev + rec * stride : nullptr));
+        done += measure_every;
+        ++rec;
+    }
+    return pt_mcs(n_mcs - done, n_metro, do_houdayer, do_exchange);
 }
 
 int pt_set_fused(int mode)

@@ -27,9 +27,13 @@ def run_like_bench(w, n_mcs):
     """The step of bench.py: pt_mcs in one call (or in chunks of measure_every with the measurement between)."""
     recs = []
     if w.measure_every:
-        for _ in range(n_mcs // w.measure_every):
-            B.pt_mcs(w.measure_every, 1, w.houdayer, True)
-            recs.append(B.pt_measure_overlap())
+        import torch
+        n_rec = n_mcs // w.measure_every
+        Qr = torch.empty((n_rec, w.S, w.T), dtype=torch.int32, device="cuda")
+        QLr = torch.empty_like(Qr)
+        B.pt_mcs_measure_device(n_mcs, 1, w.houdayer, True, w.measure_every, Qr, QLr)
+        Qh, QLh = Qr.cpu().numpy(), QLr.cpu().numpy()
+        recs = [(Qh[r], QLh[r]) for r in range(n_rec)]
     else:
         B.pt_mcs(n_mcs, 1, w.houdayer, True)
     return recs

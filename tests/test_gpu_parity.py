@@ -207,3 +207,35 @@ def test_single_temperature_and_counters():
     with pytest.raises(B.PTError) as e:
         B.pt_sweep(-1)
     assert e.value.code == B.PT_ERR_ARG
+
+
+@pytest.mark.parametrize("L,d,S,T,houd,general,n_mcs,every", [
+    (8, 3, 5, 6, False, False, 30, 10),        # C3-like: one fused launch, records from the resident state
+    (32, 2, 3, 8, True, False, 12, 1),         # a record after every MCS, with the cluster move
+    (16, 2, 2, 40, True, False, 25, 10),       # n_mcs not a multiple: two records, five more MCS
+    (16, 3, 2, 40, False, False, 20, 5),       # T*W >= 512 without cluster moves: chain-split CTAs -> the separate calls
+    (6, 2, 2, 4, True, True, 9, 3),            # general-L path -> the separate calls
+    (64, 2, 1, 3, True, False, 6, 2)])
+def test_mcs_with_fused_overlap_records(L, d, S, T, houd, general, n_mcs, every):
+    import torch
+
+    betas = wl.betas_geometric(0.3, 1.6, T)
+    o = open_both(L, d, S, T, betas, offset=3, general=general)
+    n_rec = n_mcs // every
+    Qr = torch.full((max(n_rec, 1), S, T), -12345, dtype=torch.int32, device="cuda")
+    QLr = torch.full_like(Qr, -12345)
+    B.pt_mcs_measure_device(n_mcs, 1, houd, True, every, Qr, QLr)
+    Qh, QLh = Qr.cpu().numpy(), QLr.cpu().numpy()
+    for r in range(n_rec):
+        o.mcs(every, 1, houd, True)
+        Qo, QLo = o.measure_overlap()
+        assert np.array_equal(Qo, Qh[r]) and np.array_equal(QLo, QLh[r]), r
+    o.mcs(n_mcs - n_rec * every, 1, houd, True)
+    assert_same_state(o, "after the call")
+    # Q only
+    B.pt_mcs_measure_device(every, 1, houd, True, every, Qr, None)
+    o.mcs(every, 1, houd, True)
+    assert np.array_equal(o.measure_overlap()[0], Qr.cpu().numpy()[0])
+    assert_same_state(o, "Q only")
+    with pytest.raises(B.PTError):
+        B.pt_mcs_measure_device(4, 1, houd, True, 0, Qr, QLr)
