@@ -338,6 +338,22 @@ def main():
     roofline["sweep_only"] = {"kernel": "k_sweep", "flips_per_ns": so, "frac": A * so / peak_ops,
                               "what": "pt_sweep(%d) launches, no Houdayer / exchange" % a.mcs_per_step}
     assert B.pt_recompute_energy()[1] == 0
+    # the two measurement kernels alone (a6 and the NEXT-2 overlap profile), CUDA events around 20 calls each
+    prof_d = torch.empty((w.S, w.T, w.d, w.L), dtype=torch.int32, device=dev)
+    meas_us = {}
+    for label, fn in (("overlap", lambda: B.pt_measure_overlap_device(Qrec[0], QLrec[0])),
+                      ("overlap_profile", lambda: B.pt_measure_overlap_profile_device(prof_d))):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        m0.record()
+        for _ in range(20):
+            fn()
+        m1.record()
+        torch.cuda.synchronize()
+        meas_us[label] = m0.elapsed_time(m1) / 20 * 1e3
+    roofline["measurement_us_per_call"] = meas_us
 
     cpu = None
     if not a.no_cpu_baseline:
