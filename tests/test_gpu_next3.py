@@ -119,3 +119,36 @@ def test_gaussian_C2_shape_sampled_samples():
         for k in a:
             if k != "counters":
                 assert np.array_equal(a[k][0], st[k][g]), (g, k)
+
+
+@pytest.mark.parametrize("L,d,S,T,general", [(32, 2, 2, 6, False), (8, 3, 2, 5, False), (64, 2, 1, 3, False), (6, 2, 2, 4, True)])
+def test_gaussian_with_cluster_variants_and_records(L, d, S, T, general):
+    """Fixed-point couplings together with the NEXT-4 variants (move counts in the fused kernel, multi-cluster step) and
+    with pt_mcs_measure_device (which issues the separate calls in this model)."""
+    import torch
+
+    betas = wl.betas_geometric(0.2, 1.4, T)
+    fbits = 12 if L >= 64 else 16                      # d N max|Jq| must stay below 2^31
+    Jq = wl.gaussian_couplings_fixed(wl.SEED, S, d, L ** d, fbits, sample_offset=4)
+    o = ref.Oracle(L, d, S, T, betas, wl.SEED, 4)
+    o.set_couplings_fixed(Jq, fbits)
+    B.pt_open(L, d, S, T, betas, wl.SEED, 4, general=general)
+    B.pt_set_couplings_fixed(Jq, fbits)
+    n_clu = np.array([(3 * t) % 4 for t in range(T)], dtype=np.int32)
+    o.set_cluster_moves(n_clu); B.pt_set_cluster_moves(n_clu)
+    o.mcs(6, 1, 1, True); B.pt_mcs(6, 1, 1, True)
+    same_state(o, "move counts")
+    o.set_cluster_moves(None); B.pt_set_cluster_moves(None)
+    o.houdayer_multi_step(); B.houdayer_multi_step()
+    same_state(o, "multi-cluster step")
+    o.mcs(4, 1, 2, True); B.pt_mcs(4, 1, 2, True)
+    same_state(o, "mcs with the multi-cluster step")
+    Qr = torch.empty((2, S, T), dtype=torch.int32, device="cuda")
+    QLr = torch.empty_like(Qr)
+    B.pt_mcs_measure_device(7, 1, 1, True, 3, Qr, QLr)
+    for r in range(2):
+        o.mcs(3, 1, 1, True)
+        Qo, QLo = o.measure_overlap()
+        assert np.array_equal(Qo, Qr.cpu().numpy()[r]) and np.array_equal(QLo, QLr.cpu().numpy()[r])
+    o.mcs(1, 1, 1, True)
+    same_state(o, "records")
