@@ -239,3 +239,25 @@ def test_mcs_with_fused_overlap_records(L, d, S, T, houd, general, n_mcs, every)
     assert_same_state(o, "Q only")
     with pytest.raises(B.PTError):
         B.pt_mcs_measure_device(4, 1, houd, True, 0, Qr, QLr)
+
+
+def test_very_long_ladder_walks_on_global_scratch():
+    """T > 4096: the PT walk of k_exchange no longer fits its shared-memory scratch and runs on global memory
+    (k_exchange<GLOBAL_SCRATCH>); a sample no longer fits the fused kernel either, so pt_mcs issues the separate kernels."""
+    L, d, S, T = 8, 2, 2, 4200
+    betas = wl.betas_linear(0.1, 2.0, T)
+    o = ref.Oracle(L, d, S, T, betas, SEED, 7)
+    B.pt_open(L, d, S, T, betas, SEED, 7, track_round_trips=True)
+    assert B.pt_get_fused() == 0
+    assert_same_state(o, "init")
+    for step in range(3):
+        o.sweep(1); B.pt_sweep(1)
+        o.houdayer_step(); B.houdayer_step()
+        o.exchange(); B.pt_exchange()
+        assert_same_state(o, "step %d" % step)
+    o.mcs(3, 1, True, True); B.pt_mcs(3, 1, True, True)
+    assert_same_state(o, "mcs")
+    for a, b in zip(o.get_round_trips(), B.pt_get_round_trips()):
+        assert np.array_equal(a, b)
+    att, acc = B.pt_get_swap_counts()
+    assert (att == 6).all() and acc.sum() > 0
