@@ -183,6 +183,15 @@ int pt_get_thresholds(uint32_t *thrM /* [T][d], k=1..d at [t][k-1]; may be NULL 
                       uint32_t *thrX /* [T-1][thrX_stride], entry m = |dE|/4; may be NULL */, size_t thrX_stride);
 int pt_get_counters(uint32_t *n_sweep, uint32_t *n_exchange, uint32_t *n_houdayer);
 int pt_set_spins(const int8_t *spins);      /* values must be +1/-1 (PT_ERR_ARG otherwise); recomputes E */
+/* Checkpoint / resume.  The RNG is counter-based, so the complete state of a run is: the couplings (or the
+ * seed), the spins, the slot_of_temp maps and the three step counters; energies follow from the spins.  A run resumed with
+ * pt_init (same arguments) + pt_set_spins + pt_set_perm + pt_set_counters continues bit-identically (the observables that
+ * count since init -- swap counts, cumulative cluster sizes, round trips -- restart from zero).
+ * pt_set_perm: HOST [S][2][T]; every row must be a permutation of 0..T-1 (PT_ERR_ARG otherwise); temp_of_slot is its
+ * inverse.  pt_set_counters also lets a caller place a run anywhere in the Philox streams; a later call that would pass
+ * 2^32 - 1 returns PT_ERR_OVERFLOW and leaves the state unchanged. */
+int pt_set_perm(const int32_t *slot_of_temp);
+int pt_set_counters(uint32_t n_sweep, uint32_t n_exchange, uint32_t n_houdayer);
 int pt_set_couplings(const int8_t *J);      /* values must be +1/-1; recomputes E */
 /* NEXT-3 (R33-R35): replace the couplings by fixed-point numbers J = Jq * 2^-frac_bits
  * (HOST int32 [S][d][N], Jq[mu][i] = bond i -> i+e_mu; e.g. a rounded standard-normal sample -- the couplings are an input

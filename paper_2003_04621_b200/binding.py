@@ -31,6 +31,8 @@ SYMBOLS = {
     "houdayer_multi_step": (_i, []),
     "pt_set_cluster_moves": (_i, [_vp]),
     "pt_mcs": (_i, [_i, _i, _i, _i]),
+    "pt_set_perm": (_i, [_vp]),
+    "pt_set_counters": (_i, [C.c_uint32, C.c_uint32, C.c_uint32]),
     "pt_mcs_measure_device": (_i, [_i, _i, _i, _i, _i, _vp, _vp]),
     "pt_set_fused": (_i, [_i]),
     "pt_get_fused": (_i, [_vp]),
@@ -222,6 +224,17 @@ def pt_mcs_measure_device(n_mcs, n_metro, do_houdayer, do_exchange, measure_ever
     """Q_rec_dev / QL_rec_dev: torch int32 CUDA tensors [n_mcs // measure_every][S][T] (QL optional)."""
     _ck(lib().pt_mcs_measure_device(n_mcs, n_metro, int(do_houdayer), int(do_exchange), int(measure_every),
                                     Q_rec_dev.data_ptr(), None if QL_rec_dev is None else QL_rec_dev.data_ptr()))
+
+
+def pt_set_perm(slot_of_temp):
+    a = np.ascontiguousarray(slot_of_temp, dtype=np.int32)
+    if a.shape != (_shape["S"], 2, _shape["T"]):
+        raise PTError(PT_ERR_ARG, "slot_of_temp must have shape [S][2][T]")
+    _ck(lib().pt_set_perm(_p(a)))
+
+
+def pt_set_counters(n_sweep, n_exchange, n_houdayer):
+    _ck(lib().pt_set_counters(int(n_sweep), int(n_exchange), int(n_houdayer)))
 
 
 def pt_set_fused(mode):

@@ -946,6 +946,38 @@ int pt_get_counters(uint32_t *n_sweep, uint32_t *n_exchange, uint32_t *n_houdaye
     return PT_OK;
 }
 
+// ---- checkpoint / resume: the RNG is counter-based, so the complete state of a run is the spins, the
+// couplings (or the seed), the slot_of_temp maps and the three step counters; energies follow from the spins.
+
+int pt_set_counters(uint32_t n_sweep, uint32_t n_exchange, uint32_t n_houdayer)
+{
+    NEED_INIT();
+    G.n_sweep = n_sweep;
+    G.n_exchange = n_exchange;
+    G.n_houdayer = n_houdayer;
+    return PT_OK;
+}
+
+int pt_set_perm(const int32_t *slot_of_temp)
+{
+    NEED_INIT();
+    if (!slot_of_temp) return fail(PT_ERR_ARG, "slot_of_temp is NULL");
+    const int T = G.P.T;
+    const size_t chains = (size_t)G.P.S * 2, n = chains * T;
+    std::vector<int32_t> tos(n, -1);
+    for (size_t c = 0; c < chains; ++c)
+        for (int t = 0; t < T; ++t) {
+            const int32_t r = slot_of_temp[c * T + t];
+            if (r < 0 || r >= T || tos[c * T + r] != -1)
+                return fail(PT_ERR_ARG, "pt_set_perm: row %zu of slot_of_temp is not a permutation of 0..%d", c, T - 1);
+            tos[c * T + r] = t;
+        }
+    CK(cudaMemcpyAsync(G.P.d.sot, slot_of_temp, n * 4, cudaMemcpyHostToDevice, G.stream));
+    CK(cudaMemcpyAsync(G.P.d.tos, tos.data(), n * 4, cudaMemcpyHostToDevice, G.stream));
+    CK(cudaStreamSynchronize(G.stream));
+    return PT_OK;
+}
+
 // +-1 validation of the staged int8 input, on the device (k_check_pm1 counts offenders into mismatch[1])
 static int check_pm1_staged(size_t n, const char *what)
 {

@@ -261,3 +261,49 @@ def test_very_long_ladder_walks_on_global_scratch():
         assert np.array_equal(a, b)
     att, acc = B.pt_get_swap_counts()
     assert (att == 6).all() and acc.sum() > 0
+
+
+@pytest.mark.parametrize("L,d,S,T,general", [(32, 2, 3, 8, False), (8, 3, 2, 6, False), (128, 2, 1, 3, False), (6, 2, 2, 4, True)])
+def test_checkpoint_and_resume_continue_bit_identically(L, d, S, T, general):
+    """spins + slot_of_temp + the three counters (and the seed) are the complete state (counter-based RNG): a run that is
+    re-initialised and restored from them continues exactly like the uninterrupted run and like the oracle."""
+    betas = wl.betas_geometric(0.3, 1.6, T)
+    o = open_both(L, d, S, T, betas, offset=9, general=general)
+    o.mcs(7, 1, True, True); B.pt_mcs(7, 1, True, True)
+    o.sweep(2); B.pt_sweep(2)                                   # counters no longer equal to one another
+    spins, (tos, sot), counters = B.pt_get_spins(), B.pt_get_perm(), B.pt_get_counters()
+    B.pt_open(L, d, S, T, betas, SEED, 9, general=general)      # a fresh context: same couplings from the seed
+    B.pt_set_spins(spins)
+    B.pt_set_perm(sot)
+    B.pt_set_counters(*counters)
+    assert np.array_equal(B.pt_get_perm()[0], tos)
+    o.mcs(9, 1, True, True); B.pt_mcs(9, 1, True, True)
+    a, b = o.state(), B.state()
+    for k in ("spins", "energy", "temp_of_slot", "slot_of_temp", "last_size", "counters"):
+        assert np.array_equal(a[k], b[k]), k
+    assert B.pt_recompute_energy()[1] == 0
+    with pytest.raises(B.PTError) as e:                         # not a permutation
+        bad = sot.copy(); bad[0, 0, 0] = bad[0, 0, 1]
+        B.pt_set_perm(bad)
+    assert e.value.code == B.PT_ERR_ARG
+
+
+def test_counter_overflow_is_refused_and_leaves_the_state_alone():
+    L, d, S, T = 8, 2, 2, 4
+    betas = wl.betas_geometric(0.3, 1.6, T)
+    o = open_both(L, d, S, T, betas)
+    top = 2 ** 32 - 1
+    B.pt_set_counters(top - 2, top - 1, top - 1)
+    B.pt_mcs(1, 2, True, True)                                  # reaches (top, top, top) exactly: allowed
+    assert tuple(B.pt_get_counters()) == (top, top, top)
+    st0 = B.state()
+    for fn in (lambda: B.pt_sweep(1), B.pt_exchange, B.houdayer_step, B.houdayer_multi_step,
+               lambda: B.pt_mcs(1, 1, True, True), lambda: B.pt_mcs(1, 0, False, True), lambda: B.pt_mcs(1, 0, 2, False)):
+        with pytest.raises(B.PTError) as e:
+            fn()
+        assert e.value.code == B.PT_ERR_OVERFLOW
+    st1 = B.state()
+    for k in st0:
+        assert np.array_equal(st0[k], st1[k]), k
+    B.pt_mcs(0, 1, True, True)                                  # nothing to do: fine
+    o.close()
