@@ -106,8 +106,8 @@ int houdayer_step(void);
  * probability 1/2: the component whose smallest site index is i_min is exchanged iff the top bit of word (i_min & 3) of
  * the Philox block ctr = (i_min >> 2, step, g, tag(5, aux 1, 0, t)) is set.  E1 + E2 is conserved for any such union
  * (P:138).  last / cumulative count exchanged sites; the Houdayer step counter advances by one.  Components are found by
- * label propagation in shared memory, one CTA per (sample, temperature): PT_ERR_ARG if 4 N bytes of labels do not fit
- * (N <= ~56000 sites).  In pt_mcs it is do_houdayer = 2 (separate kernels, not fused). */
+ * label propagation in shared memory, one CTA per (sample, temperature): PT_ERR_ARG if 6 N bytes of labels and site list do not
+ * fit (N <= ~36000 sites: up to 2D L = 128, 3D L = 32).  In pt_mcs it is do_houdayer = 2 (separate kernels, not fused). */
 int pt_set_cluster_moves(const int32_t *n_clu);
 int houdayer_multi_step(void);
 

@@ -31,7 +31,7 @@ __device__ __forceinline__ uint32_t min_neighbour_label(const uint32_t *lab, int
     }
 }
 
-// dynamic smem: Neg[2][W] | Cl[2][W] | red[2 * nwarps + 2] | lab[N]
+// dynamic smem: Neg[2][W] | Cl[2][W] | red[2 * nwarps + 2] | lab[N] | act[N] (uint16: list of the q = -1 sites, N <= 65536)
 template <class LAT>
 __global__ void __launch_bounds__(512) k_houdayer_multi(LAT lat, Params P, uint32_t step)
 {
@@ -41,6 +41,8 @@ __global__ void __launch_bounds__(512) k_houdayer_multi(LAT lat, Params P, uint3
     uint32_t *Neg = hsm, *Cl = hsm + 2 * W;
     int *red = (int *)(Cl + 2 * W);
     uint32_t *lab = (uint32_t *)(red + 2 * nwarps + 2);
+    uint16_t *act = (uint16_t *)(lab + P.N);
+    int *n_act_s = red + 2 * nwarps;                 // red[2 nwarps]: number of q = -1 sites (red[0 .. 2 nwarps) is used by the tail only)
     const int t = blockIdx.x, s = blockIdx.y, tid = threadIdx.x;
     const int L = P.L, D = P.D, N = P.N;
     const size_t repA = rep_index(P, s, 0, P.d.sot[rep_index(P, s, 0, t)]);
@@ -55,25 +57,40 @@ __global__ void __launch_bounds__(512) k_houdayer_multi(LAT lat, Params P, uint3
         Cl[w] = 0; Cl[W + w] = 0;
     }
     __syncthreads();
-    for (int i = tid; i < N; i += blockDim.x) {
-        const int p = nat_colour<LAT>(i, L, D), h = i >> 1;
-        lab[i] = ((Neg[p * W + (h >> 5)] >> (h & 31)) & 1u) ? (uint32_t)i : kNoLabel;
+    if (tid == 0) *n_act_s = 0;
+    __syncthreads();
+    // labels, and the compact list of the q = -1 sites (any order) that every later loop walks: about half of the sites
+    // have q = +1 and would only idle their lanes.  Warp-aggregated append: one atomicAdd per 32 sites.
+    for (int i0 = (tid & ~31); i0 < N; i0 += blockDim.x) {
+        const int i = i0 + (tid & 31);
+        bool on = false;
+        if (i < N) {
+            const int p = nat_colour<LAT>(i, L, D), h = i >> 1;
+            on = (Neg[p * W + (h >> 5)] >> (h & 31)) & 1u;
+            lab[i] = on ? (uint32_t)i : kNoLabel;
+        }
+        const unsigned m = __ballot_sync(0xFFFFFFFFu, on);
+        int base = 0;
+        if ((tid & 31) == 0 && m) base = atomicAdd(n_act_s, __popc(m));
+        base = __shfl_sync(0xFFFFFFFFu, base, 0);
+        if (on) act[base + __popc(m & ((1u << (tid & 31)) - 1u))] = (uint16_t)i;
     }
     __syncthreads();
+    const int n_act = *n_act_s;
 
     // label equivalence to the fixed point
     for (;;) {
         int changed = 0;
-        for (int i = tid; i < N; i += blockDim.x) {                      // scan: merge trees at their roots
+        for (int k = tid; k < n_act; k += blockDim.x) {                  // scan: merge trees at their roots
+            const int i = act[k];
             const uint32_t l = lab[i];
-            if (l == kNoLabel) continue;
             const uint32_t m = min_neighbour_label<LAT, 0>(lab, i, L, D, l);
             if (m < l) { atomicMin(lab + l, m); changed = 1; }
         }
         if (!__syncthreads_or(changed)) break;
-        for (int i = tid; i < N; i += blockDim.x) {                      // flatten: every site points at its root
+        for (int k = tid; k < n_act; k += blockDim.x) {                  // flatten: every site points at its root
+            const int i = act[k];
             uint32_t l = lab[i];
-            if (l == kNoLabel) continue;
             for (uint32_t up = lab[l]; up != l; up = lab[l]) l = up;
             lab[i] = l;
         }
@@ -81,7 +98,8 @@ __global__ void __launch_bounds__(512) k_houdayer_multi(LAT lat, Params P, uint3
     }
 
     // one coin per component, thrown by its root (the site that is its own label)
-    for (int i = tid; i < N; i += blockDim.x) {
+    for (int k = tid; k < n_act; k += blockDim.x) {
+        const int i = act[k];
         if (lab[i] != (uint32_t)i) continue;
         uint32_t w4[4];
         philox4x32_10((uint32_t)(i >> 2), step, P.g0 + (uint32_t)s, make_tag(DOM_HOUD, 1, 0, t), P.rk, w4[0], w4[1], w4[2], w4[3]);

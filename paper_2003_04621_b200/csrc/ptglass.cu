@@ -364,7 +364,7 @@ int multi_threads()
     return t;
 }
 
-size_t multi_smem_bytes(int threads) { return ((size_t)4 * G.P.W + 2 * (threads / 32) + 2 + (size_t)G.P.N) * 4; }
+size_t multi_smem_bytes(int threads) { return ((size_t)4 * G.P.W + 2 * (threads / 32) + 2 + (size_t)G.P.N) * 4 + (size_t)G.P.N * 2 + 16; }
 
 cudaError_t launch_houdayer_multi()
 {
