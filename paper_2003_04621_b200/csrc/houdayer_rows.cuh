@@ -58,6 +58,13 @@ __device__ __forceinline__ bool row_close(const uint32_t (&neg)[WR], const uint3
     return diff != 0;
 }
 
+__device__ __forceinline__ void cswap(uint32_t &a, uint32_t &b, bool c)
+{
+    const uint32_t t = c ? a : b;
+    a = c ? b : a;
+    b = t;
+}
+
 // Same contract as houdayer_pair (houdayer.cuh); scratch: 2W words of the warp's shared memory.
 template <class LAT>
 __device__ __forceinline__ int houdayer_pair_rows(const LAT &lat, uint32_t *A0, uint32_t *A1, uint32_t *B0, uint32_t *B1,
@@ -111,24 +118,49 @@ __device__ __forceinline__ int houdayer_pair_rows(const LAT &lat, uint32_t *A0, 
         rem -= c;
     }
 
-    // grow to the fixed point
-    const int lane_up = (lane - 1) & (LANES - 1), lane_dn = (lane + 1) & (LANES - 1);
-    for (;;) {
-        uint32_t upB[WR], dnB[WR];
+    // grow to the fixed point.  ODD lanes keep their strip in REVERSE row order, so the same index sweep 0 -> RPL-1 runs
+    // down the lattice on even lanes and up on odd lanes: with the boundary rows exchanged before each of the two sweeps of
+    // a round, membership crosses TWO strips per round in either direction (even: down then up, odd: up then down) instead
+    // of one.  The row beyond index 0 is the neighbour lane's index-0 row, the row beyond index RPL-1 its index-(RPL-1) row
+    // (row_close is symmetric in its two vertical neighbours).  Any order of monotone row closures reaches the same least
+    // fixed point; a round that changes nothing has evaluated every row against final values.
+    const bool odd = lane & 1;
+#pragma unroll
+    for (int r = 0; r < RPL / 2; ++r)
 #pragma unroll
         for (int j = 0; j < WR; ++j) {
-            upB[j] = __shfl_sync(FULL, cl[RPL - 1][j], lane_up);        // last row of the strip above (periodic)
-            dnB[j] = __shfl_sync(FULL, cl[0][j], lane_dn);              // first row of the strip below
+            cswap(neg[r][j], neg[RPL - 1 - r][j], odd);
+            cswap(rneg[r][j], rneg[RPL - 1 - r][j], odd);
+            cswap(cl[r][j], cl[RPL - 1 - r][j], odd);
+        }
+    const int lane_up = (lane - 1) & (LANES - 1), lane_dn = (lane + 1) & (LANES - 1);
+    const int src0 = odd ? lane_dn : lane_up;          // holds the row beyond my index 0
+    const int srcL = odd ? lane_up : lane_dn;          // holds the row beyond my index RPL-1
+    for (;;) {
+        uint32_t b0[WR], bL[WR];
+#pragma unroll
+        for (int j = 0; j < WR; ++j) {
+            b0[j] = __shfl_sync(FULL, cl[0][j], src0);
+            bL[j] = __shfl_sync(FULL, cl[RPL - 1][j], srcL);
         }
         bool changed = false;
 #pragma unroll
         for (int r = 0; r < RPL; ++r)
-            changed |= row_close<WR>(neg[r], rneg[r], cl[r], r > 0 ? cl[r - 1] : upB, r < RPL - 1 ? cl[r + 1] : dnB);
+            changed |= row_close<WR>(neg[r], rneg[r], cl[r], r > 0 ? cl[r - 1] : b0, r < RPL - 1 ? cl[r + 1] : bL);
 #pragma unroll
-        for (int r = RPL - 2; r >= 0; --r)
-            changed |= row_close<WR>(neg[r], rneg[r], cl[r], r > 0 ? cl[r - 1] : upB, r < RPL - 1 ? cl[r + 1] : dnB);
+        for (int j = 0; j < WR; ++j) {
+            b0[j] = __shfl_sync(FULL, cl[0][j], src0);
+            bL[j] = __shfl_sync(FULL, cl[RPL - 1][j], srcL);
+        }
+#pragma unroll
+        for (int r = RPL - 1; r >= 0; --r)
+            changed |= row_close<WR>(neg[r], rneg[r], cl[r], r > 0 ? cl[r - 1] : b0, r < RPL - 1 ? cl[r + 1] : bL);
         if (!__any_sync(FULL, changed)) break;
     }
+#pragma unroll
+    for (int r = 0; r < RPL / 2; ++r)
+#pragma unroll
+        for (int j = 0; j < WR; ++j) cswap(cl[r][j], cl[RPL - 1 - r][j], odd);
 
     // cluster in the colour layout
     int size = 0;
