@@ -40,6 +40,7 @@ struct DevPtrs {
     unsigned long long *rtSum, *rtCnt;          // [S][2][32] per (sample, chain), bin = floor(log2 pass)
     // cluster-move variants (NEXT-4, R36): single-cluster moves per houdayer_step at temperature index t
     int32_t *nclu;              // [T]
+    int32_t *tcold;             // [T] temperature indices by descending beta: the pairs with the largest clusters first
 };
 
 struct Params {
@@ -712,9 +713,12 @@ __global__ void __launch_bounds__(128, 6) k_houdayer(LAT lat, Params P, uint32_t
 {
     extern __shared__ uint32_t hsm[];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
-    const long pair = (long)blockIdx.x * wpb + wib;
-    if (pair >= (long)P.S * P.T) return;
-    const int s = (int)(pair / P.T), t = (int)(pair - (long)s * P.T);
+    // Launch order: coldest temperature first, all samples of one temperature next to each other.  Cluster sizes (and with
+    // them the rounds a pair needs) grow with beta, so the long pairs start first and the four pairs of a CTA take alike.
+    const long gw = (long)blockIdx.x * wpb + wib;
+    if (gw >= (long)P.S * P.T) return;
+    const int t = P.d.tcold[gw / P.S], s = (int)(gw % P.S);
+    const long pair = (long)s * P.T + t;
     if (move >= (uint32_t)P.d.nclu[t]) {                    // R36: this temperature makes no move number `move`
         if (move == 0 && lane == 0) P.d.last[pair] = 0;
         return;

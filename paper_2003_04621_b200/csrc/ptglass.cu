@@ -202,6 +202,7 @@ size_t carve(void *base, int L, int d, int S, int T, uint32_t strideX, DevPtrs *
     p.rtSum = c.take<unsigned long long>(base, (size_t)S * 2 * 32);
     p.rtCnt = c.take<unsigned long long>(base, (size_t)S * 2 * 32);
     p.nclu = c.take<int32_t>(base, (size_t)T);
+    p.tcold = c.take<int32_t>(base, (size_t)T);
     const size_t sb = std::max(R * N, (size_t)S * d * N);
     p.stage = c.take<int8_t>(base, sb);
     if (out) *out = p;
@@ -559,6 +560,10 @@ int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas,
     {
         const std::vector<int32_t> ones((size_t)n_temps, 1);
         CK(cudaMemcpyAsync(P.d.nclu, ones.data(), ones.size() * 4, cudaMemcpyHostToDevice, G.stream));
+        std::vector<int32_t> cold((size_t)n_temps);
+        for (int t = 0; t < n_temps; ++t) cold[t] = t;
+        std::stable_sort(cold.begin(), cold.end(), [&](int a, int b) { return betas[a] > betas[b]; });
+        CK(cudaMemcpyAsync(P.d.tcold, cold.data(), cold.size() * 4, cudaMemcpyHostToDevice, G.stream));
         CK(cudaStreamSynchronize(G.stream));
     }
 
