@@ -464,6 +464,8 @@ __device__ __forceinline__ bool swap_accept(const Params &P, int t, uint32_t u, 
     return u < swap_threshold(P, t, absdE);
 }
 
+constexpr int kExchangeTableT = 64;     // ladders up to this length evaluate all (carried, rung) decisions in parallel
+
 // dynamic smem: per warp [T] energies by temperature + [T] slot_of_temp + [T] draws + [T] signs / accept flags.  GLOBAL_SCRATCH (very long ladders):
 // the same walk on outE / slot_of_temp in global memory.
 template <bool GLOBAL_SCRATCH>
@@ -498,7 +500,59 @@ __global__ void k_exchange(Params P, uint32_t step)
             SG[t] = P.d.sgn[t];
         }
         __syncwarp();
-        if (lane == 0 && T > 1) {
+        if (T > 1 && T <= kExchangeTableT) {
+            // Short ladders: the walk is one dependent chain per (sample, chain) and the threshold lookup from L2 per rung
+            // is half of its stall samples.  The replica carried up to rung t is the ORIGINAL resident of some position
+            // j <= t, so every decision the walk can meet is one of the T (T-1) / 2 pairs (j, t): all lanes evaluate them
+            // side by side, eight independent lookups in flight per lane, then lane 0 walks with one byte load per rung.
+            uint8_t *ACC = (uint8_t *)(xsm + (size_t)wpb * 4 * T) + (size_t)wib * T * T;       // ACC[t * T + j]
+            for (int j = lane; j < T - 1; j += 32) {
+                const int32_t ej = Et[j];
+                for (int t0 = j; t0 < T - 1; t0 += 8) {
+                    if (!P.gauss) {
+                        uint32_t thr[8];
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) {
+                            const int t = min(t0 + k, T - 2);
+                            const int32_t dE = ej - Et[t + 1];
+                            const uint32_t m = (uint32_t)(dE < 0 ? -dE : dE) >> 2;
+                            thr[k] = __ldg(P.d.thrX + (size_t)t * P.strideX + min(m, P.strideX - 1u));
+                            if (m >= P.strideX) thr[k] = 0u;
+                        }
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) {
+                            const int t = t0 + k;
+                            if (t < T - 1) {
+                                const int32_t dE = ej - Et[t + 1];
+                                ACC[t * T + j] = ((long long)SG[t] * dE <= 0 || U[t] < thr[k]) ? 1 : 0;
+                            }
+                        }
+                    } else {
+                        for (int t = t0; t < min(t0 + 8, T - 1); ++t) {
+                            const int32_t dE = ej - Et[t + 1];
+                            bool acc = (long long)SG[t] * dE <= 0;
+                            if (!acc) acc = swap_accept(P, t, U[t], (uint32_t)(dE < 0 ? -dE : dE));
+                            ACC[t * T + j] = acc ? 1 : 0;
+                        }
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) {
+                ra = so[0];
+                int j = 0;
+                int32_t rb = so[1];
+                for (int t = 0; t < T - 1; ++t) {
+                    const int32_t rbn = (t + 2 < T) ? so[t + 2] : 0;       // positions > t + 1 are not modified before they are read
+                    const bool acc = ACC[t * T + j] != 0;
+                    so[t] = acc ? rb : ra;                                  // position t is final
+                    if (acc) SG[t] = 2;
+                    ra = acc ? ra : rb;
+                    j = acc ? j : t + 1;
+                    rb = rbn;
+                }
+            }
+        } else if (lane == 0 && T > 1) {
             ea = Et[0]; ra = so[0];
             int32_t eb = Et[1], rb = so[1];
             for (int t = 0; t < T - 1; ++t) {

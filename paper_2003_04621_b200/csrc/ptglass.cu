@@ -311,8 +311,8 @@ cudaError_t launch_exchange()
     const long chains = (long)G.P.S * 2;
     int wpb = 4;
     while (wpb > 1 && (size_t)wpb * 4 * T * 4 > 64 * 1024) wpb >>= 1;
-    const size_t smem = (size_t)wpb * 4 * T * 4;
-    if (smem > 64 * 1024) {      // very long ladders: walk on global scratch instead of shared memory
+    const size_t smem = (size_t)wpb * 4 * T * 4 + (T <= kExchangeTableT ? (size_t)wpb * T * T : 0);      // + the decision table
+    if ((size_t)wpb * 4 * T * 4 > 64 * 1024) {      // very long ladders: walk on global scratch instead of shared memory
         k_exchange<true><<<(unsigned)chains, 32, 0, G.stream>>>(G.P, G.n_exchange);
     } else {
         cudaError_t err = allow_smem(k_exchange<false>, smem);
