@@ -285,18 +285,26 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                     const int *Ec = sE + c * T;
                     int ra = so[0], ea = Ec[ra];
                     int rb = so[1], eb = Ec[rb];
-                    for (int t = 0; t < T - 1; ++t) {
-                        int rbn = 0, ebn = 0;
-                        if (t + 2 < T) { rbn = so[t + 2]; ebn = Ec[rbn]; }     // positions > t are not modified before they are read
+                    const uint32_t *Uc = sU + c * T;
+                    uint32_t *Ac = sAcc + c * T;
+                    const uint32_t *trow = P.d.thrX;                            // row of rung t of the +-J swap table
+#pragma unroll 1
+                    for (int t = 0; t < T - 1; ++t, trow += P.strideX) {
+                        const int tn = min(t + 2, T - 1);                       // positions > t are not modified before they are read
+                        const int rbn = so[tn], ebn = Ec[rbn];
                         const int dE = ea - eb;
                         bool acc = sSgn[t] * dE <= 0;
-                        if (!acc) {
-                            const uint32_t adE = (uint32_t)(dE < 0 ? -dE : dE);
-                            if constexpr (GAUSS != 0) acc = swap_accept(P, t, sU[c * T + t], adE);
-                            else acc = sU[c * T + t] < thrX_lookup(P, t, adE >> 2);
+                        if constexpr (GAUSS != 0) {
+                            if (!acc) acc = swap_accept(P, t, Uc[t], (uint32_t)(dE < 0 ? -dE : dE));
+                        } else {                                                // branch-free: the lookup is issued for every rung
+                            const uint32_t mm = (uint32_t)(dE < 0 ? -dE : dE) >> 2;
+                            const uint32_t thr = __ldg(trow + min(mm, P.strideX - 1u));
+                            acc = acc || (mm < P.strideX && Uc[t] < thr);
                         }
-                        if (acc) { so[t] = rb; sAcc[c * T + t] += 1u; }        // position t is final; (ea, ra) moves up
-                        else     { so[t] = ra; ea = eb; ra = rb; }
+                        so[t] = acc ? rb : ra;                                  // position t is final; on accept (ea, ra) moves up
+                        Ac[t] += acc ? 1u : 0u;
+                        ea = acc ? ea : eb;
+                        ra = acc ? ra : rb;
                         rb = rbn; eb = ebn;
                     }
                     so[T - 1] = ra;
