@@ -295,7 +295,7 @@ __global__ void __launch_bounds__(128) k_sweep_q(LAT lat, Params P, int R, uint3
                 const int dE = update_word_q<LAT, SMALL>(lat, sS + (qi * 2 + p) * W, sS + (qi * 2 + (1 - p)) * W, Jp, W, w, p, sC2[qi],
                                                          P.d.betasD + sT[qi], P.fbits, step0 + (uint32_t)it, g,
                                                          make_tag(DOM_METRO, p, c, r), P.rk);
-                if (dE != 0) atomicAdd(sdE + qi, dE);
+                atomicAdd(sdE + qi, dE);
             }
             __syncthreads();
         }

@@ -136,25 +136,22 @@ __device__ __forceinline__ int houdayer_lane(const LAT &lat, uint32_t *A0, uint3
         uint32_t nbC[2 * D];
         lat.gather_f([CC1](int i) { return CC1[i * SP]; }, w, 0, nbC);
         const uint32_t cb = CC0[w * SP];
-        uint32_t any = 0;
+        // no test for "no boundary bond in this word": with 32 pairs side by side some lane always has one
+        uint32_t nbA[2 * D];
+        lat.gather(A1, w, 0, nbA);
+        const uint32_t ab = A0[w];
 #pragma unroll
-        for (int k = 0; k < 2 * D; ++k) { nbC[k] ^= cb; any |= nbC[k]; }
-        if (any) {
-            uint32_t nbA[2 * D];
-            lat.gather(A1, w, 0, nbA);
-            const uint32_t ab = A0[w];
-#pragma unroll
-            for (int k = 0; k < 2 * D; ++k) {
-                const uint32_t uns = ab ^ nbA[k] ^ Jb[k * W + w];
-                dl += __popc(nbC[k]) - 2 * __popc(nbC[k] & uns);
-            }
+        for (int k = 0; k < 2 * D; ++k) {
+            const uint32_t bnd = nbC[k] ^ cb;
+            const uint32_t uns = ab ^ nbA[k] ^ Jb[k * W + w];
+            dl += __popc(bnd) - 2 * __popc(bnd & uns);
         }
     }
     // every read of the old A is done (same lane, program order): negate the cluster in both configurations
     for (int w = 0; w < W; ++w) {
         const uint32_t x0 = CC0[w * SP], x1 = CC1[w * SP];
-        if (x0) { A0[w] ^= x0; B0[w] ^= x0; }
-        if (x1) { A1[w] ^= x1; B1[w] ^= x1; }
+        A0[w] ^= x0; B0[w] ^= x0;
+        A1[w] ^= x1; B1[w] ^= x1;
     }
     delta = 2 * dl;
     return size;

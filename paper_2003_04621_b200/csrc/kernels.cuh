@@ -393,7 +393,7 @@ __global__ void __launch_bounds__(128, 7) k_sweep(LAT lat, Params P, int R, uint
                 for (int k = 0; k < D; ++k) thr[k] = sThr[4 * qi + k];
                 const int dE = update_word(lat, sS + (qi * 2 + p) * W, sS + (qi * 2 + (1 - p)) * W, sJ + p * 2 * D * W,
                                            W, w, p, thr, step0 + (uint32_t)it, g, make_tag(DOM_METRO, p, c, r), P.rk);
-                if (dE != 0) atomicAdd(sdE + qi, dE);
+                atomicAdd(sdE + qi, dE);
             }
             __syncthreads();
         }

@@ -183,7 +183,7 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                         dE = update_word(lat, sS + q * RS + p * W, sS + q * RS + (1 - p) * W, sJ + p * 2 * D * W, W, w,
                                          p, thr, step, g, make_tag(DOM_METRO, p, c, r), P.rk);
                     }
-                    if (dE != 0) atomicAdd(sE + q, dE);
+                    atomicAdd(sE + q, dE);
                 }
                 __syncthreads();
             }
