@@ -176,9 +176,9 @@ __device__ __forceinline__ int update_word_q(const LAT &lat, uint32_t *Sown, con
     const Round0Shared r0 = philox_round0_shared(step, g, tag, rk);
     uint32_t flip = 0;
     int dE = 0;
-#pragma unroll 2
+#pragma unroll 4        // measured: 2 -> 4 is +1.3 % on the fused Gaussian MCS, 8 is -14 % (instruction cache)
     for (int B = 0; B < 8; ++B) {
-        if ((vv & 0xFu) != 0u) {
+        if (LAT::kFast || (vv & 0xFu) != 0u) {          // the word-parallel lattices have no partial words
             uint32_t u[4];
             philox4x32_10_shared(8u * (uint32_t)w + (uint32_t)B, r0, rk, u[0], u[1], u[2], u[3]);
             int4 Jv[2 * D];
