@@ -36,7 +36,7 @@ UNIT = "flips/ns"
 SM_COUNT = 148
 INT32_LANES_PER_SM_CLK = 128       # 4 SMSPs x 1 warp-instruction/clk x 32 lanes (fma + alu pipes, 64 each)
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu --set full
-# capture of the same build (profiles/r1_v4_final.md): the packed state of C2 is read once per k_mcs launch (10.68 MB,
+# capture of the same build (profiles/r1_v5_variants_and_gauss.md; r1_v4_final.md before it): the packed state of C2 is read once per k_mcs launch (10.68 MB,
 # independent of the number of MCS per launch) and its write-back stays in L2 (0 B).  None where no capture exists.
 NCU_DRAM_BYTES_PER_LAUNCH = {("C2", "k_mcs"): 10.68e6}
 ALGO_OPS_PER_FLIP = {2: 20, 3: 22}  # Philox share 10 + 2d field terms + 6 decide/flip/accumulate
