@@ -268,10 +268,17 @@ __device__ __forceinline__ int houdayer_pair(const LAT &lat, uint32_t *A0, uint3
     // strips; chaotic relaxation of a monotone map reaches the same least fixed point in any order).
     const int n_lo = 2 * w_lo, n_hi = 2 * w_hi;
     auto ldCl = [Cl](int i) { return Cl[i + i / CHN]; };
+    // Even lanes sweep their strip down then up, odd lanes up then down, and the second sweep starts on the word the first
+    // one ended on: a front that reaches the bottom of an even strip is picked up by the odd strip below at the start of
+    // its downward sweep in the same round (and the mirror image upwards), so membership crosses two strips per round in
+    // either direction instead of one (as in houdayer_rows.cuh).
+    const int len = n_hi - n_lo;
+    const bool odd = lane & 1;
     for (;;) {
         bool changed = false;
-        for (int k = 0; k < 2 * (n_hi - n_lo) - 1; ++k) {
-            const int n = (k < n_hi - n_lo) ? n_lo + k : n_hi - 2 - (k - (n_hi - n_lo));
+        for (int k = 0; k < 2 * len; ++k) {
+            const int j = (k < len) ? k : 2 * len - 1 - k;          // 0 .. len-1, len-1 .. 0
+            const int n = odd ? n_hi - 1 - j : n_lo + j;
             const uint32_t neg = Neg[pos(n)], cur = Cl[pos(n)];
             if (neg & ~cur) {
                 const uint32_t seeds = (cur | NL::neighbour_union_f(ldCl, n, cur)) & neg;
