@@ -60,8 +60,10 @@ int pt_bind(void *device_workspace, size_t bytes, void *cuda_stream);
  * (R5, R6):  thrM[t][k] = THR(-(betas[t]*4k)), k = 1..d;  thrX[t][m] = THR(-(|betas[t+1]-betas[t]|*4m));
  * THR(x) = min(2^32-1, floor(2^32 exp(x))).
  * betas: HOST array [n_temps], any order, duplicates allowed (R7); index t = position in this array.
- * PT_ERR_ARG: d not in {2,3}; L < 2 or odd (checkerboard needs a bipartite periodic lattice, R3); n_samples < 1;
- * n_temps < 1 or > 65535; betas NULL, negative or non-finite; N*d > 2^31-1; sample_offset+n_samples > 2^32.
+ * PT_ERR_ARG: d not in {2,3}; L < 2 or odd (checkerboard needs a bipartite periodic lattice, R3); n_samples < 1 or
+ * > 65535 per context (larger sets: several shards through pt_init_shard); n_temps < 1 or > 65535; betas NULL, negative
+ * or non-finite; N*d > 2^31-1; a lattice whose coupling bits (4 d N / 8 bytes per sample) plus one replica exceed the
+ * 227 KiB of shared memory of a CTA (2D: L > 608, 3D: L > 62); sample_offset+n_samples > 2^32.
  * PT_ERR_STATE: no workspace bound or workspace too small. */
 int pt_init(int L, int d, int n_samples, int n_temps, const double *betas, uint64_t seed);
 /* Same, for a shard holding global samples [sample_offset, sample_offset + n_samples) (multi-GPU). */

@@ -35,6 +35,8 @@ struct Context {
     std::vector<double> betas;
     uint64_t seed = 0;
     uint32_t n_sweep = 0, n_exchange = 0, n_houdayer = 0;
+    uint64_t n_passes = 0;      // PT passes since pt_init = swap attempts per pair (R20); NOT the Philox step counter
+                                // n_exchange, which pt_set_counters overwrites on a resume
     bool q_small = false;       // fixed-point couplings with 2 D max|Jq| < 2^23 (gauss.cuh: accept_site<SMALL>)
     int max_clu = 1;            // max over t of the per-temperature cluster-move counts (NEXT-4, R36)
     uint64_t launches = 0;
@@ -122,6 +124,11 @@ int check_shape(int L, int d, int S, int T)
     if (T < 1 || T > 65535) return fail(PT_ERR_ARG, "n_temps must be in [1, 65535] (got %d)", T);
     const double Nd = std::pow((double)L, d) * d;
     if (Nd > 2147483647.0) return fail(PT_ERR_ARG, "N*d overflows int32");
+    if (S > 65535) return fail(PT_ERR_ARG, "n_samples must be <= 65535 per context (got %d): shard larger sets with pt_init_shard", S);
+    // the sweep kernel keeps a sample's coupling bits and at least one replica in shared memory
+    const double W = std::ceil(std::pow((double)L, d) / 64.0);
+    if ((2.0 * 2 * d * W + 2 * W + 8) * 4 > 227.0 * 1024)
+        return fail(PT_ERR_ARG, "lattice too large: %.0f KiB of coupling bits per sample do not fit in shared memory", 2.0 * 2 * d * W * 4 / 1024);
     return PT_OK;
 }
 
@@ -222,6 +229,9 @@ bool fast_supported(int L, int d)
     if (L < 8 || (L & (L - 1))) return false;
     int lg = 0;
     while ((1 << lg) < L) ++lg;
+#ifdef PTG_DEV_D
+    return d == PTG_DEV_D && lg == PTG_DEV_LG;      // development build: one fast lattice only (build.py)
+#endif
     return d == 2 ? (lg >= 3 && lg <= 8) : (lg >= 3 && lg <= 5);
 }
 
@@ -237,12 +247,18 @@ int grid_for(long total, int block) { return (int)std::min<long>((total + block 
 
 template <class F> void with_lattice(F body)
 {
+#ifdef PTG_DEV_D
+    if (G.fast) { FAST_CASE(PTG_DEV_D, PTG_DEV_LG) }
+    GenLat<PTG_DEV_D> dev_lat(G.P.L);
+    body(dev_lat);
+#else
     if (G.fast) {
         FAST_CASE(2, 3) FAST_CASE(2, 4) FAST_CASE(2, 5) FAST_CASE(2, 6) FAST_CASE(2, 7) FAST_CASE(2, 8)
         FAST_CASE(3, 3) FAST_CASE(3, 4) FAST_CASE(3, 5)
     }
     if (G.P.D == 2) { GenLat<2> lat(G.P.L); body(lat); }
     else            { GenLat<3> lat(G.P.L); body(lat); }
+#endif
 }
 
 template <class K> cudaError_t allow_smem(K kernel, size_t bytes)
@@ -556,6 +572,7 @@ int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas,
         return fail(PT_ERR_STATE, "workspace too small: %zu bytes bound, %zu needed", G.ws_bytes, need);
     G.fast = (G.force_general != 0) && fast_supported(L, d);
     G.n_sweep = G.n_exchange = G.n_houdayer = 0;
+    G.n_passes = 0;
     G.max_clu = 1;
     {
         const std::vector<int32_t> ones((size_t)n_temps, 1);
@@ -640,6 +657,7 @@ int pt_exchange(void)
     if (G.n_exchange == 4294967295u) return fail(PT_ERR_OVERFLOW, "exchange counter would overflow");
     CK(launch_exchange());
     G.n_exchange += 1;
+    G.n_passes += 1;
     return PT_OK;
 }
 
@@ -701,13 +719,13 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
         CK(launch_mcs(a));
         G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
         if (do_houdayer) G.n_houdayer += (uint32_t)M;
-        if (do_exchange) G.n_exchange += (uint32_t)M;
+        if (do_exchange) { G.n_exchange += (uint32_t)M; G.n_passes += M; }
         return PT_OK;
     }
     for (int m = 0; m < n_mcs; ++m) {
         if (n_metro > 0) { CK(launch_sweep(n_metro)); G.n_sweep += (uint32_t)n_metro; }
         if (do_houdayer) { CK(launch_houdayer_any(do_houdayer)); G.n_houdayer += 1; }
-        if (do_exchange) { CK(launch_exchange()); G.n_exchange += 1; }
+        if (do_exchange) { CK(launch_exchange()); G.n_exchange += 1; G.n_passes += 1; }
     }
     return PT_OK;
 }
@@ -719,21 +737,23 @@ int pt_mcs_measure_device(int n_mcs, int n_metro, int do_houdayer, int do_exchan
     if (measure_every < 1) return fail(PT_ERR_ARG, "pt_mcs_measure_device: measure_every must be >= 1");
     if (!Q_rec_dev) return fail(PT_ERR_ARG, "pt_mcs_measure_device: Q_rec_dev is NULL");
     if (n_mcs < 0 || n_metro < 0) return fail(PT_ERR_ARG, "pt_mcs_measure_device: n_mcs and n_metro must be >= 0");
+    if (do_houdayer < 0 || do_houdayer > 2) return fail(PT_ERR_ARG, "pt_mcs_measure_device: do_houdayer must be 0, 1 or 2");
     const size_t stride = (size_t)G.P.S * G.P.T;
+    const uint64_t M = (uint64_t)n_mcs;
+    // refused before anything runs, whichever path serves the call: the state is left unchanged (R21)
+    if ((uint64_t)G.n_sweep + M * (uint64_t)n_metro > 4294967295ull ||
+        (do_exchange && (uint64_t)G.n_exchange + M > 4294967295ull) ||
+        (do_houdayer && (uint64_t)G.n_houdayer + M > 4294967295ull))
+        return fail(PT_ERR_OVERFLOW, "a step counter would overflow");
     // ONE launch for the whole call where a CTA holds both chains of a sample: the records come from the resident state
     if (!G.P.gauss && n_mcs >= measure_every && (do_houdayer == 0 || do_houdayer == 1) && mcs_fused_eligible(nullptr, do_houdayer, true) &&
         !mcs_split_chains(do_houdayer) && (n_metro > 0 || do_houdayer || do_exchange)) {
-        const uint64_t M = (uint64_t)n_mcs;
-        if ((uint64_t)G.n_sweep + M * (uint64_t)n_metro > 4294967295ull ||
-            (do_exchange && (uint64_t)G.n_exchange + M > 4294967295ull) ||
-            (do_houdayer && (uint64_t)G.n_houdayer + M > 4294967295ull))
-            return fail(PT_ERR_OVERFLOW, "a step counter would overflow");
         const McsArgs a{n_mcs, n_metro, do_houdayer ? 1 : 0, do_exchange ? 1 : 0, 0, G.max_clu, G.n_sweep, G.n_houdayer,
                         G.n_exchange, measure_every, Q_rec_dev, QL_rec_dev};
         CK(launch_mcs(a));
         G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
         if (do_houdayer) G.n_houdayer += (uint32_t)M;
-        if (do_exchange) G.n_exchange += (uint32_t)M;
+        if (do_exchange) { G.n_exchange += (uint32_t)M; G.n_passes += M; }
         return PT_OK;
     }
     // otherwise exactly the calls it stands for
@@ -880,7 +900,7 @@ int pt_get_swap_counts(uint64_t *attempts, uint64_t *accepts)
         if (rc) return rc;
     }
     if (attempts)                                   // every pass proposes every neighbouring pair once (R9)
-        for (size_t k = 0; k < n; ++k) attempts[k] = G.n_exchange;
+        for (size_t k = 0; k < n; ++k) attempts[k] = G.n_passes;
     return PT_OK;
 }
 

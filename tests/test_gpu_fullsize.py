@@ -4,6 +4,9 @@ whole S on the device): C2-C5.  The oracle cannot run a whole config, so
        (every sample is a pure function of (seed, g), pin P8) and compared bit for bit, and
   (ii) size-independent invariants are checked on ALL samples: tracked E == recomputed E, the two maps are inverse
        permutations, attempts == number of passes, accepts <= attempts, Houdayer conserves E1+E2 and Q.
+and (iii), SURVEY 8(d)'s parity subset part (i): ALL S samples for the first 16 MCS, full state, against the oracle run
+as one process per host core over disjoint `sample_offset` ranges (tests/oracle_pool.py).  Part (ii) of the subset (sampled
+samples for the whole 10^4 MCS) is tests/test_gpu_zz_fulllength.py.
 Run on the B200 box with `-m gpu`."""
 import numpy as np
 import pytest
@@ -12,6 +15,7 @@ from oracle import ref
 from paper_2003_04621_b200 import binding as B
 from paper_2003_04621_b200 import build as build_mod
 from paper_2003_04621_b200 import workloads as wl
+from tests import oracle_pool as OP
 
 pytestmark = pytest.mark.gpu
 
@@ -120,32 +124,30 @@ def test_fused_and_separate_launches_agree_at_full_size():
         assert np.array_equal(fused[k], sep[k]), k
 
 
-@pytest.mark.parametrize("name,n_mcs,g", [("C2", 10000, 777), ("C3", 10000, 1301), ("C4", 2000, 77), ("C5", 500, 101)])
-def test_full_length_run_one_sample_against_the_oracle(name, n_mcs, g):
-    """The config's whole run of 10^4 MCS (C2, C3; a bounded prefix of it for C4, C5, whose single-core oracle needs
-    minutes per sample) at full S, L, T in bench.py's launch configuration (50 MCS per pt_mcs call, the overlap
-    measurement every k-th MCS where the config asks for it); global sample g is recomputed by the oracle through
-    sample_offset and compared bit for bit at MCS 10, 100, 1000 and at the end, with every overlap record in between."""
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
+def test_all_samples_first_16_mcs_full_state(name):
+    """SURVEY 8(d) parity subset (i): every one of the S samples of the config for its first 16 MCS in bench.py's launch
+    configuration (one pt_mcs / pt_mcs_measure_device call), compared bit for bit on the full state: spins, energies, both
+    maps, swap attempts / accepts, last and cumulative cluster sizes, Q, QL (and C3's overlap record after MCS 10).  A
+    blockIdx-dependent slip (a wrong Philox counter or slot index for some range of samples) cannot pass this."""
     w = wl.CONFIGS[name]
-    B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED)
-    o = ref.Oracle(w.L, w.d, 1, w.T, w.betas(), wl.SEED, g)
-    chunk = w.measure_every if w.measure_every else 50
-    checkpoints = {10, 100, 1000, n_mcs}
-    done = 0
-    while done < n_mcs:
-        n = min(chunk, n_mcs - done, min(c for c in checkpoints if c > done) - done)
-        B.pt_mcs(n, 1, w.houdayer, True)
-        o.mcs(n, 1, w.houdayer, True)
-        done += n
-        if w.measure_every and done % w.measure_every == 0:
-            Qg, QLg = B.pt_measure_overlap()
-            Qo, QLo = o.measure_overlap()
-            assert np.array_equal(Qo[0], Qg[g]) and np.array_equal(QLo[0], QLg[g]), (name, done)
-        if done in checkpoints:
-            st, a = B.state(), o.state()
-            for k in a:
-                if k != "counters":
-                    assert np.array_equal(a[k][0], st[k][g]), "%s sample %d after %d MCS: %s differs" % (name, g, done, k)
-    assert B.pt_recompute_energy()[1] == 0
-    assert tuple(B.pt_get_counters()) == (n_mcs, n_mcs, n_mcs if w.houdayer else 0)
-    o.close()
+    n_mcs = 16
+    pool = OP.OraclePool()
+    try:
+        futs = pool.submit_all_samples(w, n_mcs)                # the oracle runs on all host cores while the GPU works
+        B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED)
+        recs = run_like_bench(w, n_mcs)
+        st = B.state()
+        st["Q"], st["QL"] = B.pt_measure_overlap()
+        assert B.pt_recompute_energy()[1] == 0
+        want, orecs = OP.gather(futs, n_mcs)
+    finally:
+        pool.close()
+    for k in OP.STATE_KEYS + ("Q", "QL"):
+        if not np.array_equal(want[k], st[k]):
+            bad = np.argwhere(want[k] != st[k])
+            raise AssertionError("%s after %d MCS: %s differs at %d places, first at %s (sample %d)" % (
+                name, n_mcs, k, len(bad), bad[0], bad[0][0]))
+    assert len(orecs) == len(recs) == (n_mcs // w.measure_every if w.measure_every else 0)
+    for (qa, qla), (qb, qlb) in zip(orecs, recs):
+        assert np.array_equal(qa, qb) and np.array_equal(qla, qlb)

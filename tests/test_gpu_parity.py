@@ -57,6 +57,32 @@ def test_philox_device_known_answers_and_oracle():
         assert np.array_equal(got[n], ref.philox(key, ctr[n]))
 
 
+def test_philox_device_against_the_toolkits_curand_philox():
+    """Pin P1, second half (PAPER.md:167 refs [70, 71]): the library's device Philox, the oracle's and the
+    CUDA toolkit's own curand_Philox4x32_10(ctr, key) give the same four words, in the same order (R25), for the known
+    answers and for counters laid out like the method's five domains."""
+    import json, os
+    from tests import native
+
+    B.pt_open(32, 2, 8, 8, wl.betas_linear(0.2, 1.0, 8), SEED)
+    with open(os.path.join(os.path.dirname(__file__), "golden", "philox_known_answers.json")) as f:
+        for v in json.load(f)["vectors"]:
+            out = native.curand_philox([int(k, 16) for k in v["key"]], [[int(c, 16) for c in v["ctr"]]])
+            assert ["%08x" % x for x in out[0]] == v["out"]
+    rng = np.random.default_rng(11)
+    ctr = rng.integers(0, 2 ** 32, size=(4096, 4), dtype=np.uint64).astype(np.uint32)
+    # counters shaped like the method's: (index, step, global sample, (domain << 28) | (aux << 24) | (chain << 16) | idx16)
+    for k in range(2048):
+        dom = 1 + k % 5
+        ctr[k] = (k * 7, k // 3, 1000 + k % 11, (dom << 28) | ((k % 3) << 24) | ((k & 1) << 16) | (k % 48))
+    key = np.array([SEED & 0xFFFFFFFF, SEED >> 32], dtype=np.uint32)
+    lib_words = B.pt_philox_selftest(key, ctr)
+    cur_words = native.curand_philox(key, ctr)
+    assert np.array_equal(lib_words, cur_words)
+    for n in range(0, 4096, 131):
+        assert np.array_equal(cur_words[n], ref.philox(key, ctr[n]))
+
+
 # (L, d, S, T): fast path = L a power of two >= 8; the others run the general-L kernels
 SHAPES = [(8, 2, 4, 8), (16, 2, 3, 5), (32, 2, 3, 6), (64, 2, 2, 3), (128, 2, 1, 3),
           (8, 3, 3, 4), (16, 3, 2, 3),
@@ -282,6 +308,8 @@ def test_checkpoint_and_resume_continue_bit_identically(L, d, S, T, general):
     for k in ("spins", "energy", "temp_of_slot", "slot_of_temp", "last_size", "counters"):
         assert np.array_equal(a[k], b[k]), k
     assert B.pt_recompute_energy()[1] == 0
+    # the observables that count since init restart at the re-init (ptglass.h): 9 passes, not the restored step counter
+    assert (b["attempts"] == 9).all() and (b["accepts"] <= b["attempts"]).all()
     with pytest.raises(B.PTError) as e:                         # not a permutation
         bad = sot.copy(); bad[0, 0, 0] = bad[0, 0, 1]
         B.pt_set_perm(bad)
@@ -297,8 +325,13 @@ def test_counter_overflow_is_refused_and_leaves_the_state_alone():
     B.pt_mcs(1, 2, True, True)                                  # reaches (top, top, top) exactly: allowed
     assert tuple(B.pt_get_counters()) == (top, top, top)
     st0 = B.state()
+    assert (st0["attempts"] == 1).all()                         # passes since init, whatever pt_set_counters placed (R20)
+    import torch
+    Qr = torch.empty((4, S, T), dtype=torch.int32, device="cuda")
     for fn in (lambda: B.pt_sweep(1), B.pt_exchange, B.houdayer_step, B.houdayer_multi_step,
-               lambda: B.pt_mcs(1, 1, True, True), lambda: B.pt_mcs(1, 0, False, True), lambda: B.pt_mcs(1, 0, 2, False)):
+               lambda: B.pt_mcs(1, 1, True, True), lambda: B.pt_mcs(1, 0, False, True), lambda: B.pt_mcs(1, 0, 2, False),
+               lambda: B.pt_mcs_measure_device(4, 1, True, True, 1, Qr), lambda: B.pt_mcs_measure_device(3, 0, 2, True, 1, Qr),
+               lambda: B.pt_mcs_measure_device(2, 1, False, False, 2, Qr)):
         with pytest.raises(B.PTError) as e:
             fn()
         assert e.value.code == B.PT_ERR_OVERFLOW
