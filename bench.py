@@ -1,18 +1,26 @@
 #!/usr/bin/env python
 """bench.py -- attempted spin flips / ns on B200 for the PT spin-glass hot path (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5] [--impl ours|reference]
 
-A STEP is `--mcs-per-step` Monte Carlo steps (one Metropolis sweep of every replica, one
-Houdayer cluster exchange per equal-temperature pair where the config enables it, one parallel-tempering pass,
-plus the overlap measurement every k-th MCS where the config asks for it) of the whole workload, issued as one
-pt_mcs() / pt_mcs_measure_device() call through the C ABI.  At N=1 the workload is BASELINE.json configs[1] (C2: 2D L=32, 1024 samples x
-32 temperatures x 2 chains, Houdayer + PT every sweep).  With the default K=200, 50 MCS per step the timed region is
-exactly the config's 10^4 MCS.  Inputs are synthetic (seeded +-J samples) and resident in HBM when the
-timed region starts; L2 is flushed between steps (untimed); each step is timed with CUDA events on the library's
-stream; multi-GPU = independent sample shards (weak scaling, no data-path collective), max over ranks.
+A STEP is `--mcs-per-step` Monte Carlo steps (one Metropolis sweep of every replica, one Houdayer
+cluster exchange per equal-temperature pair where the config enables it, one parallel-tempering pass, plus the overlap
+measurement every k-th MCS where the config asks for it) of the whole workload, issued as one pt_mcs() /
+pt_mcs_measure_device() call through the C ABI.
 
-`--impl reference` times the CPU oracle (oracle/, as it stands, one core) on a bounded sample of the same workload.
+BASELINE.json's metric names no config, so the HEADLINE workload is the largest single-GPU configuration, C5 (2D L=128,
+128 samples x 48 temperatures x 2 chains, Houdayer + PT every sweep: 2.0e12 attempted flips in its 10^4 MCS); with the
+default K=200, 50 MCS per step the timed region is exactly the config's 10^4 MCS.  The other configs C1-C4 are timed in
+the same run, each over `--config-steps` steps, and reported in the `per_config` block of the same JSON line (value,
+ms_per_step, roofline, clocks, kernel and phase times).  Inputs are synthetic (seeded +-J samples) and
+resident in HBM when the timed region starts; L2 is flushed between steps (untimed); each step is timed with CUDA events
+on the library's stream; multi-GPU = independent sample shards (weak scaling, no data-path collective), max over ranks.
+
+The timed region runs WITHOUT per-launch instrumentation; the per-kernel-class CUDA-event times and the phase clocks of
+the fused kernel come from a second, instrumented pass of a few steps right after it (`roofline.kernel_ms_pass`).
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on all host cores, one process per core on disjoint
+sample ranges, each step a bounded sample of the same workload.
 """
 from __future__ import annotations
 
@@ -35,11 +43,16 @@ METRIC = "attempted_spin_flips_per_ns"
 UNIT = "flips/ns"
 SM_COUNT = 148
 INT32_LANES_PER_SM_CLK = 128       # 4 SMSPs x 1 warp-instruction/clk x 32 lanes (fma + alu pipes, 64 each)
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu --set full
-# capture of the same build (profiles/r1_v5_variants_and_gauss.md; r1_v4_final.md before it): the packed state of C2 is read once per k_mcs launch (10.68 MB,
-# independent of the number of MCS per launch) and its write-back stays in L2 (0 B).  None where no capture exists.
-NCU_DRAM_BYTES_PER_LAUNCH = {("C2", "k_mcs"): 10.68e6}
 ALGO_OPS_PER_FLIP = {2: 20, 3: 22}  # Philox share 10 + 2d field terms + 6 decide/flip/accumulate
+KERNEL_CLASSES = ["k_sweep", "k_houdayer", "k_exchange", "k_measure", "k_mcs"]
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from committed `ncu --set full` captures
+# (never measured in this run: a number taken under a profiler is not a bench value).  (workload, kernel) -> (bytes, file)
+NCU_TRAFFIC = {}
+try:
+    with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as _f:
+        NCU_TRAFFIC = {tuple(k.split("/")): (v["dram_bytes_per_launch"], v["source"]) for k, v in json.load(_f).items()}
+except Exception:
+    pass
 
 
 def parse():
@@ -47,11 +60,13 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="C2", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--workload", default="C5", choices=sorted(wl.CONFIGS))
     ap.add_argument("--mcs-per-step", type=int, default=50)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true")
+    ap.add_argument("--config-steps", type=int, default=20, help="timed steps of each per_config entry")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--gaussian", action="store_true", help="NEXT-3: Gaussian couplings in fixed point (16 fractional bits)")
     ap.add_argument("--track-round-trips", action="store_true", help="NEXT-1: tunnelling-time bookkeeping in every PT pass")
@@ -83,11 +98,7 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
 
-    def stop(self, t0, t1):
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
+    def window(self, t0, t1):
         rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.15 and len(r) >= 8] or [r for (_, r) in self.rows[-3:]]
         sm = [float(r[0]) for r in rows if r[0].replace(".", "").isdigit()]
         reasons = set()
@@ -100,6 +111,10 @@ class ClockSampler:
                 "power_w_max": max([float(r[2]) for r in rows if r[2].replace(".", "").isdigit()] or [0.0]),
                 "samples": len(rows), "reasons": sorted(reasons)}
 
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
+
 
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -109,64 +124,79 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
-# --------------------------------------------------------------------------------------------------------------
-def oracle_time(w, S, n_mcs, seed=wl.SEED, gaussian=False, cluster="single"):
-    """Time the oracle as it stands on one host core; returns (flips/ns, seconds, flips)."""
-    from oracle import ref
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
 
-    o = ref.Oracle(w.L, w.d, S, w.T, w.betas(), seed)
-    if gaussian:
-        o.set_couplings_fixed(wl.gaussian_couplings_fixed(seed, S, w.d, w.N, 16), 16)
-    hd = (2 if cluster == "multi" else 1) if w.houdayer else 0
-    if w.houdayer and cluster == "counts":
-        o.set_cluster_moves(np.array([1 + (3 * t) // max(w.T - 1, 1) for t in range(w.T)], dtype=np.int32)[::-1].copy())
-    t0 = time.perf_counter()
-    for m in range(1, n_mcs + 1):
-        o.mcs(1, 1, hd, True)
-        if w.measure_every and m % w.measure_every == 0:
-            o.measure_overlap()
-    dt = time.perf_counter() - t0
-    flips = w.flips_per_sweep(S) * n_mcs
-    o.close()
-    return flips / dt * 1e-9, dt, flips
+
+def cluster_args(a, w):
+    """(do_houdayer mode, per-temperature move counts or None) of the workload under --cluster."""
+    hd = (2 if a.cluster == "multi" else 1) if w.houdayer else 0
+    n_clu = None
+    if w.houdayer and a.cluster == "counts":       # index 0 is the lowest beta = the hot end
+        n_clu = np.array([1 + (3 * t) // max(w.T - 1, 1) for t in range(w.T)], dtype=np.int32)[::-1].copy()
+    return hd, n_clu
+
+
+# --------------------------------------------------------------------------------------------------------------
+def oracle_rate(a, w, procs, samples_per_proc, target_flips_per_proc):
+    """The oracle as it stands on `procs` host cores (one single-threaded process per core, disjoint sample ranges,
+    PAPER.md:241).  Returns (aggregate flips/ns, seconds, flips, MCS)."""
+    from oracle import pool as OP
+
+    hd, n_clu = cluster_args(a, w)
+    fixed = None
+    if a.gaussian:
+        fixed = (wl.gaussian_couplings_fixed(wl.SEED, procs * samples_per_proc, w.d, w.N, 16), 16)
+    n_mcs = max(1, int(target_flips_per_proc / w.flips_per_sweep(samples_per_proc)))
+    po = OP.PersistentOracles(w, procs, samples_per_proc, houdayer_mode=hd, fixed=fixed,
+                              n_clu=None if n_clu is None else n_clu.tolist())
+    try:
+        po.step(1)                                   # first touch of every page
+        t0 = time.perf_counter()
+        po.step(n_mcs)
+        dt = time.perf_counter() - t0
+    finally:
+        po.close()
+    flips = w.flips_per_sweep(procs * samples_per_proc) * n_mcs
+    return flips / dt * 1e-9, dt, flips, n_mcs
 
 
 def run_reference(a, w, rank):
-    """--impl reference: the CPU oracle, one core, each step a bounded sample (2 samples) of the workload."""
+    """--impl reference: the CPU oracle on all host cores; each step a bounded sample of the workload."""
     if rank != 0:
         return
-    S_ref = 2
-    from oracle import ref
+    from oracle import pool as OP
 
-    o = ref.Oracle(w.L, w.d, S_ref, w.T, w.betas(), wl.SEED)
-    if a.gaussian:
-        o.set_couplings_fixed(wl.gaussian_couplings_fixed(wl.SEED, S_ref, w.d, w.N, 16), 16)
-
-    hd = (2 if a.cluster == "multi" else 1) if w.houdayer else 0
-    if w.houdayer and a.cluster == "counts":
-        o.set_cluster_moves(np.array([1 + (3 * t) // max(w.T - 1, 1) for t in range(w.T)], dtype=np.int32)[::-1].copy())
-
-    def step():
-        o.mcs(a.mcs_per_step, 1, hd, True)
-        if w.measure_every:
-            for _ in range(a.mcs_per_step // w.measure_every):
-                o.measure_overlap()
-
-    for _ in range(a.warmup):
-        step()
-    t0 = time.perf_counter()
-    for _ in range(a.steps):
-        step()
-    dt = time.perf_counter() - t0
-    flips = w.flips_per_sweep(S_ref) * a.mcs_per_step * a.steps
+    P = OP.n_cores()
+    hd, n_clu = cluster_args(a, w)
+    fixed = (wl.gaussian_couplings_fixed(wl.SEED, P, w.d, w.N, 16), 16) if a.gaussian else None
+    ref_mcs = max(1, min(a.mcs_per_step, int(round(0.25 / (w.flips_per_sweep(1) * 30e-9)))))
+    po = OP.PersistentOracles(w, P, 1, houdayer_mode=hd, fixed=fixed, n_clu=None if n_clu is None else n_clu.tolist())
+    try:
+        for _ in range(a.warmup):
+            po.step(ref_mcs)
+        t0 = time.perf_counter()
+        for _ in range(a.steps):
+            po.step(ref_mcs)
+        dt = time.perf_counter() - t0
+    finally:
+        po.close()
+    flips = w.flips_per_sweep(P) * ref_mcs * a.steps
     v = flips / dt * 1e-9
-    sample = "%s restricted to the first %d samples, %d MCS per step" % (w.name, S_ref, a.mcs_per_step)
+    sample = "%s restricted to %d samples (one oracle process per host core), %d MCS per step" % (w.name, P, ref_mcs)
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
         "warmup": a.warmup, "ms_per_step": dt / a.steps * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "int32", "data": "synthetic",
         "config": config_of(a, w, a.gpus, sample=sample),
-        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": P, "kind": "oracle", "sample": sample, "cpu": cpu_model()},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
@@ -184,6 +214,195 @@ def config_of(a, w, n_gpus, sample=None):
     if sample:
         c["sample"] = sample
     return c
+
+
+# --------------------------------------------------------------------------------------------------------------
+class GpuRun:
+    """One workload on this rank's GPU: the context, the step, the timed region, the instrumented pass."""
+
+    def __init__(self, a, w, rank, world, dev, flush):
+        import torch
+        from paper_2003_04621_b200 import binding as B
+
+        self.a, self.w, self.rank, self.world, self.dev, self.flush, self.B, self.torch = a, w, rank, world, dev, flush, B, torch
+        B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED, sample_offset=rank * w.S, device=dev,
+                  track_round_trips=a.track_round_trips)
+        if a.gaussian:
+            B.pt_set_couplings_fixed(wl.gaussian_couplings_fixed(wl.SEED, w.S, w.d, w.N, 16, sample_offset=rank * w.S), 16)
+        self.hd, n_clu = cluster_args(a, w)
+        if n_clu is not None:
+            B.pt_set_cluster_moves(n_clu)
+        self.n_meas = (a.mcs_per_step // w.measure_every) if w.measure_every else 0
+        self.Qrec = torch.empty((max(self.n_meas, 1), w.S, w.T), dtype=torch.int32, device=dev)
+        self.QLrec = torch.empty_like(self.Qrec)
+        self.flips_step = w.flips_per_sweep() * a.mcs_per_step
+
+    def step(self):
+        if self.n_meas == 0:
+            self.B.pt_mcs(self.a.mcs_per_step, 1, self.hd, True)
+        else:                                    # the MCS with the overlap records fused in (one launch where eligible)
+            self.B.pt_mcs_measure_device(self.a.mcs_per_step, 1, self.hd, True, self.w.measure_every, self.Qrec, self.QLrec)
+
+    def barrier(self):
+        self.torch.cuda.synchronize()
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+            self.torch.cuda.synchronize()
+
+    def max_over_ranks(self, x):
+        if self.world > 1:
+            import torch.distributed as dist
+            t = self.torch.tensor([x], dtype=self.torch.float64, device=self.dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            return float(t.item())
+        return x
+
+    def timed(self, steps, warmup, sampler):
+        """W untimed warm-up steps, then exactly `steps` steps, each bracketed by CUDA events on the library's stream
+        (the L2 flush between steps is outside the events); barrier + synchronize on both sides; max over ranks."""
+        torch, B = self.torch, self.B
+        for _ in range(warmup):
+            self.step()
+        self.barrier()
+        launches0 = B.pt_get_launch_count()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        self.barrier()
+        t0 = time.time()
+        for k in range(steps):
+            self.flush.fill_(k & 0xFF)
+            evs[k][0].record()
+            self.step()
+            evs[k][1].record()
+        self.barrier()
+        t1 = time.time()
+        ms_total = self.max_over_ranks(sum(e0.elapsed_time(e1) for e0, e1 in evs))
+        launches = B.pt_get_launch_count() - launches0
+        assert B.pt_recompute_energy()[1] == 0, "tracked energies diverged from recomputed energies"
+        return {"value": self.world * self.flips_step * steps / (ms_total * 1e6), "ms_per_step": ms_total / steps,
+                "ms_total": ms_total, "steps": steps, "gpu_launches": int(launches),
+                "clocks": sampler.window(t0, t1) if sampler else None}
+
+    def instrumented(self, steps, t):
+        """Second pass (outside the timed region): every launch bracketed by CUDA events (per-class kernel times), the fused
+        kernel's phase clocks on, then the Metropolis sweeps alone.  Returns the roofline block."""
+        torch, B, a, w = self.torch, self.B, self.a, self.w
+        peaks, peaks_kind = measured_peaks()
+        B.pt_set_sample_groups(1)                 # one stream: per-class kernel times that do not overlap one another
+        B.pt_set_profiling(True)
+        B.pt_set_phase_clocks(True)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        for _ in range(steps):
+            self.step()
+        ev1.record()
+        kms, kn = B.pt_get_kernel_times()
+        pclk = B.pt_get_phase_clocks().astype(np.float64)
+        B.pt_set_phase_clocks(False)
+        B.pt_set_profiling(False)
+        B.pt_set_sample_groups(-1)
+        pass_ms = ev0.elapsed_time(ev1)
+        fused = kn[4] > 0
+        dom = 4 if fused else 0                   # the roofline is quoted for the kernel that does the Metropolis sweeps
+        n_mcs_pass = a.mcs_per_step * steps
+        if fused:                                 # one launch per step: the un-instrumented step time IS the launch time
+            mcs_per_launch = max(1, n_mcs_pass // max(int(kn[4]), 1))
+            dom_ms = t["ms_per_step"] * mcs_per_launch / a.mcs_per_step
+        else:
+            mcs_per_launch = 1
+            dom_ms = kms[0] / max(int(kn[0]), 1)
+        flips_per_launch = w.flips_per_sweep() * mcs_per_launch
+        dom_flips_ns = flips_per_launch / (dom_ms * 1e6) if dom_ms > 0 else 0.0
+        A = ALGO_OPS_PER_FLIP[w.d]
+        f_max = peaks.get("sm_max_mhz", 1965.0) / 1e3
+        peak_ops = SM_COUNT * INT32_LANES_PER_SM_CLK * f_max
+        # ---- per-phase time per spin in the paper's normalisation, Eq. (11): t_update = t_kernel / (N_T N_R N_C N_B L^d)
+        spins_mcs = float(w.flips_per_sweep())
+        if fused:
+            share = pclk / max(pclk.sum(), 1.0)
+            per_mcs_us = t["ms_per_step"] / a.mcs_per_step * 1e3
+            ph = {"metropolis": share[0] * per_mcs_us, "houdayer": share[1] * per_mcs_us, "exchange": share[2] * per_mcs_us,
+                  "rest": share[3] * per_mcs_us}
+            how = "fused launch: un-instrumented time per MCS x the CTA clock64() share of each phase (pt_set_phase_clocks)"
+        else:
+            ph = {"metropolis": kms[0] / n_mcs_pass * 1e3, "houdayer": kms[1] / n_mcs_pass * 1e3,
+                  "exchange": kms[2] / n_mcs_pass * 1e3, "rest": max(pass_ms - kms[:4].sum(), 0.0) / n_mcs_pass * 1e3}
+            how = ("separate launches: CUDA events around every launch of the instrumented pass, which runs on ONE stream "
+                   "(pt_set_sample_groups(1)); rest = gaps between launches; the timed region overlaps sample groups on streams")
+        phases = {"us_per_mcs": ph, "ns_per_spin": {k: v * 1e3 / spins_mcs for k, v in ph.items()},
+                  "houdayer_over_metropolis": (ph["houdayer"] / ph["metropolis"]) if ph["metropolis"] > 0 else None,
+                  "exchange_over_metropolis": (ph["exchange"] / ph["metropolis"]) if ph["metropolis"] > 0 else None,
+                  "how": how, "paper": "cluster update 2-5x the Metropolis time per spin (P:197); PT small (P:231)"}
+        traffic = NCU_TRAFFIC.get((w.name, KERNEL_CLASSES[dom])) if not a.gaussian and a.cluster == "single" else None
+        roofline = {
+            "bound": "alu", "kernel": KERNEL_CLASSES[dom], "achieved": A * dom_flips_ns, "peak": peak_ops,
+            "unit": "Gop/s (INT32 thread-ops)", "frac": A * dom_flips_ns / peak_ops,
+            "traffic": traffic[0] if traffic else None,
+            "traffic_source": traffic[1] if traffic else None,
+            "peak_how": "derived: 148 SMs x 128 INT32 lanes/clk (fma+alu pipes) x %.3f GHz max SM clock; achieved = A x attempted flips "
+                        "per launch / launch time with A = %d ALGORITHMIC ops/flip (Philox 10 + field 2d + decide 6), not an ncu counter; "
+                        "a %s launch = %d MCS = %d attempted flips" % (f_max, A, KERNEL_CLASSES[dom], mcs_per_launch, flips_per_launch),
+            "flips_per_ns": dom_flips_ns, "ms_per_launch": dom_ms,
+            "whole_mcs_frac": A * t["value"] / self.world / peak_ops,
+            "hbm": {"algorithmic_bytes_per_flip": 0.25 / mcs_per_launch, "achieved_gbs": 0.25 / mcs_per_launch * dom_flips_ns,
+                    "peak_gbs": peaks.get("hbm_gbs"), "peak_kind": peaks_kind,
+                    "frac": 0.25 / mcs_per_launch * dom_flips_ns / peaks.get("hbm_gbs", 6650.0)},
+            "kernel_ms": {n: float(kms[i]) for i, n in enumerate(KERNEL_CLASSES)},
+            "kernel_launches": {n: int(kn[i]) for i, n in enumerate(KERNEL_CLASSES)},
+            "kernel_ms_pass": "%d instrumented steps (%d MCS) after the timed region, %.3f ms in all" % (steps, n_mcs_pass, pass_ms),
+            "phases": phases,
+        }
+        # the Metropolis sweeps alone (a1-a3; Eq. (11) normalisation), same state, resident for mcs_per_step sweeps
+        B.pt_set_profiling(True)
+        for _ in range(3):
+            B.pt_sweep(a.mcs_per_step)
+        sms, sn = B.pt_get_kernel_times()
+        B.pt_set_profiling(False)
+        so = w.flips_per_sweep() * a.mcs_per_step / (sms[0] / max(int(sn[0]), 1) * 1e6)
+        roofline["sweep_only"] = {"kernel": "k_sweep", "flips_per_ns": so, "frac": A * so / peak_ops,
+                                  "what": "pt_sweep(%d) launches, no Houdayer / exchange" % a.mcs_per_step}
+        assert B.pt_recompute_energy()[1] == 0
+        return roofline
+
+    def measurement_kernels(self):
+        """The two measurement kernels alone (a6 and the NEXT-2 overlap profile), CUDA events around 20 calls each."""
+        torch, B, w = self.torch, self.B, self.w
+        prof_d = torch.empty((w.S, w.T, w.d, w.L), dtype=torch.int32, device=self.dev)
+        out = {}
+        for label, fn in (("overlap", lambda: B.pt_measure_overlap_device(self.Qrec[0], self.QLrec[0])),
+                          ("overlap_profile", lambda: B.pt_measure_overlap_profile_device(prof_d))):
+            for _ in range(3):
+                fn()
+            torch.cuda.synchronize()
+            m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            m0.record()
+            for _ in range(20):
+                fn()
+            m1.record()
+            torch.cuda.synchronize()
+            out[label] = m0.elapsed_time(m1) / 20 * 1e3
+        return out
+
+    def e2e(self, steps):
+        """End to end through the C ABI with HOST buffers: H2D of the int8 spins, the step, D2H of the energies."""
+        torch, B, w = self.torch, self.B, self.w
+        host_spins = torch.empty((w.S, 2, w.T, w.N), dtype=torch.int8).pin_memory()
+        host_E = torch.empty((w.S, 2, w.T), dtype=torch.int32).pin_memory()
+        hs, hE = host_spins.numpy(), host_E.numpy()
+        B.pt_get_spins(out=hs)
+        for _ in range(2):
+            B.pt_set_spins(hs); self.step(); B.pt_get_energy(out=hE)
+        self.barrier()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            B.pt_set_spins(hs)
+            self.step()
+            B.pt_get_energy(out=hE)            # synchronises
+        self.barrier()
+        dt = self.max_over_ranks(time.perf_counter() - t0)
+        return {"value": self.world * self.flips_step * steps / (dt * 1e9), "unit": UNIT,
+                "h2d_bytes_per_step": int(hs.nbytes), "d2h_bytes_per_step": int(hE.nbytes),
+                "steps": steps, "what": "pt_set_spins(host int8, pinned) + step + pt_get_energy(host), wall clock"}
 
 
 # --------------------------------------------------------------------------------------------------------------
@@ -212,86 +431,14 @@ def main():
         dist.barrier()
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-
-    # weak scaling: every rank holds the full per-GPU workload on its own range of global sample indices
-    B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED, sample_offset=rank * w.S, device=dev,
-              track_round_trips=a.track_round_trips)
-    if a.gaussian:
-        B.pt_set_couplings_fixed(wl.gaussian_couplings_fixed(wl.SEED, w.S, w.d, w.N, 16, sample_offset=rank * w.S), 16)
     flush = torch.empty(512 * 2 ** 20, dtype=torch.uint8, device=dev)
-    n_meas = (a.mcs_per_step // w.measure_every) if w.measure_every else 0
-    hd = (2 if a.cluster == "multi" else 1) if w.houdayer else 0
-    if w.houdayer and a.cluster == "counts":       # index 0 is the lowest beta = the hot end
-        B.pt_set_cluster_moves(np.array([1 + (3 * t) // max(w.T - 1, 1) for t in range(w.T)], dtype=np.int32)[::-1].copy())
-
-    Qrec = torch.empty((max(n_meas, 1), w.S, w.T), dtype=torch.int32, device=dev)
-    QLrec = torch.empty_like(Qrec)
-
-    def step():
-        if n_meas == 0:
-            B.pt_mcs(a.mcs_per_step, 1, hd, True)
-        else:                                    # the MCS with the overlap records fused in (one launch where eligible)
-            B.pt_mcs_measure_device(a.mcs_per_step, 1, hd, True, w.measure_every, Qrec, QLrec)
-
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-            torch.cuda.synchronize()
-
-    for _ in range(a.warmup):
-        step()
-    barrier()
     sampler = ClockSampler(local) if rank == 0 else None
-    B.pt_set_profiling(True)
-    launches0 = B.pt_get_launch_count()
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(a.steps)]
-    barrier()
-    t_wall0 = time.time()
-    for k in range(a.steps):
-        flush.fill_(k & 0xFF)                 # L2 flush, outside the timed events
-        evs[k][0].record()
-        step()
-        evs[k][1].record()
-    barrier()
-    t_wall1 = time.time()
-    ms_total = sum(e0.elapsed_time(e1) for e0, e1 in evs)
-    kms, kn = B.pt_get_kernel_times()
-    B.pt_set_profiling(False)
-    launches = B.pt_get_launch_count() - launches0
-    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    flips_step = w.flips_per_sweep() * a.mcs_per_step
-    value = world * flips_step * a.steps / (ms_total * 1e6)
-    assert B.pt_recompute_energy()[1] == 0, "tracked energies diverged from recomputed energies"
 
-    # ---- end to end through the C ABI with HOST buffers: H2D of the int8 spins, the step, D2H of the energies
-    e2e = None
-    if not a.no_e2e:
-        host_spins = torch.empty((w.S, 2, w.T, w.N), dtype=torch.int8).pin_memory()
-        host_E = torch.empty((w.S, 2, w.T), dtype=torch.int32).pin_memory()
-        hs, hE = host_spins.numpy(), host_E.numpy()
-        B.pt_get_spins(out=hs)
-        for _ in range(2):
-            B.pt_set_spins(hs); step(); B.pt_get_energy(out=hE)
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(a.e2e_steps):
-            B.pt_set_spins(hs)
-            step()
-            B.pt_get_energy(out=hE)            # synchronises
-        barrier()
-        dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-        e2e = {"value": world * flips_step * a.e2e_steps / (dt * 1e9), "unit": UNIT,
-               "h2d_bytes_per_step": int(hs.nbytes), "d2h_bytes_per_step": int(hE.nbytes),
-               "steps": a.e2e_steps, "what": "pt_set_spins(host int8) + step + pt_get_energy(host), wall clock"}
+    # ---- headline: weak scaling, every rank holds the full per-GPU workload on its own range of global sample indices
+    run = GpuRun(a, w, rank, world, dev, flush)
+    t = run.timed(a.steps, a.warmup, sampler)
+    roofline = run.instrumented(min(a.steps, 10), t) if rank == 0 or world > 1 else None
+    e2e = None if a.no_e2e else run.e2e(a.e2e_steps)
 
     if rank != 0:
         if world > 1:
@@ -299,75 +446,54 @@ def main():
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel of the timed region (INT32 issue; live CUDA-event launch times)
-    peaks, peaks_kind = measured_peaks()
-    f_ghz = (clocks["sm_mhz"] or peaks.get("sm_max_mhz", 1965.0)) / 1e3 if clocks else 1.965
-    names = ["k_sweep", "k_houdayer", "k_exchange", "k_measure", "k_mcs"]
-    dom = int(np.argmax(kms))
-    if dom not in (0, 4):          # the roofline is quoted for the kernel that does the Metropolis sweeps
-        dom = 4 if kn[4] > 0 else 0
-    mcs_per_launch = 1 if dom == 0 else max(1, (a.mcs_per_step * a.steps) // max(int(kn[4]), 1))
-    dom_ms = kms[dom] / max(int(kn[dom]), 1)
-    flips_per_launch = w.flips_per_sweep() * mcs_per_launch
-    dom_flips_ns = flips_per_launch / (dom_ms * 1e6) if dom_ms > 0 else 0.0
-    A = ALGO_OPS_PER_FLIP[w.d]
-    peak_ops = SM_COUNT * INT32_LANES_PER_SM_CLK * (peaks.get("sm_max_mhz", 1965.0) / 1e3)
+    peaks, _ = measured_peaks()
+    roofline["clock_ghz_during_run"] = (t["clocks"]["sm_mhz"] or peaks.get("sm_max_mhz", 1965.0)) / 1e3 if t["clocks"] else None
     philox_ops, _ = B.pt_microbench(4, 8, 1000, device=dev)     # measured live: Philox-only ceiling
-    roofline = {
-        "bound": "alu", "kernel": names[dom], "achieved": A * dom_flips_ns, "peak": peak_ops,
-        "unit": "Gop/s (INT32 thread-ops)", "frac": A * dom_flips_ns / peak_ops,
-        "traffic": None if a.gaussian else NCU_DRAM_BYTES_PER_LAUNCH.get((w.name, names[dom])),
-        "peak_how": "derived: 148 SMs x 128 INT32 lanes/clk (fma+alu pipes) x %.3f GHz max SM clock; A = %d algorithmic "
-                    "ops/flip (Philox 10 + field 2d + decide 6); a %s launch = %d MCS = %d attempted flips" % (
-                        peaks.get("sm_max_mhz", 1965.0) / 1e3, A, names[dom], mcs_per_launch, flips_per_launch),
-        "flips_per_ns": dom_flips_ns, "ms_per_launch": dom_ms, "launches": int(kn[dom]),
-        "philox_only_flips_per_ns": philox_ops / 10.0,
-        "hbm": {"algorithmic_bytes_per_flip": 0.25 / mcs_per_launch, "achieved_gbs": 0.25 / mcs_per_launch * dom_flips_ns,
-                "peak_gbs": peaks.get("hbm_gbs"), "peak_kind": peaks_kind,
-                "frac": 0.25 / mcs_per_launch * dom_flips_ns / peaks.get("hbm_gbs", 6650.0)},
-        "kernel_ms": {n: float(kms[i]) for i, n in enumerate(names)}, "step_total_ms": ms_total,
-        "clock_ghz_during_run": f_ghz,
-    }
-    # the Metropolis sweeps alone (a1-a3; Eq. (11) normalisation), same state, after the timed region
-    B.pt_set_profiling(True)
-    for _ in range(5):
-        B.pt_sweep(a.mcs_per_step)
-    sms, sn = B.pt_get_kernel_times()
-    B.pt_set_profiling(False)
-    so = w.flips_per_sweep() * a.mcs_per_step / (sms[0] / max(int(sn[0]), 1) * 1e6)
-    roofline["sweep_only"] = {"kernel": "k_sweep", "flips_per_ns": so, "frac": A * so / peak_ops,
-                              "what": "pt_sweep(%d) launches, no Houdayer / exchange" % a.mcs_per_step}
-    assert B.pt_recompute_energy()[1] == 0
-    # the two measurement kernels alone (a6 and the NEXT-2 overlap profile), CUDA events around 20 calls each
-    prof_d = torch.empty((w.S, w.T, w.d, w.L), dtype=torch.int32, device=dev)
-    meas_us = {}
-    for label, fn in (("overlap", lambda: B.pt_measure_overlap_device(Qrec[0], QLrec[0])),
-                      ("overlap_profile", lambda: B.pt_measure_overlap_profile_device(prof_d))):
-        for _ in range(3):
-            fn()
-        torch.cuda.synchronize()
-        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        m0.record()
-        for _ in range(20):
-            fn()
-        m1.record()
-        torch.cuda.synchronize()
-        meas_us[label] = m0.elapsed_time(m1) / 20 * 1e3
-    roofline["measurement_us_per_call"] = meas_us
+    roofline["philox_only_flips_per_ns"] = philox_ops / 10.0
+    roofline["measurement_us_per_call"] = run.measurement_kernels()
+    fast_path = bool(B.pt_get_path())
+
+    # ---- the other configs, same run, same protocol with fewer steps (N = 1 only: they are not part of the scaling line)
+    per_config = None
+    if not a.no_per_config and world == 1:
+        per_config = {w.name: {"value": t["value"], "ms_per_step": t["ms_per_step"], "steps": t["steps"],
+                               "frac": roofline["frac"], "whole_mcs_frac": roofline["whole_mcs_frac"], "headline": True}}
+        for name in sorted(wl.CONFIGS):
+            if name == w.name:
+                continue
+            wc = wl.CONFIGS[name]
+            rc = GpuRun(a, wc, rank, world, dev, flush)
+            tc = rc.timed(a.config_steps, a.warmup, sampler)
+            rf = rc.instrumented(min(a.config_steps, 5), tc)
+            per_config[name] = {
+                "workload": config_of(a, wc, world)["workload"], "value": tc["value"], "unit": UNIT,
+                "ms_per_step": tc["ms_per_step"], "steps": tc["steps"], "mcs_per_step": a.mcs_per_step,
+                "gpu_launches": tc["gpu_launches"], "clocks": tc["clocks"],
+                "roofline": {k: rf[k] for k in ("kernel", "frac", "whole_mcs_frac", "flips_per_ns", "ms_per_launch", "sweep_only",
+                                                "kernel_ms", "kernel_launches", "kernel_ms_pass", "phases", "traffic", "traffic_source")},
+            }
+    if sampler:
+        sampler.stop()
 
     cpu = None
     if not a.no_cpu_baseline:
-        S_cpu, mcs_cpu = 4, max(1, int(3.0e8 / (w.flips_per_sweep(4))))
-        v, dt, flips = oracle_time(w, S_cpu, mcs_cpu, gaussian=a.gaussian, cluster=a.cluster)
-        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
-               "sample": "%s restricted to the first %d samples x %d MCS (%.2e flips), same MCS order" % (w.name, S_cpu, mcs_cpu, flips)}
+        from oracle import pool as OP
+
+        P = OP.n_cores()
+        v1, dt1, flips1, mcs1 = oracle_rate(a, w, 1, 1, 2.5e8)
+        vP, dtP, flipsP, mcsP = oracle_rate(a, w, P, 1, 2.5e8)
+        cpu = {"value": vP, "unit": UNIT, "cores": P, "kind": "oracle", "seconds": dtP, "cpu": cpu_model(),
+               "sample": "%s restricted to %d samples (one single-threaded oracle process per host core on disjoint sample_offset "
+                         "ranges, PAPER.md:241) x %d MCS (%.2e flips), same MCS order" % (w.name, P, mcsP, flipsP),
+               "one_core": {"value": v1, "unit": UNIT, "cores": 1, "seconds": dt1,
+                            "sample": "%s restricted to the first sample x %d MCS (%.2e flips)" % (w.name, mcs1, flips1)}}
 
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
-        "ms_per_step": ms_total / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": t["value"], "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+        "ms_per_step": t["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "int32", "data": "synthetic", "config": config_of(a, w, world),
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
-        "fast_path": bool(B.pt_get_path()),
+        "clocks": t["clocks"], "e2e": e2e, "gpu_launches": t["gpu_launches"], "roofline": roofline, "cpu_baseline": cpu,
+        "per_config": per_config, "fast_path": fast_path,
     }
     print(json.dumps(out))
     if world > 1:

@@ -218,6 +218,22 @@ int pt_get_launch_count(uint64_t *n_launches);     /* kernels launched by this l
  * pt_get_kernel_times synchronises and returns the summed milliseconds and launch counts since then. */
 int pt_set_profiling(int on);
 int pt_get_kernel_times(double ms[5], uint64_t launches[5]);
+/* Where pt_mcs runs the three separate kernels per MCS (a sample does not fit a CTA's shared memory: BASELINE config 5),
+ * the samples are cut into n groups, each issuing its sweep -> cluster -> exchange chain on its own stream (group 0 on the
+ * bound stream, the others on library-owned side streams that fork from and join the bound stream inside the call), so
+ * that the low-occupancy tail of one group's cluster kernel and its latency-bound exchange kernel overlap another group's
+ * sweep.  Samples never interact (P:7), so results are bit-identical for every n.  n = -1: automatic (up to 3 groups while
+ * each group still fills the GPU twice over); n = 1: one stream (used for per-kernel timing). */
+int pt_set_sample_groups(int n);
+/* Phase split of the FUSED launch (pt_mcs where one CTA keeps a sample resident): CUDA events cannot separate the
+ * Metropolis sweeps, the Houdayer moves and the PT pass inside one kernel, so when on, thread 0 of every CTA sums the SM
+ * clocks it spends in each phase (a clock64() read after the CTA barrier that ends the phase) and adds them to four
+ * device counters at the end of the launch: clocks[0] sweeps, [1] Houdayer, [2] PT pass, [3] the rest (load / store of
+ * the state, overlap records).  clocks[k] / sum = the share of the launch time a CTA spends in phase k, which gives the
+ * per-spin update times of Eq. (11) P:189 for the cluster move and the PT pass on the fused path.
+ * pt_set_phase_clocks zeroes the counters; off by default (the timed bench region runs without it). */
+int pt_set_phase_clocks(int on);
+int pt_get_phase_clocks(uint64_t clocks[4]);
 /* Which code path the bound problem uses: 1 = word-parallel kernels specialised for L a power of two >= 8,
  * 0 = general-L kernels.  force = -1 leaves the choice to the library, 0 forces the general path (tests). */
 int pt_get_path(int *fast);

@@ -3,9 +3,11 @@
 Every sample is a pure function of (seed, global sample index) (pin P8), so a run of S samples is the
 concatenation of runs over any partition of [0, S) through `sample_offset` -- the paper's own way of using a multi-core
 host ("24 disorder realizations in parallel", PAPER.md:241).  The oracle itself stays single-threaded and untouched;
-this module only starts processes and concatenates what they return.  TEST INFRASTRUCTURE ONLY (it imports oracle/).
+this module only starts processes and concatenates what they return.  TEST INFRASTRUCTURE ONLY, like the rest of
+oracle/: tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import it, the product
+never does.  It holds none of the method's arithmetic.
 
-Worker processes are *spawned* (not forked): the parent holds a CUDA context in the GPU tests.
+Worker processes are *spawned* (not forked): the parent holds a CUDA context in the GPU tests and in bench.py.
 """
 from __future__ import annotations
 
@@ -82,3 +84,66 @@ def gather(futures, n_mcs):
     recs = [(np.concatenate([p[3][r][0] for p in parts], axis=0), np.concatenate([p[3][r][1] for p in parts], axis=0))
             for r in range(n_rec)]
     return out, recs
+
+
+# ---- persistent workers: P oracle processes that each keep one simulation alive and advance it on request (bench.py) ----
+
+def _persistent_worker(conn, job):
+    from oracle import ref
+
+    (L, d, T, betas, seed, g0, n, houdayer, measure_every, fixed, n_clu) = job
+    o = ref.Oracle(L, d, n, T, np.asarray(betas, dtype=np.float64), seed, g0)
+    if fixed is not None:
+        o.set_couplings_fixed(fixed[0], fixed[1])
+    if n_clu is not None:
+        o.set_cluster_moves(np.asarray(n_clu, dtype=np.int32))
+    conn.send("ready")
+    done = 0
+    while True:
+        msg = conn.recv()
+        if msg is None:
+            break
+        for _ in range(int(msg)):                   # one MCS at a time, the measurement where the config asks for it (R26)
+            o.mcs(1, 1, int(houdayer), True)
+            done += 1
+            if measure_every and done % measure_every == 0:
+                o.measure_overlap()
+        conn.send(done)
+    o.close()
+    conn.close()
+
+
+class PersistentOracles:
+    """P oracle processes on disjoint sample ranges [g0 + k n, g0 + (k + 1) n), each alive across step() calls."""
+
+    def __init__(self, w, procs, samples_per_proc, houdayer_mode=None, fixed=None, n_clu=None, seed=None, g0=0):
+        from paper_2003_04621_b200 import workloads as wl
+
+        ctx = mp.get_context("spawn")
+        self.procs, self.conns = [], []
+        hd = (1 if w.houdayer else 0) if houdayer_mode is None else houdayer_mode
+        for k in range(procs):
+            a, b = ctx.Pipe()
+            fx = None if fixed is None else (fixed[0][k * samples_per_proc:(k + 1) * samples_per_proc], fixed[1])
+            job = (w.L, w.d, w.T, w.betas().tolist(), wl.SEED if seed is None else seed, g0 + k * samples_per_proc,
+                   samples_per_proc, hd, int(w.measure_every), fx, n_clu)
+            p = ctx.Process(target=_persistent_worker, args=(b, job), daemon=True)
+            p.start()
+            self.procs.append(p)
+            self.conns.append(a)
+        for c in self.conns:
+            assert c.recv() == "ready"
+
+    def step(self, n_mcs):
+        for c in self.conns:
+            c.send(int(n_mcs))
+        return [c.recv() for c in self.conns]
+
+    def close(self):
+        for c in self.conns:
+            try:
+                c.send(None)
+            except Exception:
+                pass
+        for p in self.procs:
+            p.join(timeout=5)

@@ -62,6 +62,9 @@ SYMBOLS = {
     "pt_get_launch_count": (_i, [_vp]),
     "pt_set_profiling": (_i, [_i]),
     "pt_get_kernel_times": (_i, [_vp, _vp]),
+    "pt_set_sample_groups": (_i, [_i]),
+    "pt_set_phase_clocks": (_i, [_i]),
+    "pt_get_phase_clocks": (_i, [_vp]),
     "pt_get_path": (_i, [_vp]),
     "pt_force_general_path": (_i, [_i]),
     "pt_philox_selftest": (_i, [_vp, _vp, _vp, _i]),
@@ -380,6 +383,21 @@ def pt_get_kernel_times():
     n = np.zeros(5, dtype=np.uint64)
     _ck(lib().pt_get_kernel_times(_p(ms), _p(n)))
     return ms, n
+
+
+def pt_set_sample_groups(n):
+    _ck(lib().pt_set_sample_groups(int(n)))
+
+
+def pt_set_phase_clocks(on):
+    _ck(lib().pt_set_phase_clocks(int(on)))
+
+
+def pt_get_phase_clocks():
+    """SM clocks summed over the CTAs of the fused launches since pt_set_phase_clocks: sweeps, Houdayer, PT pass, rest."""
+    c = np.zeros(4, dtype=np.uint64)
+    _ck(lib().pt_get_phase_clocks(_p(c)))
+    return c
 
 
 def pt_get_path() -> int:

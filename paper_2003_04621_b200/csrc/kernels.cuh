@@ -41,6 +41,7 @@ struct DevPtrs {
     // cluster-move variants (NEXT-4, R36): single-cluster moves per houdayer_step at temperature index t
     int32_t *nclu;              // [T]
     int32_t *tcold;             // [T] temperature indices by descending beta: the pairs with the largest clusters first
+    unsigned long long *phaseClk;   // [4] SM clocks summed over the CTAs of k_mcs: sweeps | Houdayer | PT pass | rest (pt_set_phase_clocks)
 };
 
 struct Params {

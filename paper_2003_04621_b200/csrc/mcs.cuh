@@ -20,13 +20,14 @@ struct McsArgs {
     uint32_t sweep0, houd0, exch0;          // counter values at the start of the call
     int measure_every;                      // > 0: overlap record after every measure_every-th MCS of the call (whole-sample CTAs only)
     int32_t *recQ, *recQL;                  // device records [n_mcs / measure_every][S][T]; recQL may be null
+    int phase_clocks;                       // 1: thread 0 of every CTA sums clock64() per phase into P.d.phaseClk (Eq. (11) split of the fused launch)
 };
 
 // shared-memory carve-up, shared by host (size) and device (pointers); all offsets in 32-bit words.
 // A replica occupies RS = 2W + 1 words (colour 0 | colour 1 | pad): the odd stride lets 32 lanes that each own a
 // different replica (lane-per-pair Houdayer) hit 32 different banks.
 struct McsSmem {
-    int RS, oJ, oS, oE, oTos, oSot, oThr, oAcc, oLast, oCum, oU, oSgn, oC2, oPair, oTot, oMeas, oScr, words;
+    int RS, oJ, oS, oE, oTos, oSot, oThr, oAcc, oLast, oCum, oU, oSgn, oC2, oPair, oTot, oMeas, oScr, oPh, words;
     // nch: chains held by the CTA (2 = the whole sample, 1 = one chain)
     // extras: the arrays only the fixed-point (GAUSS) and fused-measurement (MEAS) variants use, placed after the scratch so
     // that the plain +-J kernel keeps its layout
@@ -47,6 +48,8 @@ struct McsSmem {
         oCum = o;  o += 2 * T;              // 64-bit
         oU = o;    o += 2 * T;              // PT draws of the current pass, [chain][pair]
         oSgn = o;  o += T;
+        o = (o + 1) & ~1;
+        oPh = o;   o += 10;                 // 64-bit: last time stamp | clocks in sweeps, Houdayer, PT pass, rest
         oScr = o;
         if (nch < 2) {
             // no Houdayer phase, no scratch
@@ -103,6 +106,15 @@ __device__ __noinline__ void mcs_overlap_record(LAT lat, const Params &P, const 
     }
 }
 
+// Phase clocks (Eq. (11) P:189 asks for the time per spin of each update; inside ONE fused launch CUDA events cannot
+// separate them): thread 0 adds the SM clocks since the last stamp to phase `k`.  Called right after a CTA barrier.
+__device__ __forceinline__ void phase_stamp(unsigned long long *sPh, int k)
+{
+    const unsigned long long now = (unsigned long long)clock64();
+    sPh[1 + k] += now - sPh[0];
+    sPh[0] = now;
+}
+
 // GAUSS: 0 = +-J bit couplings; 1 / 2 = fixed-point couplings (gauss.cuh) with / without the host's range guarantee
 // 2 D max|Jq| < 2^23.  With fixed-point couplings the sweep walks its word site by site (update_word_q), the energies are
 // recomputed from scratch after the cluster moves (field_sum_word_q; the cluster itself depends on q only) and the PT walk
@@ -125,6 +137,9 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
     int *sPair = (int *)(msm + L.oPair), *sTot = (int *)(msm + L.oTot);
     int *sE = (int *)(msm + L.oE), *sTos = (int *)(msm + L.oTos), *sSot = (int *)(msm + L.oSot), *sSgn = (int *)(msm + L.oSgn);
     unsigned long long *sCum = (unsigned long long *)(msm + L.oCum);
+    unsigned long long *sPh = (unsigned long long *)(msm + L.oPh);
+    const bool clk = a.phase_clocks && threadIdx.x == 0;
+    if (clk) { sPh[0] = (unsigned long long)clock64(); sPh[1] = sPh[2] = sPh[3] = sPh[4] = 0ull; }
     const int s = a.split_chains ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
     const int c0 = a.split_chains ? (int)(blockIdx.x & 1) : 0;      // first chain of this CTA
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -162,6 +177,7 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
     }
     __syncthreads();
 
+    if (clk) phase_stamp(sPh, 3);
     for (int m = 0; m < a.n_mcs; ++m) {
         // ---- a1-a3: n_metro checkerboard sweeps
         for (int it = 0; it < a.n_metro; ++it) {
@@ -188,6 +204,7 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                 __syncthreads();
             }
         }
+        if (clk) phase_stamp(sPh, 0);
         // ---- a5: Houdayer exchange
         if (a.do_houdayer && NCH == 2) {
             const uint32_t step = a.houd0 + (uint32_t)m;
@@ -267,6 +284,7 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                 __syncthreads();
             }
         }
+        if (clk) phase_stamp(sPh, 1);
         // ---- a4: PT pass (R9: sequential walk, each step seeing the previous).  Warp 0: all lanes draw the Philox
         // words, then one lane per chain walks its ladder; only the two index maps change.
         if (a.do_exchange && T > 1) {
@@ -323,12 +341,14 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
             }
             __syncthreads();
         }
+        if (clk) phase_stamp(sPh, 2);
         // ---- a6: overlap record (Eq. (4), link overlap R14) of the pairs now at equal temperature, from the resident
         // state: what pt_measure_overlap would return after this MCS.  gather() is a bit permutation, so the neighbour
         // bits of q = A ^ B are gather(A) ^ gather(B).
         if constexpr (MEAS)
             if (a.measure_every > 0 && NCH == 2 && (m + 1) % a.measure_every == 0)
                 mcs_overlap_record<LAT, NT>(lat, P, sS, sSot, (int *)(msm + L.oMeas), s, (size_t)((m + 1) / a.measure_every - 1), a.recQ, a.recQL);
+        if (clk) phase_stamp(sPh, 3);
     }
 
     for (int i = tid; i < R * 2 * W; i += NT) {
@@ -350,6 +370,10 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
             P.d.last[(size_t)s * T + i] = sLast[i];
             P.d.cum[(size_t)s * T + i] += sCum[i];
         }
+    if (clk) {
+        phase_stamp(sPh, 3);
+        for (int k = 0; k < 4; ++k) atomicAdd(P.d.phaseClk + k, sPh[1 + k]);
+    }
 }
 
 }  // namespace ptg

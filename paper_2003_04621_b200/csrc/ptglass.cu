@@ -38,6 +38,8 @@ struct Context {
     uint64_t n_passes = 0;      // PT passes since pt_init = swap attempts per pair (R20); NOT the Philox step counter
                                 // n_exchange, which pt_set_counters overwrites on a resume
     bool q_small = false;       // fixed-point couplings with 2 D max|Jq| < 2^23 (gauss.cuh: accept_site<SMALL>)
+    int sample_groups = -1;     // pt_set_sample_groups: -1 = automatic
+    int phase_clocks = 0;       // pt_set_phase_clocks
     int max_clu = 1;            // max over t of the per-temperature cluster-move counts (NEXT-4, R36)
     uint64_t launches = 0;
     size_t stage_bytes = 0;
@@ -81,16 +83,17 @@ Profiler PROF;
 
 struct ProfScope {
     int cls;
+    cudaStream_t st;
     cudaEvent_t a = nullptr;
-    explicit ProfScope(int c) : cls(c)
+    explicit ProfScope(int c, cudaStream_t stream = nullptr) : cls(c), st(stream ? stream : G.stream)
     {
-        if (PROF.on) { a = PROF.get(); cudaEventRecord(a, G.stream); }
+        if (PROF.on) { a = PROF.get(); cudaEventRecord(a, st); }
     }
     ~ProfScope()
     {
         if (a) {
             cudaEvent_t b = PROF.get();
-            cudaEventRecord(b, G.stream);
+            cudaEventRecord(b, st);
             PROF.pending.push_back({cls, a, b});
         }
     }
@@ -210,6 +213,7 @@ size_t carve(void *base, int L, int d, int S, int T, uint32_t strideX, DevPtrs *
     p.rtCnt = c.take<unsigned long long>(base, (size_t)S * 2 * 32);
     p.nclu = c.take<int32_t>(base, (size_t)T);
     p.tcold = c.take<int32_t>(base, (size_t)T);
+    p.phaseClk = c.take<unsigned long long>(base, 4);
     const size_t sb = std::max(R * N, (size_t)S * d * N);
     p.stage = c.take<int8_t>(base, sb);
     if (out) *out = p;
@@ -267,14 +271,18 @@ template <class K> cudaError_t allow_smem(K kernel, size_t bytes)
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
-cudaError_t launch_energy(int mode)
+// Every launch function takes the problem it works on -- the whole bound problem G.P, or a VIEW of a contiguous range of
+// its samples (sub_view) -- and the stream it is issued on: the separate-kernel path of pt_mcs runs sample groups on
+// side streams so that one group's cluster and exchange kernels fill the SMs another group's sweep leaves idle.
+cudaError_t launch_energy(int mode, const Params &P = G.P, cudaStream_t st = nullptr)
 {
+    if (!st) st = G.stream;
     cudaError_t err = cudaSuccess;
     with_lattice([&](auto lat) {
-        const long reps = (long)G.P.S * 2 * G.P.T;
+        const long reps = (long)P.S * 2 * P.T;
         const int wpb = 4;
-        if (G.P.gauss) k_energy_q<<<(unsigned)((reps + wpb - 1) / wpb), wpb * 32, 0, G.stream>>>(lat, G.P, mode);
-        else k_energy<<<(unsigned)((reps + wpb - 1) / wpb), wpb * 32, 0, G.stream>>>(lat, G.P, mode);
+        if (P.gauss) k_energy_q<<<(unsigned)((reps + wpb - 1) / wpb), wpb * 32, 0, st>>>(lat, P, mode);
+        else k_energy<<<(unsigned)((reps + wpb - 1) / wpb), wpb * 32, 0, st>>>(lat, P, mode);
         ++G.launches;
         err = cudaGetLastError();
     });
@@ -290,21 +298,22 @@ int sweep_group(int T, int W)
     return best;
 }
 
-cudaError_t launch_sweep(int n)
+cudaError_t launch_sweep(int n, uint32_t step0, const Params &P = G.P, cudaStream_t st = nullptr)
 {
-    ProfScope prof(0);
+    if (!st) st = G.stream;
+    ProfScope prof(0, st);
     cudaError_t err = cudaSuccess;
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
-        const int W = G.P.W, D = G.P.D;
-        const int R = sweep_group(G.P.T, W);
-        if (G.P.gauss) {
+        const int W = P.W, D = P.D;
+        const int R = sweep_group(P.T, W);
+        if (P.gauss) {
             const size_t smq = ((size_t)R * 2 * W + 3 * (size_t)R) * 4;
             auto kq = G.q_small ? k_sweep_q<LAT, true> : k_sweep_q<LAT, false>;
             err = allow_smem(kq, smq);
             if (err != cudaSuccess) return;
-            dim3 gq((unsigned)(2 * G.P.T / R), (unsigned)G.P.S);
-            kq<<<gq, 128, smq, G.stream>>>(lat, G.P, R, G.n_sweep, n);
+            dim3 gq((unsigned)(2 * P.T / R), (unsigned)P.S);
+            kq<<<gq, 128, smq, st>>>(lat, P, R, step0, n);
             ++G.launches;
             err = cudaGetLastError();
             return;
@@ -312,37 +321,38 @@ cudaError_t launch_sweep(int n)
         const size_t smem = ((size_t)2 * 2 * D * W + (size_t)R * 2 * W + (size_t)R * 4 + (size_t)R) * 4;
         err = allow_smem(k_sweep<LAT>, smem);
         if (err != cudaSuccess) return;
-        dim3 grid((unsigned)(2 * G.P.T / R), (unsigned)G.P.S);
-        k_sweep<LAT><<<grid, 128, smem, G.stream>>>(lat, G.P, R, G.n_sweep, n);
+        dim3 grid((unsigned)(2 * P.T / R), (unsigned)P.S);
+        k_sweep<LAT><<<grid, 128, smem, st>>>(lat, P, R, step0, n);
         ++G.launches;
         err = cudaGetLastError();
     });
     return err;
 }
 
-cudaError_t launch_exchange()
+cudaError_t launch_exchange(uint32_t step, const Params &P = G.P, cudaStream_t st = nullptr)
 {
-    ProfScope prof(2);
-    const int T = G.P.T;
-    const long chains = (long)G.P.S * 2;
+    if (!st) st = G.stream;
+    ProfScope prof(2, st);
+    const int T = P.T;
+    const long chains = (long)P.S * 2;
     int wpb = 4;
     while (wpb > 1 && (size_t)wpb * 4 * T * 4 > 64 * 1024) wpb >>= 1;
     const size_t smem = (size_t)wpb * 4 * T * 4 + (T <= kExchangeTableT ? (size_t)wpb * T * T : 0);      // + the decision table
     if ((size_t)wpb * 4 * T * 4 > 64 * 1024) {      // very long ladders: walk on global scratch instead of shared memory
-        k_exchange<true><<<(unsigned)chains, 32, 0, G.stream>>>(G.P, G.n_exchange);
+        k_exchange<true><<<(unsigned)chains, 32, 0, st>>>(P, step);
     } else {
         cudaError_t err = allow_smem(k_exchange<false>, smem);
         if (err != cudaSuccess) return err;
-        k_exchange<false><<<(unsigned)((chains + wpb - 1) / wpb), wpb * 32, smem, G.stream>>>(G.P, G.n_exchange);
+        k_exchange<false><<<(unsigned)((chains + wpb - 1) / wpb), wpb * 32, smem, st>>>(P, step);
     }
     ++G.launches;
     return cudaGetLastError();
 }
 
 // One launch per move number (R36): move j touches the temperatures with nclu[t] > j; a default run makes one launch.
-cudaError_t launch_houdayer()
+cudaError_t launch_houdayer(uint32_t step, const Params &P, cudaStream_t st)
 {
-    ProfScope prof(1);
+    ProfScope prof(1, st);
     cudaError_t err = cudaSuccess;
     for (uint32_t move = 0; move < (uint32_t)std::max(G.max_clu, 1) && err == cudaSuccess; ++move)
     with_lattice([&](auto lat) {
@@ -354,15 +364,15 @@ cudaError_t launch_houdayer()
             const size_t smem = (size_t)wpb * kPairScratchWords<LAT> * 4;
             err = allow_smem(k_houdayer<LAT>, smem);
             if (err != cudaSuccess) return;
-            const long pairs = (long)G.P.S * G.P.T;
-            k_houdayer<LAT><<<(unsigned)((pairs + wpb - 1) / wpb), wpb * 32, smem, G.stream>>>(lat, G.P, G.n_houdayer, move);
+            const long pairs = (long)P.S * P.T;
+            k_houdayer<LAT><<<(unsigned)((pairs + wpb - 1) / wpb), wpb * 32, smem, st>>>(lat, P, step, move);
         } else {
             const int threads = 128;
-            const size_t smem = ((size_t)4 * G.P.W + 2 * (threads / 32) + 2) * 4;
+            const size_t smem = ((size_t)4 * P.W + 2 * (threads / 32) + 2) * 4;
             err = allow_smem(k_houdayer_gen<LAT>, smem);
             if (err != cudaSuccess) return;
-            dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
-            k_houdayer_gen<LAT><<<grid, threads, smem, G.stream>>>(lat, G.P, G.n_houdayer, move);
+            dim3 grid((unsigned)P.T, (unsigned)P.S);
+            k_houdayer_gen<LAT><<<grid, threads, smem, st>>>(lat, P, step, move);
         }
         ++G.launches;
         err = cudaGetLastError();
@@ -383,9 +393,9 @@ int multi_threads()
 
 size_t multi_smem_bytes(int threads) { return ((size_t)4 * G.P.W + 2 * (threads / 32) + 2 + (size_t)G.P.N) * 4 + (size_t)G.P.N * 2 + 16; }
 
-cudaError_t launch_houdayer_multi()
+cudaError_t launch_houdayer_multi(uint32_t step, const Params &P, cudaStream_t st)
 {
-    ProfScope prof(1);
+    ProfScope prof(1, st);
     cudaError_t err = cudaSuccess;
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
@@ -393,8 +403,8 @@ cudaError_t launch_houdayer_multi()
         const size_t smem = multi_smem_bytes(threads);
         err = allow_smem(k_houdayer_multi<LAT>, smem);
         if (err != cudaSuccess) return;
-        dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
-        k_houdayer_multi<LAT><<<grid, threads, smem, G.stream>>>(lat, G.P, G.n_houdayer);
+        dim3 grid((unsigned)P.T, (unsigned)P.S);
+        k_houdayer_multi<LAT><<<grid, threads, smem, st>>>(lat, P, step);
         ++G.launches;
         err = cudaGetLastError();
     });
@@ -402,11 +412,59 @@ cudaError_t launch_houdayer_multi()
 }
 
 // mode 1: single-cluster moves (R36 counts), mode 2: multi-cluster (R37)
-cudaError_t launch_houdayer_any(int mode = 1)
+cudaError_t launch_houdayer_any(int mode, uint32_t step, const Params &P = G.P, cudaStream_t st = nullptr)
 {
-    cudaError_t err = (mode == 2) ? launch_houdayer_multi() : launch_houdayer();
-    if (err == cudaSuccess && G.P.gauss) err = launch_energy(0);
+    if (!st) st = G.stream;
+    cudaError_t err = (mode == 2) ? launch_houdayer_multi(step, P, st) : launch_houdayer(step, P, st);
+    if (err == cudaSuccess && P.gauss) err = launch_energy(0, P, st);
     return err;
+}
+
+// The problem restricted to samples [s0, s0 + n): every per-sample array advanced, the global sample index with it.
+Params sub_view(const Params &P, int s0, int n)
+{
+    Params V = P;
+    const size_t s = (size_t)s0, R = s * 2 * P.T;
+    V.S = n;
+    V.g0 = P.g0 + (uint32_t)s0;
+    V.d.spin += R * 2 * P.W;
+    V.d.Jn += s * 2 * 2 * P.D * P.W;
+    V.d.E += R; V.d.tos += R; V.d.sot += R; V.d.outE += R;
+    V.d.accepts += s * 2 * (size_t)(P.T - 1);
+    V.d.last += s * P.T; V.d.cum += s * P.T; V.d.outQ += s * P.T; V.d.outQL += s * P.T;
+    V.d.outProf += s * P.T * P.D * P.L;
+    V.d.JqNat += s * P.D * P.N;
+    V.d.Jdev += s * 2 * 2 * P.D * 32 * P.W;
+    V.d.rtLabel += R; V.d.rtStart += R; V.d.rtTrips += R;
+    V.d.rtSum += s * 2 * 32; V.d.rtCnt += s * 2 * 32;
+    return V;
+}
+
+// Side streams of the separate-kernel MCS loop (created on first use, never destroyed before process exit) and the
+// events that fork them from / join them to the caller's stream.
+constexpr int kMaxGroups = 8;
+cudaStream_t g_side[kMaxGroups] = {};
+cudaEvent_t g_fork = nullptr, g_join[kMaxGroups] = {};
+
+cudaError_t ensure_side_streams(int n)
+{
+    cudaError_t e = cudaSuccess;
+    if (!g_fork) e = cudaEventCreateWithFlags(&g_fork, cudaEventDisableTiming);
+    for (int k = 1; k < n && e == cudaSuccess; ++k) {
+        if (!g_side[k]) e = cudaStreamCreateWithFlags(&g_side[k], cudaStreamNonBlocking);
+        if (e == cudaSuccess && !g_join[k]) e = cudaEventCreateWithFlags(&g_join[k], cudaEventDisableTiming);
+    }
+    return e;
+}
+
+// sample groups of a separate-kernel pt_mcs call.  Automatic: one group per wave of sweep CTAs (148 SMs x 7 CTAs), at most
+// kMaxGroups -- measured on C5 (5.9 waves): 1 group 733, 2: 811, 4: 852, 6: 862, 8: 862 flips/ns.
+int mcs_groups()
+{
+    if (G.sample_groups > 0) return std::min(std::min(G.sample_groups, kMaxGroups), G.P.S);
+    const long ctas = (long)G.P.S * (2 * G.P.T / sweep_group(G.P.T, G.P.W));     // sweep CTAs of the whole problem
+    const long waves = (ctas + 148L * 7 - 1) / (148L * 7);
+    return (int)std::max(1L, std::min<long>(std::min<long>(waves, kMaxGroups), G.P.S));
 }
 
 cudaError_t launch_measure(int32_t *Q, int32_t *QL)
@@ -646,7 +704,7 @@ int pt_sweep(int n)
     if (n < 0) return fail(PT_ERR_ARG, "pt_sweep: n must be >= 0");
     if ((uint64_t)G.n_sweep + (uint64_t)n > 4294967295ull) return fail(PT_ERR_OVERFLOW, "sweep counter would overflow");
     if (n == 0) return PT_OK;
-    CK(launch_sweep(n));
+    CK(launch_sweep(n, G.n_sweep));
     G.n_sweep += (uint32_t)n;
     return PT_OK;
 }
@@ -655,7 +713,7 @@ int pt_exchange(void)
 {
     NEED_INIT();
     if (G.n_exchange == 4294967295u) return fail(PT_ERR_OVERFLOW, "exchange counter would overflow");
-    CK(launch_exchange());
+    CK(launch_exchange(G.n_exchange));
     G.n_exchange += 1;
     G.n_passes += 1;
     return PT_OK;
@@ -665,7 +723,7 @@ int houdayer_step(void)
 {
     NEED_INIT();
     if (G.n_houdayer == 4294967295u) return fail(PT_ERR_OVERFLOW, "Houdayer counter would overflow");
-    CK(launch_houdayer_any());
+    CK(launch_houdayer_any(1, G.n_houdayer));
     G.n_houdayer += 1;
     return PT_OK;
 }
@@ -676,7 +734,7 @@ int houdayer_multi_step(void)
     if (G.n_houdayer == 4294967295u) return fail(PT_ERR_OVERFLOW, "Houdayer counter would overflow");
     if (multi_smem_bytes(multi_threads()) > 227 * 1024)
         return fail(PT_ERR_ARG, "houdayer_multi_step: %d sites of labels do not fit in shared memory", G.P.N);
-    CK(launch_houdayer_any(2));
+    CK(launch_houdayer_any(2, G.n_houdayer));
     G.n_houdayer += 1;
     return PT_OK;
 }
@@ -715,18 +773,43 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
     if (n_mcs == 0 || (n_metro == 0 && !do_houdayer && !do_exchange)) return PT_OK;
     if (do_houdayer != 2 && mcs_fused_eligible(nullptr, do_houdayer)) {
         const McsArgs a{n_mcs, n_metro, do_houdayer ? 1 : 0, do_exchange ? 1 : 0, mcs_split_chains(do_houdayer) ? 1 : 0,
-                        G.max_clu, G.n_sweep, G.n_houdayer, G.n_exchange, 0, nullptr, nullptr};
+                        G.max_clu, G.n_sweep, G.n_houdayer, G.n_exchange, 0, nullptr, nullptr, G.phase_clocks};
         CK(launch_mcs(a));
         G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
         if (do_houdayer) G.n_houdayer += (uint32_t)M;
         if (do_exchange) { G.n_exchange += (uint32_t)M; G.n_passes += M; }
         return PT_OK;
     }
-    for (int m = 0; m < n_mcs; ++m) {
-        if (n_metro > 0) { CK(launch_sweep(n_metro)); G.n_sweep += (uint32_t)n_metro; }
-        if (do_houdayer) { CK(launch_houdayer_any(do_houdayer)); G.n_houdayer += 1; }
-        if (do_exchange) { CK(launch_exchange()); G.n_exchange += 1; G.n_passes += 1; }
+    // Separate kernels.  Samples never interact (P:7), so the problem is cut into groups of samples, each
+    // running its own sweep -> cluster -> exchange chain on its own stream: while one group's cluster kernel drains (a few
+    // long pairs, low occupancy) or its exchange kernel walks its ladders (latency-bound, a handful of warps), another
+    // group's sweep fills the SMs.  Group 0 runs on the caller's stream; the side streams start after everything queued
+    // on it so far and it waits for them before the call returns.  Results do not depend on the grouping (pin P8).
+    const int NG = mcs_groups();
+    std::vector<Params> view((size_t)NG);
+    std::vector<cudaStream_t> st((size_t)NG, G.stream);
+    for (int g = 0; g < NG; ++g) {
+        const int a0 = (int)((long)G.P.S * g / NG), a1 = (int)((long)G.P.S * (g + 1) / NG);
+        view[g] = sub_view(G.P, a0, a1 - a0);
     }
+    if (NG > 1) {
+        CK(ensure_side_streams(NG));
+        CK(cudaEventRecord(g_fork, G.stream));
+        for (int g = 1; g < NG; ++g) { st[g] = g_side[g]; CK(cudaStreamWaitEvent(st[g], g_fork, 0)); }
+    }
+    for (int m = 0; m < n_mcs; ++m)
+        for (int g = 0; g < NG; ++g) {
+            if (n_metro > 0) CK(launch_sweep(n_metro, G.n_sweep + (uint32_t)m * (uint32_t)n_metro, view[g], st[g]));
+            if (do_houdayer) CK(launch_houdayer_any(do_houdayer, G.n_houdayer + (uint32_t)m, view[g], st[g]));
+            if (do_exchange) CK(launch_exchange(G.n_exchange + (uint32_t)m, view[g], st[g]));
+        }
+    for (int g = 1; g < NG; ++g) {
+        CK(cudaEventRecord(g_join[g], st[g]));
+        CK(cudaStreamWaitEvent(G.stream, g_join[g], 0));
+    }
+    G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
+    if (do_houdayer) G.n_houdayer += (uint32_t)M;
+    if (do_exchange) { G.n_exchange += (uint32_t)M; G.n_passes += M; }
     return PT_OK;
 }
 
@@ -749,7 +832,7 @@ int pt_mcs_measure_device(int n_mcs, int n_metro, int do_houdayer, int do_exchan
     if (!G.P.gauss && n_mcs >= measure_every && (do_houdayer == 0 || do_houdayer == 1) && mcs_fused_eligible(nullptr, do_houdayer, true) &&
         !mcs_split_chains(do_houdayer) && (n_metro > 0 || do_houdayer || do_exchange)) {
         const McsArgs a{n_mcs, n_metro, do_houdayer ? 1 : 0, do_exchange ? 1 : 0, 0, G.max_clu, G.n_sweep, G.n_houdayer,
-                        G.n_exchange, measure_every, Q_rec_dev, QL_rec_dev};
+                        G.n_exchange, measure_every, Q_rec_dev, QL_rec_dev, G.phase_clocks};
         CK(launch_mcs(a));
         G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
         if (do_houdayer) G.n_houdayer += (uint32_t)M;
@@ -1125,6 +1208,29 @@ int pt_get_kernel_times(double ms[5], uint64_t launches[5])
         if (launches) launches[k] = PROF.n[k];
     }
     return PT_OK;
+}
+
+int pt_set_sample_groups(int n)
+{
+    if (!G.bound) return fail(PT_ERR_STATE, "not bound");
+    if (n != -1 && (n < 1 || n > kMaxGroups)) return fail(PT_ERR_ARG, "pt_set_sample_groups: n must be -1 (automatic) or 1..%d", kMaxGroups);
+    G.sample_groups = n;
+    return PT_OK;
+}
+
+int pt_set_phase_clocks(int on)
+{
+    NEED_INIT();
+    CK(cudaMemsetAsync(G.P.d.phaseClk, 0, 4 * sizeof(unsigned long long), G.stream));
+    G.phase_clocks = on ? 1 : 0;
+    return PT_OK;
+}
+
+int pt_get_phase_clocks(uint64_t clocks[4])
+{
+    NEED_INIT();
+    if (!clocks) return fail(PT_ERR_ARG, "clocks is NULL");
+    return d2h(clocks, G.P.d.phaseClk, 4 * sizeof(unsigned long long));
 }
 
 int pt_get_launch_count(uint64_t *n_launches)

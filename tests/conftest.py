@@ -23,7 +23,7 @@ def full_length_jobs():
     idle host cores while the other GPU tests execute; longest first."""
     if _full_length["jobs"] is None:
         from paper_2003_04621_b200 import workloads as wl
-        from tests import oracle_pool as OP
+        from oracle import pool as OP
         from oracle import ref
 
         ref.build()                                  # once, before the workers race for it

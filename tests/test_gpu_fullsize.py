@@ -5,7 +5,7 @@ whole S on the device): C2-C5.  The oracle cannot run a whole config, so
   (ii) size-independent invariants are checked on ALL samples: tracked E == recomputed E, the two maps are inverse
        permutations, attempts == number of passes, accepts <= attempts, Houdayer conserves E1+E2 and Q.
 and (iii), SURVEY 8(d)'s parity subset part (i): ALL S samples for the first 16 MCS, full state, against the oracle run
-as one process per host core over disjoint `sample_offset` ranges (tests/oracle_pool.py).  Part (ii) of the subset (sampled
+as one process per host core over disjoint `sample_offset` ranges (oracle/pool.py).  Part (ii) of the subset (sampled
 samples for the whole 10^4 MCS) is tests/test_gpu_zz_fulllength.py.
 Run on the B200 box with `-m gpu`."""
 import numpy as np
@@ -15,7 +15,7 @@ from oracle import ref
 from paper_2003_04621_b200 import binding as B
 from paper_2003_04621_b200 import build as build_mod
 from paper_2003_04621_b200 import workloads as wl
-from tests import oracle_pool as OP
+from oracle import pool as OP
 
 pytestmark = pytest.mark.gpu
 

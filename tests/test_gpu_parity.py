@@ -316,6 +316,29 @@ def test_checkpoint_and_resume_continue_bit_identically(L, d, S, T, general):
     assert e.value.code == B.PT_ERR_ARG
 
 
+@pytest.mark.parametrize("L,d,general", [(64, 2, False), (8, 3, False), (6, 2, True)])
+def test_sample_groups_on_side_streams_do_not_change_results(L, d, general):
+    """The separate-kernel MCS loop cuts the samples into groups that run on their own streams (pt_set_sample_groups):
+    samples never interact (P:7), so every grouping gives the oracle's state, bit for bit (pin P8 on the device)."""
+    S, T = 11, 6
+    betas = wl.betas_geometric(0.3, 1.8, T)
+    try:
+        B.pt_set_fused(0)                                       # the three separate kernels per MCS
+        for groups in (1, 2, 5, 8, -1):
+            o = open_both(L, d, S, T, betas, offset=3, general=general)
+            B.pt_set_sample_groups(groups)
+            o.mcs(6, 1, True, True); B.pt_mcs(6, 1, True, True)
+            o.mcs(3, 2, 2, True); B.pt_mcs(3, 2, 2, True)       # multi-cluster variant, two sweeps per MCS
+            assert_same_state(o, "groups %d" % groups)
+            o.close()
+    finally:
+        B.pt_set_fused(-1)
+    with pytest.raises(B.PTError) as e:
+        B.pt_set_sample_groups(0)
+    assert e.value.code == B.PT_ERR_ARG
+    B.pt_set_sample_groups(-1)
+
+
 def test_counter_overflow_is_refused_and_leaves_the_state_alone():
     L, d, S, T = 8, 2, 2, 4
     betas = wl.betas_geometric(0.3, 1.6, T)

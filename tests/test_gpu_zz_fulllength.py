@@ -4,7 +4,7 @@ MCS launch), compared bit for bit with the oracle at MCS 10, 100, 1000 and 10^4 
 every one of C3's 1000 overlap records.
 
 The oracle needs about 20 s (C2), 10 s (C3), 1.5 min (C4) and 8 min (C5) per sample on one host core, so all fourteen
-oracle runs are started as separate processes (tests/oracle_pool.py) when the test session starts (tests/conftest.py) and
+oracle runs are started as separate processes (oracle/pool.py) when the test session starts (tests/conftest.py) and
 this module -- collected last -- only waits for what is still running: about the C5 time on a host with >= 14 cores.
 Run on the B200 box with `-m gpu`; deselect with `-m "gpu and not fulllength"` while iterating."""
 import numpy as np
@@ -13,7 +13,7 @@ import pytest
 from paper_2003_04621_b200 import binding as B
 from paper_2003_04621_b200 import build as build_mod
 from paper_2003_04621_b200 import workloads as wl
-from tests import oracle_pool as OP
+from oracle import pool as OP
 from tests.conftest import FULL_LENGTH_SAMPLES, full_length_jobs
 
 pytestmark = [pytest.mark.gpu, pytest.mark.fulllength]

@@ -1,10 +1,10 @@
-"""The multi-process oracle harness (tests/oracle_pool.py) against the single-process oracle: a run over all samples
+"""The multi-process oracle harness (oracle/pool.py) against the single-process oracle: a run over all samples
 is the concatenation of runs over disjoint `sample_offset` ranges (pin P8)."""
 import numpy as np
 
 from oracle import ref
 from paper_2003_04621_b200 import workloads as wl
-from tests import oracle_pool as OP
+from oracle import pool as OP
 
 
 def test_pool_of_oracle_processes_equals_one_oracle():
@@ -36,3 +36,13 @@ def test_pool_of_oracle_processes_equals_one_oracle():
     for (a, b), (c, e) in zip(recs, want_recs):
         assert np.array_equal(a, c) and np.array_equal(b, e)
     assert sorted(one[2]) == [10, 20, 24]
+
+
+def test_persistent_oracle_processes_advance_like_one_oracle():
+    w = wl.Workload("t", 3, 4, 4, 3, "geometric", 0.4, 1.1, 0, False, 0)
+    po = OP.PersistentOracles(w, 2, 2)
+    try:
+        assert po.step(3) == [3, 3]
+        assert po.step(2) == [5, 5]
+    finally:
+        po.close()
