@@ -391,18 +391,19 @@ class GpuRun:
         hs, hE = host_spins.numpy(), host_E.numpy()
         B.pt_get_spins(out=hs)
         for _ in range(2):
-            B.pt_set_spins(hs); self.step(); B.pt_get_energy(out=hE)
+            B.pt_set_spins_async(hs); self.step(); B.pt_get_energy(out=hE)
         self.barrier()
         t0 = time.perf_counter()
         for _ in range(steps):
-            B.pt_set_spins(hs)
+            B.pt_set_spins_async(hs)           # sample-chunked copies; the steps of the first chunks overlap the later copies
             self.step()
             B.pt_get_energy(out=hE)            # synchronises
         self.barrier()
         dt = self.max_over_ranks(time.perf_counter() - t0)
         return {"value": self.world * self.flips_step * steps / (dt * 1e9), "unit": UNIT,
                 "h2d_bytes_per_step": int(hs.nbytes), "d2h_bytes_per_step": int(hE.nbytes),
-                "steps": steps, "what": "pt_set_spins(host int8, pinned) + step + pt_get_energy(host), wall clock"}
+                "steps": steps, "what": "pt_set_spins_async(host int8, pinned: sample-chunked H2D copies on the group streams) + step + "
+                        "pt_get_energy(host, synchronises), wall clock"}
 
 
 # --------------------------------------------------------------------------------------------------------------

@@ -185,6 +185,15 @@ int pt_get_thresholds(uint32_t *thrM /* [T][d], k=1..d at [t][k-1]; may be NULL 
                       uint32_t *thrX /* [T-1][thrX_stride], entry m = |dE|/4; may be NULL */, size_t thrX_stride);
 int pt_get_counters(uint32_t *n_sweep, uint32_t *n_exchange, uint32_t *n_houdayer);
 int pt_set_spins(const int8_t *spins);      /* values must be +1/-1 (PT_ERR_ARG otherwise); recomputes E */
+/* Same upload WITHOUT waiting for it: the samples are cut into groups; every group's host-to-device copy (~16 MiB), its
+ * packing kernel and its energy kernel are queued on that group's stream and the call returns at once.  A pt_mcs /
+ * pt_mcs_measure_device call that follows runs group by group on the same streams, so the Monte Carlo steps of the first
+ * groups overlap the copies of the later ones; every other call first makes the bound stream wait for all groups.
+ * spins: HOST [S][2][T(slot)][N], +1/-1; use pinned memory (a pageable buffer makes the copies synchronous) and do not
+ * modify it before the next call that synchronises (pt_synchronize or any call that fills a host buffer).  Values are not
+ * validated up front: a byte that is neither +1 nor -1 is taken by its sign and counted, and the next pt_synchronize()
+ * then returns PT_ERR_ARG. */
+int pt_set_spins_async(const int8_t *spins);
 /* Checkpoint / resume.  The RNG is counter-based, so the complete state of a run is: the couplings (or the
  * seed), the spins, the slot_of_temp maps and the three step counters; energies follow from the spins.  A run resumed with
  * pt_init (same arguments) + pt_set_spins + pt_set_perm + pt_set_counters continues bit-identically (the observables that

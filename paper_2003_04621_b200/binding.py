@@ -54,6 +54,7 @@ SYMBOLS = {
     "pt_get_thresholds": (_i, [_vp, _vp, _sz]),
     "pt_get_counters": (_i, [_vp, _vp, _vp]),
     "pt_set_spins": (_i, [_vp]),
+    "pt_set_spins_async": (_i, [_vp]),
     "pt_set_couplings": (_i, [_vp]),
     "pt_recompute_energy": (_i, [_vp, _vp]),
     "pt_set_couplings_fixed": (_i, [_vp, _i]),
@@ -332,6 +333,13 @@ def pt_set_spins(spins):
     if s.shape != (_shape["S"], 2, _shape["T"], _shape["N"]):
         raise PTError(PT_ERR_ARG, "spins must have shape [S][2][T][N]")
     _ck(lib().pt_set_spins(_p(s)))
+
+
+def pt_set_spins_async(spins):
+    """spins: a C-contiguous int8 numpy array [S][2][T][N] (pinned for a truly asynchronous copy); must stay alive and
+    unchanged until the next synchronising call."""
+    assert spins.dtype == np.int8 and spins.flags["C_CONTIGUOUS"]
+    _ck(lib().pt_set_spins_async(spins.ctypes.data))
 
 
 def pt_set_couplings(J):

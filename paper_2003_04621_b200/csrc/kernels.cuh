@@ -167,6 +167,71 @@ __global__ void k_unpack_spins(Params P)
     }
 }
 
+// ---- word-parallel pack / unpack on the power-of-two lattices: one thread = 64 consecutive sites of one replica = one
+// word of EACH colour.  Four 16-byte loads, sign bits gathered four at a time by a multiply (byte k's sign lands on bit
+// 24 + k of m * 0x01020408: the ten partial products fall on distinct bits, no carries), the natural-order 64-bit map is
+// split by colour with the de-interleave of houdayer.cuh.  No division, no byte loads.
+// bad (may be null): counts bytes that are neither +1 nor -1 (they are taken by their sign).
+template <class LAT>
+__global__ void k_pack_spins_fast(Params P, const int8_t *src, int *bad)
+{
+    using NL = NatLat<LAT::D, LAT::kLog2L>;
+    constexpr int W = NL::W;
+    const long total = (long)P.S * 2 * P.T * W;
+    int nbad = 0;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        const int w = (int)(id % W);
+        const long rep = id / W;
+        const uint4 *p = (const uint4 *)(src + (size_t)rep * P.N + 64 * (size_t)w);
+        uint32_t nat[2] = {0u, 0u};
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const uint4 v = __ldg(p + q);
+            const uint32_t x[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t m = (x[j] >> 7) & 0x01010101u;
+                nbad += (x[j] != 0x01010101u + m * 0xFEu);
+                nat[q >> 1] |= ((m * 0x01020408u) >> 24) << (16 * (q & 1) + 4 * j);
+            }
+        }
+        uint32_t a0, a1, b0, b1;
+        NL::deinterleave(2 * w, nat[0], a0, a1);
+        NL::deinterleave(2 * w + 1, nat[1], b0, b1);
+        uint32_t *dst = P.d.spin + (size_t)rep * 2 * W;
+        dst[w] = a0 | (b0 << 16);
+        dst[W + w] = a1 | (b1 << 16);
+    }
+    if (bad && nbad) atomicAdd(bad, nbad);
+}
+
+template <class LAT>
+__global__ void k_unpack_spins_fast(Params P, int8_t *dst)
+{
+    using NL = NatLat<LAT::D, LAT::kLog2L>;
+    constexpr int W = NL::W;
+    const long total = (long)P.S * 2 * P.T * W;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        const int w = (int)(id % W);
+        const long rep = id / W;
+        const uint32_t *sw = P.d.spin + (size_t)rep * 2 * W;
+        const uint32_t c0 = sw[w], c1 = sw[W + w];
+        const uint32_t nat[2] = {NL::interleave(2 * w, c0, c1), NL::interleave(2 * w + 1, c0 >> 16, c1 >> 16)};
+        uint4 *o = (uint4 *)(dst + (size_t)rep * P.N + 64 * (size_t)w);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            uint32_t x[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t nib = (nat[q >> 1] >> (16 * (q & 1) + 4 * j)) & 0xFu;
+                const uint32_t m = (nib * 0x00204081u) & 0x01010101u;          // bit k -> byte k
+                x[j] = 0x01010101u + m * 0xFEu;                               // 0 -> +1, 1 -> -1
+            }
+            o[q] = make_uint4(x[0], x[1], x[2], x[3]);
+        }
+    }
+}
+
 // counts staged bytes that are not +1/-1 (input validation of pt_set_spins / pt_set_couplings)
 __global__ void k_check_pm1(const int8_t *a, size_t n, int *bad)
 {

@@ -21,6 +21,7 @@ struct McsArgs {
     int measure_every;                      // > 0: overlap record after every measure_every-th MCS of the call (whole-sample CTAs only)
     int32_t *recQ, *recQL;                  // device records [n_mcs / measure_every][S][T]; recQL may be null
     int phase_clocks;                       // 1: thread 0 of every CTA sums clock64() per phase into P.d.phaseClk (Eq. (11) split of the fused launch)
+    int rec_S, rec_s0;                      // records are [rec][rec_S][T]; this launch holds samples rec_s0 ... (a launch per sample group)
 };
 
 // shared-memory carve-up, shared by host (size) and device (pointers); all offsets in 32-bit words.
@@ -76,7 +77,7 @@ struct McsSmem {
 // loop 9 % on C3 (register allocation), although it runs once per measure_every steps.  Every thread of the CTA calls.
 template <class LAT, int NT>
 __device__ __noinline__ void mcs_overlap_record(LAT lat, const Params &P, const uint32_t *sS, const int *sSot, int *sQ, int s, size_t rec,
-                                                int32_t *recQ, int32_t *recQL)
+                                                size_t rec_S, int32_t *recQ, int32_t *recQL)
 {
     constexpr int D = LAT::D, W = LAT::W, RS = 2 * W + 1;
     const int T = P.T, tid = threadIdx.x;
@@ -101,8 +102,8 @@ __device__ __noinline__ void mcs_overlap_record(LAT lat, const Params &P, const 
     }
     __syncthreads();
     for (int t = tid; t < T; t += NT) {
-        recQ[(rec * P.S + s) * T + t] = P.N - 2 * sQ[t];
-        if (recQL) recQL[(rec * P.S + s) * T + t] = P.D * P.N - 2 * sQL[t];
+        recQ[(rec * rec_S + s) * T + t] = P.N - 2 * sQ[t];
+        if (recQL) recQL[(rec * rec_S + s) * T + t] = P.D * P.N - 2 * sQL[t];
     }
 }
 
@@ -347,7 +348,8 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
         // bits of q = A ^ B are gather(A) ^ gather(B).
         if constexpr (MEAS)
             if (a.measure_every > 0 && NCH == 2 && (m + 1) % a.measure_every == 0)
-                mcs_overlap_record<LAT, NT>(lat, P, sS, sSot, (int *)(msm + L.oMeas), s, (size_t)((m + 1) / a.measure_every - 1), a.recQ, a.recQL);
+                mcs_overlap_record<LAT, NT>(lat, P, sS, sSot, (int *)(msm + L.oMeas), a.rec_s0 + s, (size_t)((m + 1) / a.measure_every - 1),
+                                            (size_t)a.rec_S, a.recQ, a.recQL);
         if (clk) phase_stamp(sPh, 3);
     }
 

@@ -39,6 +39,8 @@ struct Context {
                                 // n_exchange, which pt_set_counters overwrites on a resume
     bool q_small = false;       // fixed-point couplings with 2 D max|Jq| < 2^23 (gauss.cuh: accept_site<SMALL>)
     int sample_groups = -1;     // pt_set_sample_groups: -1 = automatic
+    int pending_groups = 0;     // > 0: pt_set_spins_async left work of that many sample groups on the side streams
+    bool async_check = false;   // the +-1 count of a pt_set_spins_async has not been read yet
     int phase_clocks = 0;       // pt_set_phase_clocks
     int max_clu = 1;            // max over t of the per-temperature cluster-move counts (NEXT-4, R36)
     uint64_t launches = 0;
@@ -114,7 +116,15 @@ int fail(int code, const char *fmt, ...)
         if (e_ != cudaSuccess) return fail(PT_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_));      \
     } while (0)
 
+int join_pending();
+
+// every call that touches the state first lets the bound stream wait for what pt_set_spins_async left on the side streams
 #define NEED_INIT()                                                                  \
+    do {                                                                             \
+        if (!G.inited) return fail(PT_ERR_STATE, "%s: pt_init has not been called", __func__); \
+        if (G.pending_groups) { const int rcj_ = join_pending(); if (rcj_) return rcj_; }      \
+    } while (0)
+#define NEED_INIT_NOJOIN()                                                           \
     do {                                                                             \
         if (!G.inited) return fail(PT_ERR_STATE, "%s: pt_init has not been called", __func__); \
     } while (0)
@@ -380,6 +390,10 @@ cudaError_t launch_houdayer(uint32_t step, const Params &P, cudaStream_t st)
     return err;
 }
 
+// groups of a sample-chunked upload (pt_set_spins_async): the grouping of the MCS loop that follows it, so that every
+// group's chain copy -> pack -> energy -> MCS kernels stays on one stream
+int upload_groups();
+
 // The cluster kernels compute delta from the +-J bit couplings; with fixed-point couplings the cluster itself is the
 // same (it depends on q only) and the energies are simply recomputed from scratch, which for integers is the same number.
 // multi-cluster variant (R37): one CTA per pair, labels in shared memory
@@ -467,6 +481,52 @@ int mcs_groups()
     return (int)std::max(1L, std::min<long>(std::min<long>(waves, kMaxGroups), G.P.S));
 }
 
+struct Groups {
+    int n = 1;
+    std::vector<Params> view;
+    std::vector<cudaStream_t> st;
+    std::vector<int> s0;
+};
+
+// cut the bound problem into n contiguous sample ranges; group 0 on the bound stream, the others on side streams
+int make_groups(int n, Groups &g)
+{
+    g.n = n;
+    g.view.resize((size_t)n);
+    g.st.assign((size_t)n, G.stream);
+    g.s0.resize((size_t)n);
+    for (int k = 0; k < n; ++k) {
+        const int a0 = (int)((long)G.P.S * k / n), a1 = (int)((long)G.P.S * (k + 1) / n);
+        g.view[k] = sub_view(G.P, a0, a1 - a0);
+        g.s0[k] = a0;
+    }
+    if (n > 1) {
+        CK(ensure_side_streams(n));
+        for (int k = 1; k < n; ++k) g.st[k] = g_side[k];
+    }
+    return PT_OK;
+}
+
+// the side streams start after everything queued on the bound stream so far
+int fork_groups(const Groups &g)
+{
+    if (g.n > 1) {
+        CK(cudaEventRecord(g_fork, G.stream));
+        for (int k = 1; k < g.n; ++k) CK(cudaStreamWaitEvent(g.st[k], g_fork, 0));
+    }
+    return PT_OK;
+}
+
+// the bound stream waits for the side streams
+int join_groups(int n)
+{
+    for (int k = 1; k < n; ++k) {
+        CK(cudaEventRecord(g_join[k], g_side[k]));
+        CK(cudaStreamWaitEvent(G.stream, g_join[k], 0));
+    }
+    return PT_OK;
+}
+
 cudaError_t launch_measure(int32_t *Q, int32_t *QL)
 {
     ProfScope prof(3);
@@ -505,9 +565,10 @@ bool mcs_fused_eligible(size_t *smem_out, int do_houdayer = 1, bool measure = fa
     return (smem + 1024) * 4 <= 227 * 1024;
 }
 
-cudaError_t launch_mcs(const McsArgs &a)
+cudaError_t launch_mcs(const McsArgs &a, const Params &P = G.P, cudaStream_t st = nullptr)
 {
-    ProfScope prof(4);
+    if (!st) st = G.stream;
+    ProfScope prof(4, st);
     cudaError_t err = cudaSuccess;
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
@@ -520,8 +581,8 @@ cudaError_t launch_mcs(const McsArgs &a)
                         : G.q_small ? k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 1, false> : k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 2, false>;
             err = allow_smem(kern, smem);
             if (err != cudaSuccess) return;
-            const unsigned grid = (unsigned)G.P.S * (a.split_chains ? 2u : 1u);
-            kern<<<grid, kMcsThreads, smem, G.stream>>>(lat, G.P, a);
+            const unsigned grid = (unsigned)P.S * (a.split_chains ? 2u : 1u);
+            kern<<<grid, kMcsThreads, smem, st>>>(lat, P, a);
             ++G.launches;
             err = cudaGetLastError();
         } else {
@@ -538,13 +599,28 @@ int d2h(void *dst, const void *src, size_t bytes)
     return PT_OK;
 }
 
-int pack_spins_and_energy()
+// staged int8 spins of the samples of view P (src = their first byte in the staging area) -> bit words, then E from scratch
+int pack_spins_and_energy(const Params &P = G.P, cudaStream_t st = nullptr, const int8_t *src = nullptr, int *bad = nullptr)
 {
-    const long total = (long)G.P.S * 2 * G.P.T * 2 * G.P.W;
-    k_pack_spins<<<grid_for(total, 256), 256, 0, G.stream>>>(G.P);
-    ++G.launches;
-    CK(cudaGetLastError());
-    CK(launch_energy(0));
+    if (!st) st = G.stream;
+    if (!src) src = P.d.stage;
+    cudaError_t err = cudaSuccess;
+    with_lattice([&](auto lat) {
+        using LAT = decltype(lat);
+        if constexpr (LAT::kFast) {
+            const long total = (long)P.S * 2 * P.T * P.W;
+            k_pack_spins_fast<LAT><<<grid_for(total, 256), 256, 0, st>>>(P, src, bad);
+        } else {
+            Params V = P;
+            V.d.stage = const_cast<int8_t *>(src);
+            const long total = (long)P.S * 2 * P.T * 2 * P.W;
+            k_pack_spins<<<grid_for(total, 256), 256, 0, st>>>(V);
+        }
+        ++G.launches;
+        err = cudaGetLastError();
+    });
+    CK(err);
+    CK(launch_energy(0, P, st));
     return PT_OK;
 }
 
@@ -555,6 +631,44 @@ int pack_couplings()
     ++G.launches;
     CK(cudaGetLastError());
     return PT_OK;
+}
+
+int join_pending()
+{
+    const int n = G.pending_groups;
+    G.pending_groups = 0;
+    return join_groups(n);
+}
+
+int upload_groups()
+{
+    if (G.sample_groups > 0) return std::min(std::min(G.sample_groups, kMaxGroups), G.P.S);
+    if (!mcs_fused_eligible(nullptr, 1)) return mcs_groups();
+    const size_t bytes = (size_t)G.P.S * 2 * G.P.T * G.P.N;
+    return (int)std::max<size_t>(1, std::min<size_t>(std::min<size_t>(bytes >> 24, kMaxGroups), (size_t)G.P.S));   // ~16 MiB chunks
+}
+
+// the fused launch(es) of one pt_mcs / pt_mcs_measure_device call: one launch, or one per sample group where
+// pt_set_spins_async left the samples' uploads on the group streams (every group's chain stays on its stream)
+int run_fused(McsArgs a)
+{
+    const int NG = G.pending_groups > 1 ? G.pending_groups : 1;
+    a.rec_S = G.P.S;
+    a.rec_s0 = 0;
+    if (NG == 1) {
+        CK(launch_mcs(a));
+        return PT_OK;
+    }
+    Groups g;
+    int rc = make_groups(NG, g);
+    if (rc) return rc;
+    if ((rc = fork_groups(g))) return rc;
+    for (int k = 0; k < NG; ++k) {
+        a.rec_s0 = g.s0[k];
+        CK(launch_mcs(a, g.view[k], g.st[k]));
+    }
+    G.pending_groups = 0;
+    return join_groups(NG);
 }
 
 }  // namespace
@@ -760,7 +874,7 @@ int pt_set_cluster_moves(const int32_t *n_clu)
 
 int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
 {
-    NEED_INIT();
+    NEED_INIT_NOJOIN();
     if (n_mcs < 0 || n_metro < 0) return fail(PT_ERR_ARG, "pt_mcs: n_mcs and n_metro must be >= 0");
     if (do_houdayer < 0 || do_houdayer > 2) return fail(PT_ERR_ARG, "pt_mcs: do_houdayer must be 0, 1 (single-cluster) or 2 (multi-cluster)");
     if (do_houdayer == 2 && multi_smem_bytes(multi_threads()) > 227 * 1024)
@@ -773,8 +887,9 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
     if (n_mcs == 0 || (n_metro == 0 && !do_houdayer && !do_exchange)) return PT_OK;
     if (do_houdayer != 2 && mcs_fused_eligible(nullptr, do_houdayer)) {
         const McsArgs a{n_mcs, n_metro, do_houdayer ? 1 : 0, do_exchange ? 1 : 0, mcs_split_chains(do_houdayer) ? 1 : 0,
-                        G.max_clu, G.n_sweep, G.n_houdayer, G.n_exchange, 0, nullptr, nullptr, G.phase_clocks};
-        CK(launch_mcs(a));
+                        G.max_clu, G.n_sweep, G.n_houdayer, G.n_exchange, 0, nullptr, nullptr, G.phase_clocks, 0, 0};
+        const int rcf = run_fused(a);
+        if (rcf) return rcf;
         G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
         if (do_houdayer) G.n_houdayer += (uint32_t)M;
         if (do_exchange) { G.n_exchange += (uint32_t)M; G.n_passes += M; }
@@ -786,27 +901,19 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
     // group's sweep fills the SMs.  Group 0 runs on the caller's stream; the side streams start after everything queued
     // on it so far and it waits for them before the call returns.  Results do not depend on the grouping (pin P8).
     const int NG = mcs_groups();
-    std::vector<Params> view((size_t)NG);
-    std::vector<cudaStream_t> st((size_t)NG, G.stream);
-    for (int g = 0; g < NG; ++g) {
-        const int a0 = (int)((long)G.P.S * g / NG), a1 = (int)((long)G.P.S * (g + 1) / NG);
-        view[g] = sub_view(G.P, a0, a1 - a0);
-    }
-    if (NG > 1) {
-        CK(ensure_side_streams(NG));
-        CK(cudaEventRecord(g_fork, G.stream));
-        for (int g = 1; g < NG; ++g) { st[g] = g_side[g]; CK(cudaStreamWaitEvent(st[g], g_fork, 0)); }
-    }
+    if (G.pending_groups && G.pending_groups != NG) { const int rcj = join_pending(); if (rcj) return rcj; }
+    Groups g;
+    int rcg = make_groups(NG, g);
+    if (rcg) return rcg;
+    if ((rcg = fork_groups(g))) return rcg;
     for (int m = 0; m < n_mcs; ++m)
-        for (int g = 0; g < NG; ++g) {
-            if (n_metro > 0) CK(launch_sweep(n_metro, G.n_sweep + (uint32_t)m * (uint32_t)n_metro, view[g], st[g]));
-            if (do_houdayer) CK(launch_houdayer_any(do_houdayer, G.n_houdayer + (uint32_t)m, view[g], st[g]));
-            if (do_exchange) CK(launch_exchange(G.n_exchange + (uint32_t)m, view[g], st[g]));
+        for (int k = 0; k < NG; ++k) {
+            if (n_metro > 0) CK(launch_sweep(n_metro, G.n_sweep + (uint32_t)m * (uint32_t)n_metro, g.view[k], g.st[k]));
+            if (do_houdayer) CK(launch_houdayer_any(do_houdayer, G.n_houdayer + (uint32_t)m, g.view[k], g.st[k]));
+            if (do_exchange) CK(launch_exchange(G.n_exchange + (uint32_t)m, g.view[k], g.st[k]));
         }
-    for (int g = 1; g < NG; ++g) {
-        CK(cudaEventRecord(g_join[g], st[g]));
-        CK(cudaStreamWaitEvent(G.stream, g_join[g], 0));
-    }
+    G.pending_groups = 0;
+    if ((rcg = join_groups(NG))) return rcg;
     G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
     if (do_houdayer) G.n_houdayer += (uint32_t)M;
     if (do_exchange) { G.n_exchange += (uint32_t)M; G.n_passes += M; }
@@ -816,7 +923,7 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
 int pt_mcs_measure_device(int n_mcs, int n_metro, int do_houdayer, int do_exchange, int measure_every, int32_t *Q_rec_dev,
                           int32_t *QL_rec_dev)
 {
-    NEED_INIT();
+    NEED_INIT_NOJOIN();
     if (measure_every < 1) return fail(PT_ERR_ARG, "pt_mcs_measure_device: measure_every must be >= 1");
     if (!Q_rec_dev) return fail(PT_ERR_ARG, "pt_mcs_measure_device: Q_rec_dev is NULL");
     if (n_mcs < 0 || n_metro < 0) return fail(PT_ERR_ARG, "pt_mcs_measure_device: n_mcs and n_metro must be >= 0");
@@ -832,14 +939,16 @@ int pt_mcs_measure_device(int n_mcs, int n_metro, int do_houdayer, int do_exchan
     if (!G.P.gauss && n_mcs >= measure_every && (do_houdayer == 0 || do_houdayer == 1) && mcs_fused_eligible(nullptr, do_houdayer, true) &&
         !mcs_split_chains(do_houdayer) && (n_metro > 0 || do_houdayer || do_exchange)) {
         const McsArgs a{n_mcs, n_metro, do_houdayer ? 1 : 0, do_exchange ? 1 : 0, 0, G.max_clu, G.n_sweep, G.n_houdayer,
-                        G.n_exchange, measure_every, Q_rec_dev, QL_rec_dev, G.phase_clocks};
-        CK(launch_mcs(a));
+                        G.n_exchange, measure_every, Q_rec_dev, QL_rec_dev, G.phase_clocks, 0, 0};
+        const int rcf = run_fused(a);
+        if (rcf) return rcf;
         G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
         if (do_houdayer) G.n_houdayer += (uint32_t)M;
         if (do_exchange) { G.n_exchange += (uint32_t)M; G.n_passes += M; }
         return PT_OK;
     }
     // otherwise exactly the calls it stands for
+    if (G.pending_groups) { const int rcj = join_pending(); if (rcj) return rcj; }
     int done = 0, rec = 0;
     while (n_mcs - done >= measure_every) {
         int rc = pt_mcs(measure_every, n_metro, do_houdayer, do_exchange);
@@ -1014,9 +1123,15 @@ int pt_get_spins(int8_t *spins)
     NEED_INIT();
     if (!spins) return fail(PT_ERR_ARG, "spins is NULL");
     const size_t n = (size_t)G.P.S * 2 * G.P.T * G.P.N;
-    k_unpack_spins<<<grid_for((long)n, 256), 256, 0, G.stream>>>(G.P);
-    ++G.launches;
-    CK(cudaGetLastError());
+    cudaError_t err = cudaSuccess;
+    with_lattice([&](auto lat) {
+        using LAT = decltype(lat);
+        if constexpr (LAT::kFast) k_unpack_spins_fast<LAT><<<grid_for((long)(n / 64), 256), 256, 0, G.stream>>>(G.P, G.P.d.stage);
+        else k_unpack_spins<<<grid_for((long)n, 256), 256, 0, G.stream>>>(G.P);
+        ++G.launches;
+        err = cudaGetLastError();
+    });
+    CK(err);
     return d2h(spins, G.P.d.stage, n);
 }
 
@@ -1113,6 +1228,26 @@ int pt_set_spins(const int8_t *spins)
     return PT_OK;
 }
 
+int pt_set_spins_async(const int8_t *spins)
+{
+    NEED_INIT();
+    if (!spins) return fail(PT_ERR_ARG, "spins is NULL");
+    Groups g;
+    int rc = make_groups(upload_groups(), g);
+    if (rc) return rc;
+    CK(cudaMemsetAsync(G.P.d.mismatch + 2, 0, sizeof(int), G.stream));
+    if ((rc = fork_groups(g))) return rc;
+    const size_t per_sample = (size_t)2 * G.P.T * G.P.N;
+    for (int k = 0; k < g.n; ++k) {
+        const size_t off = (size_t)g.s0[k] * per_sample, bytes = (size_t)g.view[k].S * per_sample;
+        CK(cudaMemcpyAsync(G.P.d.stage + off, spins + off, bytes, cudaMemcpyHostToDevice, g.st[k]));
+        if ((rc = pack_spins_and_energy(g.view[k], g.st[k], G.P.d.stage + off, G.P.d.mismatch + 2))) return rc;
+    }
+    G.pending_groups = g.n > 1 ? g.n : 0;
+    G.async_check = true;
+    return PT_OK;
+}
+
 int pt_set_couplings(const int8_t *J)
 {
     NEED_INIT();
@@ -1184,7 +1319,15 @@ int pt_recompute_energy(int32_t *E_slot_order, int *mismatch_count)
 int pt_synchronize(void)
 {
     if (!G.bound) return fail(PT_ERR_STATE, "not bound");
+    if (G.pending_groups) { const int rcj = join_pending(); if (rcj) return rcj; }
     CK(cudaStreamSynchronize(G.stream));
+    if (G.inited && G.async_check) {
+        G.async_check = false;
+        int bad = 0;
+        const int rc = d2h(&bad, G.P.d.mismatch + 2, sizeof(int));
+        if (rc) return rc;
+        if (bad) return fail(PT_ERR_ARG, "pt_set_spins_async: %d words held values other than +1/-1 (taken by their sign)", bad);
+    }
     return PT_OK;
 }
 

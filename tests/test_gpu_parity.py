@@ -339,6 +339,56 @@ def test_sample_groups_on_side_streams_do_not_change_results(L, d, general):
     B.pt_set_sample_groups(-1)
 
 
+@pytest.mark.parametrize("L,d,general,fused", [(32, 2, False, True), (32, 2, False, False), (8, 3, False, True),
+                                                 (128, 2, False, True), (6, 2, True, True), (4, 3, True, True)])
+def test_async_chunked_upload_then_mcs_matches_the_oracle(L, d, general, fused):
+    """pt_set_spins_async queues sample-chunked copies + packing + energies on the group streams and returns; the MCS that
+    follows runs group by group on the same streams.  Same state as the oracle given the same spins, for the fused launch
+    (one per group), the separate kernels, the overlap records of a fused measurement, and the general-L path."""
+    import torch
+    S, T = 7, 5
+    betas = wl.betas_geometric(0.3, 1.7, T)
+    rng = np.random.default_rng(L * 10 + d)
+    spins = (rng.integers(0, 2, size=(S, 2, T, L ** d), dtype=np.int8) * 2 - 1).astype(np.int8)
+    hs = torch.from_numpy(spins.copy()).pin_memory()
+    try:
+        B.pt_set_fused(-1 if fused else 0)
+        for groups in (3, 1, -1):
+            o = open_both(L, d, S, T, betas, offset=2, general=general)
+            B.pt_set_sample_groups(groups)
+            o.set_spins(spins)
+            B.pt_set_spins_async(hs.numpy())
+            o.mcs(5, 1, True, True); B.pt_mcs(5, 1, True, True)
+            B.pt_synchronize()
+            assert_same_state(o, "async upload, groups %d" % groups)
+            # a second upload followed by a fused measurement: the records of every group land in their own rows
+            o.set_spins(spins)
+            B.pt_set_spins_async(hs.numpy())
+            Qr = torch.zeros((2, S, T), dtype=torch.int32, device="cuda"); QLr = torch.zeros_like(Qr)
+            B.pt_mcs_measure_device(4, 1, False, True, 2, Qr, QLr)
+            recs = []
+            for _ in range(2):
+                o.mcs(2, 1, False, True)
+                recs.append(o.measure_overlap())
+            B.pt_synchronize()
+            for r in range(2):
+                assert np.array_equal(Qr[r].cpu().numpy(), recs[r][0]) and np.array_equal(QLr[r].cpu().numpy(), recs[r][1])
+            assert_same_state(o, "async upload + fused measurement, groups %d" % groups)
+            o.close()
+        # values other than +1/-1 are taken by their sign and reported by the next pt_synchronize
+        bad = hs.numpy().copy(); bad[1, 0, 2, 5] = 3; bad[2, 1, 0, 0] = -7
+        hb = torch.from_numpy(bad).pin_memory()
+        B.pt_set_spins_async(hb.numpy())
+        with pytest.raises(B.PTError) as e:
+            B.pt_synchronize()
+        assert e.value.code == B.PT_ERR_ARG
+        B.pt_synchronize()                                      # reported once
+        assert np.array_equal(B.pt_get_spins(), np.where(bad < 0, -1, 1).astype(np.int8))
+    finally:
+        B.pt_set_fused(-1)
+        B.pt_set_sample_groups(-1)
+
+
 def test_counter_overflow_is_refused_and_leaves_the_state_alone():
     L, d, S, T = 8, 2, 2, 4
     betas = wl.betas_geometric(0.3, 1.6, T)
