@@ -33,8 +33,13 @@ def run_chunk(job):
     numbers in `checkpoints`, the overlap records, and the overlaps after the last MCS."""
     from oracle import ref
 
-    (L, d, T, betas, seed, g0, n, n_mcs, houdayer, measure_every, checkpoints) = job
+    (L, d, T, betas, seed, g0, n, n_mcs, houdayer, measure_every, checkpoints) = job[:11]
     o = ref.Oracle(L, d, n, T, np.asarray(betas, dtype=np.float64), seed, g0)
+    if len(job) > 11 and job[11] is not None:       # fixed-point couplings (NEXT-3): an input of the run, drawn per global sample
+        from paper_2003_04621_b200 import workloads as wl
+
+        fbits = int(job[11])
+        o.set_couplings_fixed(wl.gaussian_couplings_fixed(seed, n, d, L ** d, fbits, sample_offset=g0), fbits)
     states, recs = {}, []
     done = 0
     stops = sorted(set(int(c) for c in checkpoints if 0 < c <= n_mcs) | {n_mcs})
@@ -59,18 +64,18 @@ class OraclePool:
         self.procs = procs or n_cores()
         self.ex = ProcessPoolExecutor(max_workers=self.procs, mp_context=mp.get_context("spawn"))
 
-    def submit(self, w, g0, n, n_mcs, checkpoints=(), seed=None):
+    def submit(self, w, g0, n, n_mcs, checkpoints=(), seed=None, gaussian_fbits=None):
         from paper_2003_04621_b200 import workloads as wl
 
         job = (w.L, w.d, w.T, w.betas().tolist(), wl.SEED if seed is None else seed, int(g0), int(n), int(n_mcs),
-               bool(w.houdayer), int(w.measure_every), tuple(checkpoints))
+               bool(w.houdayer), int(w.measure_every), tuple(checkpoints), gaussian_fbits)
         return self.ex.submit(run_chunk, job)
 
-    def submit_all_samples(self, w, n_mcs, chunks_per_proc=2):
+    def submit_all_samples(self, w, n_mcs, chunks_per_proc=2, gaussian_fbits=None):
         """All S samples of workload w in contiguous chunks; returns the list of futures."""
         n_chunks = min(w.S, self.procs * chunks_per_proc)
         edges = [round(k * w.S / n_chunks) for k in range(n_chunks + 1)]
-        return [self.submit(w, a, b - a, n_mcs) for a, b in zip(edges[:-1], edges[1:]) if b > a]
+        return [self.submit(w, a, b - a, n_mcs, gaussian_fbits=gaussian_fbits) for a, b in zip(edges[:-1], edges[1:]) if b > a]
 
     def close(self):
         self.ex.shutdown(wait=False, cancel_futures=True)

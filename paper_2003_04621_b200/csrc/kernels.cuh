@@ -977,4 +977,72 @@ __global__ void __launch_bounds__(128) k_profile(LAT lat, Params P, int32_t *out
     for (int i = tid; i < DL; i += blockDim.x) o[i] = plane - 2 * pneg[i];
 }
 
+// Same profiles on the power-of-two lattices, by popcounts on the natural-order bit map (bit i = site i) of q = -1 sites:
+// one WARP per (sample, t) pair, four pairs per CTA.  Planes of constant y (z): popcount of a row, one shared-memory add per
+// WORD (the per-site version above makes one per q = -1 site).  Planes of constant x: the column sums of a block of 32 words
+// are the popcounts of the 32 x 32 bit TRANSPOSE of the block, five shuffle-and-mask butterfly stages across the lanes,
+// after which lane b holds bit b of all 32 words.  dynamic smem: D*L counters per warp.
+template <class LAT>
+__global__ void __launch_bounds__(128) k_profile_fast(LAT lat, Params P, int32_t *out)
+{
+    using NL = NatLat<LAT::D, LAT::kLog2L>;
+    constexpr int D = LAT::D, L = NL::L, LG = LAT::kLog2L, NW = NL::NW, W = NL::W;
+    constexpr bool SMALL = NL::kSmall;                 // several rows per word (L < 32)
+    constexpr int CLS = SMALL ? 1 : NL::WR;            // classes of words that hold the same x range
+    constexpr int RPW = SMALL ? 32 / L : 1;            // rows per word
+    constexpr int DL = D * L;
+    extern __shared__ int pcnt[];
+    const unsigned FULL = 0xFFFFFFFFu;
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+    const long pair = (long)blockIdx.x * wpb + wib;
+    if (pair >= (long)P.S * P.T) return;
+    const int s = (int)(pair / P.T), t = (int)(pair - (long)s * P.T);
+    int *cnt = pcnt + wib * DL;
+    for (int i = lane; i < DL; i += 32) cnt[i] = 0;
+    __syncwarp();
+    const size_t repA = rep_index(P, s, 0, P.d.sot[rep_index(P, s, 0, t)]);
+    const size_t repB = rep_index(P, s, 1, P.d.sot[rep_index(P, s, 1, t)]);
+    const uint32_t *A0 = spin_words(P, repA, 0), *A1 = A0 + W, *B0 = spin_words(P, repB, 0), *B1 = B0 + W;
+    (void)lat;
+#pragma unroll 1
+    for (int j = 0; j < CLS; ++j) {
+        int acc = 0;                                   // lane b: number of q = -1 sites on bit b of the words of class j
+#pragma unroll 1
+        for (int base = 0; base < NW / CLS; base += 32) {
+            const int idx = base + lane;
+            uint32_t x = 0;
+            if (idx < NW / CLS) {
+                const int n = idx * CLS + j, w = n >> 1;
+                const uint32_t x0 = A0[w] ^ B0[w], x1 = A1[w] ^ B1[w];
+                x = (n & 1) ? NL::interleave(n, x0 >> 16, x1 >> 16) : NL::interleave(n, x0, x1);
+#pragma unroll
+                for (int q = 0; q < RPW; ++q) {
+                    const int r = SMALL ? n * RPW + q : idx;                    // row index y + L z
+                    const int c = SMALL ? __popc(x & (((L < 32 ? (1u << (L & 31)) : 0u) - 1u) << (q * L))) : __popc(x);
+                    if (c) {
+                        atomicAdd(cnt + L + (r & (L - 1)), c);
+                        if (D == 3) atomicAdd(cnt + 2 * L + (r >> LG), c);
+                    }
+                }
+            }
+            // 32 x 32 bit transpose across the lanes (row = lane, column = bit, LSB = column 0)
+#pragma unroll
+            for (int k = 16; k >= 1; k >>= 1) {
+                const uint32_t m = (k == 16) ? 0x0000FFFFu : (k == 8) ? 0x00FF00FFu : (k == 4) ? 0x0F0F0F0Fu : (k == 2) ? 0x33333333u : 0x55555555u;
+                const uint32_t o = __shfl_xor_sync(FULL, x, k);
+                // lanes with bit k clear keep their low part and take the partner's low part into their high part;
+                // lanes with bit k set keep their high part and take the partner's high part into their low part
+                x = (lane & k) ? ((x & ~m) | ((o >> k) & m)) : ((x & m) | ((o << k) & ~m));
+            }
+            acc += __popc(x);
+        }
+        if (SMALL) atomicAdd(cnt + (lane & (L - 1)), acc);
+        else cnt[32 * j + lane] = acc;
+    }
+    __syncwarp();
+    const int plane = P.N / L;
+    int32_t *o = out + (size_t)pair * DL;
+    for (int i = lane; i < DL; i += 32) o[i] = plane - 2 * cnt[i];
+}
+
 }  // namespace ptg

@@ -614,6 +614,11 @@ int pack_spins_and_energy(const Params &P = G.P, cudaStream_t st = nullptr, cons
             Params V = P;
             V.d.stage = const_cast<int8_t *>(src);
             const long total = (long)P.S * 2 * P.T * 2 * P.W;
+            if (bad) {
+                const size_t n = (size_t)P.S * 2 * P.T * P.N;
+                k_check_pm1<<<grid_for((long)((n + 15) / 16), 256), 256, 0, st>>>(src, n, bad);
+                ++G.launches;
+            }
             k_pack_spins<<<grid_for(total, 256), 256, 0, st>>>(V);
         }
         ++G.launches;
@@ -1065,8 +1070,13 @@ int pt_measure_overlap_profile_device(int32_t *prof_dev)
     cudaError_t err = cudaSuccess;
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
-        dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
-        k_profile<LAT><<<grid, 128, (size_t)G.P.D * G.P.L * sizeof(int), G.stream>>>(lat, G.P, prof_dev);
+        if constexpr (LAT::kFast) {
+            const long pairs = (long)G.P.S * G.P.T;
+            k_profile_fast<LAT><<<(unsigned)((pairs + 3) / 4), 128, (size_t)4 * G.P.D * G.P.L * sizeof(int), G.stream>>>(lat, G.P, prof_dev);
+        } else {
+            dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
+            k_profile<LAT><<<grid, 128, (size_t)G.P.D * G.P.L * sizeof(int), G.stream>>>(lat, G.P, prof_dev);
+        }
         ++G.launches;
         err = cudaGetLastError();
     });
@@ -1326,7 +1336,7 @@ int pt_synchronize(void)
         int bad = 0;
         const int rc = d2h(&bad, G.P.d.mismatch + 2, sizeof(int));
         if (rc) return rc;
-        if (bad) return fail(PT_ERR_ARG, "pt_set_spins_async: %d words held values other than +1/-1 (taken by their sign)", bad);
+        if (bad) return fail(PT_ERR_ARG, "pt_set_spins_async: %d bytes or words held values other than +1/-1 (taken by their sign)", bad);
     }
     return PT_OK;
 }

@@ -121,6 +121,45 @@ def test_gaussian_C2_shape_sampled_samples():
                 assert np.array_equal(a[k][0], st[k][g]), (g, k)
 
 
+def test_gaussian_C2_full_size_all_samples_and_a_thousand_mcs():
+    """The Gaussian (fixed-point) path at C2's FULL size in bench.py's launch configuration (`bench.py --gaussian`: one fused
+    launch per step): (i) all 1024 samples for their first 16 MCS, full state, against oracle processes on all host cores;
+    (ii) samples {0, 1, S/2, S-1} for 1000 MCS, compared at 10, 100 and 1000 -- about 4 x 10^7 double-exp decisions per
+    sample, the ground reading R34's agreement argument stands on."""
+    from oracle import pool as OP
+
+    w, fbits = wl.C2, 16
+    Jq = wl.gaussian_couplings_fixed(wl.SEED, w.S, w.d, w.N, fbits)
+    gs = [0, 1, w.S // 2, w.S - 1]
+    pool = OP.OraclePool()
+    try:
+        long_jobs = {g: pool.submit(w, g, 1, 1000, checkpoints=(10, 100, 1000), gaussian_fbits=fbits) for g in gs}
+        futs = pool.submit_all_samples(w, 16, gaussian_fbits=fbits)
+        B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED)
+        B.pt_set_couplings_fixed(Jq, fbits)
+        assert B.pt_get_fused() == 1
+        got, done = {}, 0
+        for stop in (10, 16, 100, 1000):
+            while done < stop:
+                n = min(50, stop - done)
+                B.pt_mcs(n, 1, True, True)
+                done += n
+            st = B.state()
+            st["Q"], st["QL"] = B.pt_measure_overlap()
+            got[stop] = st if stop == 16 else {k: st[k][gs].copy() for k in OP.STATE_KEYS + ("Q", "QL")}
+        assert B.pt_recompute_energy()[1] == 0
+        want, _ = OP.gather(futs, 16)
+        for k in OP.STATE_KEYS + ("Q", "QL"):
+            assert np.array_equal(want[k], got[16][k]), "all samples after 16 MCS: %s differs" % k
+        for i, g in enumerate(gs):
+            _, _, states, _ = long_jobs[g].result()
+            for c in (10, 100, 1000):
+                for k in OP.STATE_KEYS + ("Q", "QL"):
+                    assert np.array_equal(states[c][k][0], got[c][k][i]), "sample %d after %d MCS: %s differs" % (g, c, k)
+    finally:
+        pool.close()
+
+
 @pytest.mark.parametrize("L,d,S,T,general", [(32, 2, 2, 6, False), (8, 3, 2, 5, False), (64, 2, 1, 3, False), (6, 2, 2, 4, True)])
 def test_gaussian_with_cluster_variants_and_records(L, d, S, T, general):
     """Fixed-point couplings together with the NEXT-4 variants (move counts in the fused kernel, multi-cluster step) and
