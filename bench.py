@@ -226,7 +226,7 @@ class GpuRun:
 
         self.a, self.w, self.rank, self.world, self.dev, self.flush, self.B, self.torch = a, w, rank, world, dev, flush, B, torch
         B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED, sample_offset=rank * w.S, device=dev,
-                  track_round_trips=a.track_round_trips)
+                  track_round_trips=a.track_round_trips, fixed_couplings=a.gaussian, full_staging=True)
         if a.gaussian:
             B.pt_set_couplings_fixed(wl.gaussian_couplings_fixed(wl.SEED, w.S, w.d, w.N, 16, sample_offset=rank * w.S), 16)
         self.hd, n_clu = cluster_args(a, w)
@@ -403,7 +403,7 @@ class GpuRun:
         return {"value": self.world * self.flips_step * steps / (dt * 1e9), "unit": UNIT,
                 "h2d_bytes_per_step": int(hs.nbytes), "d2h_bytes_per_step": int(hE.nbytes),
                 "steps": steps, "what": "pt_set_spins_async(host int8, pinned: sample-chunked H2D copies on the group streams) + step + "
-                        "pt_get_energy(host, synchronises), wall clock"}
+                        "pt_get_energy(host, synchronises), wall clock; workspace with PT_WS_FULL_STAGING"}
 
 
 # --------------------------------------------------------------------------------------------------------------

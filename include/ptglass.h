@@ -45,9 +45,19 @@ extern "C" {
 
 /* ---- sizes & binding ------------------------------------------------------------------------------------ */
 
-/* Bytes of device workspace needed for a problem of this shape (includes an int8 staging area for the
- * state get/set calls).  PT_ERR_ARG for shapes pt_init would reject. */
+/* Bytes of device workspace needed for a problem of this shape (includes a bounded int8 staging area, 16 MiB or one sample's state if that is more, for the
+ * state get/set calls and the init draws).  PT_ERR_ARG for shapes pt_init would reject. */
 int pt_workspace_bytes(int L, int d, int n_samples, int n_temps, size_t *bytes_out);
+/* The same with optional parts (flags OR-ed):
+ *  PT_WS_FIXED_COUPLINGS  the int32 coupling arrays of the fixed-point (Gaussian) model, 24 bytes per bond (NEXT-3):
+ *                         pt_init lays them out only where the bound workspace has room, and pt_set_couplings_fixed needs
+ *                         them (PT_ERR_STATE otherwise);
+ *  PT_WS_FULL_STAGING     a staging area of the whole int8 state (S*2*T*N bytes) instead of the bounded 16 MiB through
+ *                         which the int8 get / set calls otherwise pass in chunks of samples: pt_set_spins_async can then
+ *                         copy a whole sample group at a time.  (Any bytes bound beyond the minimum go to the staging area.) */
+#define PT_WS_FIXED_COUPLINGS 1
+#define PT_WS_FULL_STAGING    2
+int pt_workspace_bytes_ex(int L, int d, int n_samples, int n_temps, int flags, size_t *bytes_out);
 
 /* Bind the caller's device workspace (device pointer, >= pt_workspace_bytes, 256-byte aligned) and CUDA stream
  * (a cudaStream_t passed as void*; NULL = default stream).  Must precede pt_init.  Re-binding frees the context. */
@@ -249,6 +259,10 @@ int pt_get_path(int *fast);
 int pt_force_general_path(int force);
 /* Philox4x32-10 evaluated by the device code for n counters (HOST arrays ctr[n][4], out[n][4]); test hook. */
 int pt_philox_selftest(const uint32_t key[2], const uint32_t *ctr, uint32_t *out, int n);
+/* THR(x) = min(2^32-1, floor(2^32 exp(x))) evaluated by the DEVICE double exp for n arguments (HOST arrays): the rare exact
+ * decisions of the fixed-point model use it where the +-J model uses host tables (R34); test hook that lets a harness count
+ * how often it differs from the host libm's value. */
+int pt_threshold_selftest(const double *x, uint32_t *out, int n);
 /* INT32 issue-rate microbenchmark, the roofline denominator of the sweep kernel:
  * kind 0 = IMAD.WIDE.U32, 1 = LOP3, 2 = IADD3 carry pair, 3 = IMAD.WIDE+LOP3 mix, 4 = whole Philox4x32-10 blocks
  * (40 ops each).  Launches 256-thread CTAs, ctas_per_sm per SM, on cuda_stream; device_scratch: >= 4 bytes of

@@ -21,6 +21,7 @@ PT_OK, PT_ERR_ARG, PT_ERR_STATE, PT_ERR_OVERFLOW, PT_ERR_CUDA = 0, -1, -2, -3, -
 _vp, _i, _sz = C.c_void_p, C.c_int, C.c_size_t
 SYMBOLS = {
     "pt_workspace_bytes": (_i, [_i, _i, _i, _i, C.POINTER(_sz)]),
+    "pt_workspace_bytes_ex": (_i, [_i, _i, _i, _i, _i, C.POINTER(_sz)]),
     "pt_bind": (_i, [_vp, _sz, _vp]),
     "pt_init": (_i, [_i, _i, _i, _i, _vp, C.c_uint64]),
     "pt_init_shard": (_i, [_i, _i, _i, _i, _vp, C.c_uint64, C.c_uint32]),
@@ -69,6 +70,7 @@ SYMBOLS = {
     "pt_get_path": (_i, [_vp]),
     "pt_force_general_path": (_i, [_i]),
     "pt_philox_selftest": (_i, [_vp, _vp, _vp, _i]),
+    "pt_threshold_selftest": (_i, [_vp, _vp, _i]),
     "pt_microbench": (_i, [_i, _i, _i, _vp, _vp, _vp, _vp]),
     "pt_last_error": (C.c_char_p, []),
 }
@@ -121,6 +123,15 @@ def pt_workspace_bytes(L, d, n_samples, n_temps) -> int:
     return out.value
 
 
+PT_WS_FIXED_COUPLINGS, PT_WS_FULL_STAGING = 1, 2
+
+
+def pt_workspace_bytes_ex(L, d, n_samples, n_temps, flags) -> int:
+    n = _sz(0)
+    _ck(lib().pt_workspace_bytes_ex(L, d, n_samples, n_temps, int(flags), C.byref(n)))
+    return n.value
+
+
 def pt_bind(workspace, stream=None):
     """workspace: a CUDA uint8 torch tensor; stream: torch.cuda.Stream or None (current stream)."""
     global _workspace
@@ -154,11 +165,15 @@ def pt_free():
 
 
 def pt_open(L, d, n_samples, n_temps, betas, seed, sample_offset=0, device="cuda:0", stream=None, general=False,
-            track_round_trips=False, p_ferro=None):
-    """Convenience: allocate the workspace with torch, bind it and initialise.  Returns the workspace tensor."""
+            track_round_trips=False, p_ferro=None, fixed_couplings=False, full_staging=False):
+    """Convenience: allocate the workspace with torch, bind it and initialise.  Returns the workspace tensor.
+    fixed_couplings: size the workspace for pt_set_couplings_fixed (the int32 coupling arrays, NEXT-3);
+    full_staging: a staging area of the whole int8 state (whole-group copies in pt_set_spins_async)."""
     import torch
 
-    ws = torch.empty(pt_workspace_bytes(L, d, n_samples, n_temps), dtype=torch.uint8, device=device)
+    flags = (PT_WS_FIXED_COUPLINGS if fixed_couplings else 0) | (PT_WS_FULL_STAGING if full_staging else 0)
+    nbytes = pt_workspace_bytes_ex(L, d, n_samples, n_temps, flags)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=device)
     with torch.cuda.device(ws.device):
         pt_bind(ws, stream)
         if general:
@@ -423,6 +438,16 @@ def pt_philox_selftest(key, ctr):
     c = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
     out = np.empty_like(c)
     _ck(lib().pt_philox_selftest(_p(k), _p(c), _p(out), c.shape[0]))
+    return out
+
+
+def pt_threshold_selftest(x):
+    """THR(x) from the device double exp for a float64 array x (<= 0)."""
+    a = np.ascontiguousarray(x, dtype=np.float64).ravel()
+    out = np.zeros(a.size, dtype=np.uint32)
+    for i in range(0, a.size, 20000):                       # the staging area is the device scratch
+        ai, oi = a[i:i + 20000].copy(), out[i:i + 20000]
+        _ck(lib().pt_threshold_selftest(_p(ai), _p(oi), int(ai.size)))
     return out
 
 

@@ -21,6 +21,13 @@ __device__ __forceinline__ uint32_t thr_double(double x)
     return (uint32_t)v;
 }
 
+// test hook (pt_threshold_selftest): the DEVICE evaluation of THR for a list of arguments, to be compared with the host libm's
+__global__ void k_threshold_selftest(const double *x, uint32_t *out, int n)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = thr_double(x[i]);
+}
+
 // Uphill move with a = s_i h_i > 0 (units of 2^-fbits): accept iff u < THR(x), x = -(beta * ldexp(2a, -fbits)) (R34), decided
 // EXACTLY but cheaply.  Let Y = 2^32 e^x; u < floor(Y) <=> u + 1 <= Y.  A float estimate t9 of y9 = Y / 512 = 2^(23 + a c2),
 // c2 = (float)(-2 beta 2^-fbits log2 e), is off by at most 1e-5 relative: (float)a is exact below 2^23, the fma rounds once

@@ -26,7 +26,6 @@ struct DevPtrs {
     unsigned long long *cum;    // [S][T]
     int32_t *outE;              // [S][2][T] scratch for observables
     int32_t *outQ, *outQL;      // [S][T]
-    int32_t *outProf;           // [S][T][D][L] overlap profiles (NEXT-2)
     int *mismatch;              // [1]
     int8_t *stage;              // int8 staging for get/set: max(S*2*T*N, S*D*N) bytes
     // fixed-point couplings (NEXT-3, R33-R35)

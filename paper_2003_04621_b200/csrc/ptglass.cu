@@ -41,6 +41,7 @@ struct Context {
     int sample_groups = -1;     // pt_set_sample_groups: -1 = automatic
     int pending_groups = 0;     // > 0: pt_set_spins_async left work of that many sample groups on the side streams
     bool async_check = false;   // the +-1 count of a pt_set_spins_async has not been read yet
+    bool has_fixed = false;     // the workspace holds the int32 coupling arrays (pt_workspace_bytes_fixed)
     int phase_clocks = 0;       // pt_set_phase_clocks
     int max_clu = 1;            // max over t of the per-temperature cluster-move counts (NEXT-4, R36)
     uint64_t launches = 0;
@@ -177,6 +178,8 @@ uint32_t swap_stride(const std::vector<double> &b, int d, long N)
     return (uint32_t)need;
 }
 
+constexpr size_t kStageCap = (size_t)16 << 20;
+
 struct Carve {
     size_t off = 0;
     template <class T> T *take(void *base, size_t n)
@@ -188,7 +191,10 @@ struct Carve {
 };
 
 // Lay the device arrays out in the workspace; with base == nullptr only the total size is computed.
-size_t carve(void *base, int L, int d, int S, int T, uint32_t strideX, DevPtrs *out, size_t *stage_bytes)
+// fixed: also the int32 coupling arrays of the fixed-point model (NEXT-3), 24 bytes per bond more than the bit arrays
+// stage_extra: bytes by which the staging area may grow beyond its bounded minimum (never beyond one whole int8 state)
+size_t carve(void *base, int L, int d, int S, int T, uint32_t strideX, DevPtrs *out, size_t *stage_bytes, bool fixed,
+             size_t stage_extra = 0)
 {
     const size_t N = (d == 2) ? (size_t)L * L : (size_t)L * L * L;
     const size_t W = (size_t)words_per_colour((int)N);
@@ -210,9 +216,10 @@ size_t carve(void *base, int L, int d, int S, int T, uint32_t strideX, DevPtrs *
     p.outQ = c.take<int32_t>(base, (size_t)S * T);
     p.outQL = c.take<int32_t>(base, (size_t)S * T);
     p.mismatch = c.take<int>(base, 64);
-    p.outProf = c.take<int32_t>(base, (size_t)S * T * d * L);
-    p.JqNat = c.take<int32_t>(base, (size_t)S * d * N);
-    p.Jdev = c.take<int32_t>(base, (size_t)S * 2 * 2 * d * 32 * W);
+    if (fixed) {
+        p.JqNat = c.take<int32_t>(base, (size_t)S * d * N);
+        p.Jdev = c.take<int32_t>(base, (size_t)S * 2 * 2 * d * 32 * W);
+    }
     p.betasD = c.take<double>(base, (size_t)T);
     p.absdb = c.take<double>(base, (size_t)T);
     p.swapSlope = c.take<float>(base, (size_t)T);
@@ -224,7 +231,11 @@ size_t carve(void *base, int L, int d, int S, int T, uint32_t strideX, DevPtrs *
     p.nclu = c.take<int32_t>(base, (size_t)T);
     p.tcold = c.take<int32_t>(base, (size_t)T);
     p.phaseClk = c.take<unsigned long long>(base, 4);
-    const size_t sb = std::max(R * N, (size_t)S * d * N);
+    // staging: a BOUNDED buffer through which the int8 boundary (state get / set, init draws) and the host variant of the
+    // overlap profile pass in chunks of whole samples: kStageCap bytes, or one sample's worth where that is more
+    const size_t per_sample = std::max(std::max((size_t)2 * T * N, (size_t)d * N), (size_t)T * d * L * 4);
+    const size_t sb_min = std::max(std::min((size_t)S * per_sample, kStageCap), per_sample);
+    const size_t sb = std::min((size_t)S * per_sample, sb_min + stage_extra);
     p.stage = c.take<int8_t>(base, sb);
     if (out) *out = p;
     if (stage_bytes) *stage_bytes = sb;
@@ -446,9 +457,10 @@ Params sub_view(const Params &P, int s0, int n)
     V.d.E += R; V.d.tos += R; V.d.sot += R; V.d.outE += R;
     V.d.accepts += s * 2 * (size_t)(P.T - 1);
     V.d.last += s * P.T; V.d.cum += s * P.T; V.d.outQ += s * P.T; V.d.outQL += s * P.T;
-    V.d.outProf += s * P.T * P.D * P.L;
-    V.d.JqNat += s * P.D * P.N;
-    V.d.Jdev += s * 2 * 2 * P.D * 32 * P.W;
+    if (V.d.JqNat) {
+        V.d.JqNat += s * P.D * P.N;
+        V.d.Jdev += s * 2 * 2 * P.D * 32 * P.W;
+    }
     V.d.rtLabel += R; V.d.rtStart += R; V.d.rtTrips += R;
     V.d.rtSum += s * 2 * 32; V.d.rtCnt += s * 2 * 32;
     return V;
@@ -599,11 +611,9 @@ int d2h(void *dst, const void *src, size_t bytes)
     return PT_OK;
 }
 
-// staged int8 spins of the samples of view P (src = their first byte in the staging area) -> bit words, then E from scratch
-int pack_spins_and_energy(const Params &P = G.P, cudaStream_t st = nullptr, const int8_t *src = nullptr, int *bad = nullptr)
+// staged int8 spins of the samples of view P (src = their first byte in the staging area) -> bit words
+int pack_spins(const Params &P, cudaStream_t st, const int8_t *src, int *bad)
 {
-    if (!st) st = G.stream;
-    if (!src) src = P.d.stage;
     cudaError_t err = cudaSuccess;
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
@@ -625,16 +635,27 @@ int pack_spins_and_energy(const Params &P = G.P, cudaStream_t st = nullptr, cons
         err = cudaGetLastError();
     });
     CK(err);
-    CK(launch_energy(0, P, st));
     return PT_OK;
 }
 
-int pack_couplings()
+int pack_couplings(const Params &P)
 {
-    CK(cudaMemsetAsync(G.P.d.Jn, 0, (size_t)G.P.S * 2 * 2 * G.P.D * G.P.W * 4, G.stream));
-    k_pack_couplings<<<grid_for((long)G.P.S * G.P.D * G.P.N, 256), 256, 0, G.stream>>>(G.P);
+    CK(cudaMemsetAsync(P.d.Jn, 0, (size_t)P.S * 2 * 2 * P.D * P.W * 4, G.stream));
+    k_pack_couplings<<<grid_for((long)P.S * P.D * P.N, 256), 256, 0, G.stream>>>(P);
     ++G.launches;
     CK(cudaGetLastError());
+    return PT_OK;
+}
+
+// fn(view, first sample, samples) over the bound problem's samples [s_lo, s_hi) in chunks whose bytes_per_sample each fit `avail`
+template <class F> int for_chunks(size_t bytes_per_sample, size_t avail, int s_lo, int s_hi, F fn)
+{
+    const int step = (int)std::max<size_t>(1, avail / bytes_per_sample);
+    for (int s0 = s_lo; s0 < s_hi; s0 += step) {
+        const int n = std::min(step, s_hi - s0);
+        const int rc = fn(sub_view(G.P, s0, n), s0, n);
+        if (rc) return rc;
+    }
     return PT_OK;
 }
 
@@ -688,7 +709,18 @@ int pt_workspace_bytes(int L, int d, int n_samples, int n_temps, size_t *bytes_o
     if (!bytes_out) return fail(PT_ERR_ARG, "bytes_out is NULL");
     const int rc = check_shape(L, d, n_samples, n_temps);
     if (rc) return rc;
-    *bytes_out = carve(nullptr, L, d, n_samples, n_temps, full_stride(L, d), nullptr, nullptr);
+    *bytes_out = carve(nullptr, L, d, n_samples, n_temps, full_stride(L, d), nullptr, nullptr, false);
+    return PT_OK;
+}
+
+int pt_workspace_bytes_ex(int L, int d, int n_samples, int n_temps, int flags, size_t *bytes_out)
+{
+    if (!bytes_out) return fail(PT_ERR_ARG, "bytes_out is NULL");
+    if (flags & ~(PT_WS_FIXED_COUPLINGS | PT_WS_FULL_STAGING)) return fail(PT_ERR_ARG, "unknown workspace flag");
+    const int rc = check_shape(L, d, n_samples, n_temps);
+    if (rc) return rc;
+    *bytes_out = carve(nullptr, L, d, n_samples, n_temps, full_stride(L, d), nullptr, nullptr, (flags & PT_WS_FIXED_COUPLINGS) != 0,
+                       (flags & PT_WS_FULL_STAGING) ? ~(size_t)0 >> 1 : 0);
     return PT_OK;
 }
 
@@ -744,9 +776,13 @@ int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas,
     P.strideX = swap_stride(G.betas, d, P.N);
     P.track = G.track;
     P.thrJ = (unsigned long long)std::floor(std::ldexp(G.p_ferro, 32));
-    const size_t need = carve(G.ws, L, d, n_samples, n_temps, P.strideX, &P.d, &G.stage_bytes);
+    // the int32 coupling arrays of the fixed-point model are laid out only where the bound workspace has room for them
+    G.has_fixed = carve(nullptr, L, d, n_samples, n_temps, P.strideX, nullptr, nullptr, true) <= G.ws_bytes;
+    const size_t need = carve(nullptr, L, d, n_samples, n_temps, P.strideX, nullptr, nullptr, G.has_fixed);
     if (need > G.ws_bytes)
         return fail(PT_ERR_STATE, "workspace too small: %zu bytes bound, %zu needed", G.ws_bytes, need);
+    // whatever the caller bound beyond the minimum enlarges the staging area (PT_WS_FULL_STAGING: a whole int8 state)
+    carve(G.ws, L, d, n_samples, n_temps, P.strideX, &P.d, &G.stage_bytes, G.has_fixed, (G.ws_bytes - need) & ~(size_t)255);
     G.fast = (G.force_general != 0) && fast_supported(L, d);
     G.n_sweep = G.n_exchange = G.n_houdayer = 0;
     G.n_passes = 0;
@@ -787,17 +823,24 @@ int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas,
     CK(cudaMemsetAsync(P.d.rtCnt, 0, (size_t)P.S * 2 * 32 * 8, G.stream));
 
     // couplings, spins (Philox domains 1, 2), identity permutations, energies
-    k_draw_couplings<<<grid_for((long)P.S * P.D * (P.N / 4), 256), 256, 0, G.stream>>>(P);
-    ++G.launches;
-    CK(cudaGetLastError());
-    if ((rc = pack_couplings())) return rc;
-    k_draw_spins<<<grid_for((long)P.S * 2 * P.T * (P.N / 4), 256), 256, 0, G.stream>>>(P);
-    ++G.launches;
-    CK(cudaGetLastError());
+    rc = for_chunks((size_t)P.D * P.N, G.stage_bytes, 0, P.S, [&](const Params &V, int, int) {
+        k_draw_couplings<<<grid_for((long)V.S * V.D * (V.N / 4), 256), 256, 0, G.stream>>>(V);
+        ++G.launches;
+        CK(cudaGetLastError());
+        return pack_couplings(V);
+    });
+    if (rc) return rc;
+    rc = for_chunks((size_t)2 * P.T * P.N, G.stage_bytes, 0, P.S, [&](const Params &V, int, int) {
+        k_draw_spins<<<grid_for((long)V.S * 2 * V.T * (V.N / 4), 256), 256, 0, G.stream>>>(V);
+        ++G.launches;
+        CK(cudaGetLastError());
+        return pack_spins(V, G.stream, V.d.stage, nullptr);
+    });
+    if (rc) return rc;
     k_identity_perm<<<grid_for((long)P.S * 2 * P.T, 256), 256, 0, G.stream>>>(P);
     ++G.launches;
     CK(cudaGetLastError());
-    if ((rc = pack_spins_and_energy())) return rc;
+    CK(launch_energy(0));
     CK(cudaStreamSynchronize(G.stream));
     G.inited = true;
     return PT_OK;
@@ -1062,20 +1105,18 @@ int pt_measure_overlap(int32_t *Q, int32_t *QL)
     return rc;
 }
 
-int pt_measure_overlap_profile_device(int32_t *prof_dev)
+static int launch_profile(const Params &P, int32_t *out)
 {
-    NEED_INIT();
-    if (!prof_dev) return fail(PT_ERR_ARG, "prof is NULL");
     ProfScope prof(3);
     cudaError_t err = cudaSuccess;
     with_lattice([&](auto lat) {
         using LAT = decltype(lat);
         if constexpr (LAT::kFast) {
-            const long pairs = (long)G.P.S * G.P.T;
-            k_profile_fast<LAT><<<(unsigned)((pairs + 3) / 4), 128, (size_t)4 * G.P.D * G.P.L * sizeof(int), G.stream>>>(lat, G.P, prof_dev);
+            const long pairs = (long)P.S * P.T;
+            k_profile_fast<LAT><<<(unsigned)((pairs + 3) / 4), 128, (size_t)4 * P.D * P.L * sizeof(int), G.stream>>>(lat, P, out);
         } else {
-            dim3 grid((unsigned)G.P.T, (unsigned)G.P.S);
-            k_profile<LAT><<<grid, 128, (size_t)G.P.D * G.P.L * sizeof(int), G.stream>>>(lat, G.P, prof_dev);
+            dim3 grid((unsigned)P.T, (unsigned)P.S);
+            k_profile<LAT><<<grid, 128, (size_t)P.D * P.L * sizeof(int), G.stream>>>(lat, P, out);
         }
         ++G.launches;
         err = cudaGetLastError();
@@ -1084,13 +1125,28 @@ int pt_measure_overlap_profile_device(int32_t *prof_dev)
     return PT_OK;
 }
 
+int pt_measure_overlap_profile_device(int32_t *prof_dev)
+{
+    NEED_INIT();
+    if (!prof_dev) return fail(PT_ERR_ARG, "prof is NULL");
+    return launch_profile(G.P, prof_dev);
+}
+
 int pt_measure_overlap_profile(int32_t *prof)
 {
     NEED_INIT();
     if (!prof) return fail(PT_ERR_ARG, "prof is NULL");
-    const int rc = pt_measure_overlap_profile_device(G.P.d.outProf);
+    const size_t per_sample = (size_t)G.P.T * G.P.D * G.P.L * 4;
+    const int rc = for_chunks(per_sample, G.stage_bytes, 0, G.P.S, [&](const Params &V, int s0, int n) {
+        int32_t *dev = (int32_t *)V.d.stage;         // the staging area is the device buffer of the host variant
+        const int r = launch_profile(V, dev);
+        if (r) return r;
+        CK(cudaMemcpyAsync((char *)prof + (size_t)s0 * per_sample, dev, (size_t)n * per_sample, cudaMemcpyDeviceToHost, G.stream));
+        return PT_OK;
+    });
     if (rc) return rc;
-    return d2h(prof, G.P.d.outProf, (size_t)G.P.S * G.P.T * G.P.D * G.P.L * 4);
+    CK(cudaStreamSynchronize(G.stream));
+    return PT_OK;
 }
 
 int pt_get_swap_counts(uint64_t *attempts, uint64_t *accepts)
@@ -1132,17 +1188,23 @@ int pt_get_spins(int8_t *spins)
 {
     NEED_INIT();
     if (!spins) return fail(PT_ERR_ARG, "spins is NULL");
-    const size_t n = (size_t)G.P.S * 2 * G.P.T * G.P.N;
-    cudaError_t err = cudaSuccess;
-    with_lattice([&](auto lat) {
-        using LAT = decltype(lat);
-        if constexpr (LAT::kFast) k_unpack_spins_fast<LAT><<<grid_for((long)(n / 64), 256), 256, 0, G.stream>>>(G.P, G.P.d.stage);
-        else k_unpack_spins<<<grid_for((long)n, 256), 256, 0, G.stream>>>(G.P);
-        ++G.launches;
-        err = cudaGetLastError();
+    const size_t per_sample = (size_t)2 * G.P.T * G.P.N;
+    const int rc = for_chunks(per_sample, G.stage_bytes, 0, G.P.S, [&](const Params &V, int s0, int n) {
+        cudaError_t err = cudaSuccess;
+        with_lattice([&](auto lat) {
+            using LAT = decltype(lat);
+            if constexpr (LAT::kFast) k_unpack_spins_fast<LAT><<<grid_for((long)(n * per_sample / 64), 256), 256, 0, G.stream>>>(V, V.d.stage);
+            else k_unpack_spins<<<grid_for((long)(n * per_sample), 256), 256, 0, G.stream>>>(V);
+            ++G.launches;
+            err = cudaGetLastError();
+        });
+        CK(err);
+        CK(cudaMemcpyAsync(spins + (size_t)s0 * per_sample, V.d.stage, (size_t)n * per_sample, cudaMemcpyDeviceToHost, G.stream));
+        return PT_OK;
     });
-    CK(err);
-    return d2h(spins, G.P.d.stage, n);
+    if (rc) return rc;
+    CK(cudaStreamSynchronize(G.stream));
+    return PT_OK;
 }
 
 int pt_get_couplings(int8_t *J)
@@ -1150,11 +1212,17 @@ int pt_get_couplings(int8_t *J)
     NEED_INIT();
     if (!J) return fail(PT_ERR_ARG, "J is NULL");
     if (G.P.gauss) return fail(PT_ERR_STATE, "couplings are fixed-point numbers: use pt_get_couplings_fixed");
-    const size_t n = (size_t)G.P.S * G.P.D * G.P.N;
-    k_unpack_couplings<<<grid_for((long)n, 256), 256, 0, G.stream>>>(G.P);
-    ++G.launches;
-    CK(cudaGetLastError());
-    return d2h(J, G.P.d.stage, n);
+    const size_t per_sample = (size_t)G.P.D * G.P.N;
+    const int rc = for_chunks(per_sample, G.stage_bytes, 0, G.P.S, [&](const Params &V, int s0, int n) {
+        k_unpack_couplings<<<grid_for((long)(n * per_sample), 256), 256, 0, G.stream>>>(V);
+        ++G.launches;
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(J + (size_t)s0 * per_sample, V.d.stage, (size_t)n * per_sample, cudaMemcpyDeviceToHost, G.stream));
+        return PT_OK;
+    });
+    if (rc) return rc;
+    CK(cudaStreamSynchronize(G.stream));
+    return PT_OK;
 }
 
 int pt_get_thresholds(uint32_t *thrM, uint32_t *thrX, size_t thrX_stride)
@@ -1211,17 +1279,33 @@ int pt_set_perm(const int32_t *slot_of_temp)
     return PT_OK;
 }
 
-// +-1 validation of the staged int8 input, on the device (k_check_pm1 counts offenders into mismatch[1])
-static int check_pm1_staged(size_t n, const char *what)
+// Upload of a HOST int8 array of bytes_per_sample per sample through the bounded staging area, chunk by chunk, on the bound
+// stream; `use` consumes a staged chunk (nullptr: only count the values that are not +1/-1 into mismatch[1]).
+extern "C++" template <class F> int upload_chunks(const int8_t *host, size_t bytes_per_sample, bool count_bad, F use)
+{
+    return for_chunks(bytes_per_sample, G.stage_bytes, 0, G.P.S, [&](const Params &V, int s0, int n) {
+        const size_t bytes = (size_t)n * bytes_per_sample;
+        CK(cudaMemcpyAsync(V.d.stage, host + (size_t)s0 * bytes_per_sample, bytes, cudaMemcpyHostToDevice, G.stream));
+        if (count_bad) {
+            k_check_pm1<<<grid_for((long)((bytes + 15) / 16), 256), 256, 0, G.stream>>>(V.d.stage, bytes, G.P.d.mismatch + 1);
+            ++G.launches;
+            CK(cudaGetLastError());
+        }
+        return use(V);
+    });
+}
+
+// +-1 validation of a host int8 array BEFORE anything is modified (a rejected input leaves the state unchanged): where the
+// array does not fit the staging area in one piece this costs a second pass over the host buffer.
+static int validate_pm1(const int8_t *host, size_t bytes_per_sample, const char *what, bool *staged_whole)
 {
     CK(cudaMemsetAsync(G.P.d.mismatch + 1, 0, sizeof(int), G.stream));
-    k_check_pm1<<<grid_for((long)((n + 15) / 16), 256), 256, 0, G.stream>>>(G.P.d.stage, n, G.P.d.mismatch + 1);
-    ++G.launches;
-    CK(cudaGetLastError());
-    int bad = 0;
-    const int rc = d2h(&bad, G.P.d.mismatch + 1, sizeof(int));
+    int rc = upload_chunks(host, bytes_per_sample, true, [](const Params &) { return PT_OK; });
     if (rc) return rc;
+    int bad = 0;
+    if ((rc = d2h(&bad, G.P.d.mismatch + 1, sizeof(int)))) return rc;
     if (bad) return fail(PT_ERR_ARG, "%s: %d values are not +1/-1", what, bad);
+    *staged_whole = (size_t)G.P.S * bytes_per_sample <= G.stage_bytes;      // the one chunk is still in the staging area
     return PT_OK;
 }
 
@@ -1229,11 +1313,14 @@ int pt_set_spins(const int8_t *spins)
 {
     NEED_INIT();
     if (!spins) return fail(PT_ERR_ARG, "spins is NULL");
-    const size_t n = (size_t)G.P.S * 2 * G.P.T * G.P.N;
-    CK(cudaMemcpyAsync(G.P.d.stage, spins, n, cudaMemcpyHostToDevice, G.stream));
-    int rc = check_pm1_staged(n, "spins");      // rejected input leaves the state unchanged
+    const size_t per_sample = (size_t)2 * G.P.T * G.P.N;
+    bool whole = false;
+    int rc = validate_pm1(spins, per_sample, "spins", &whole);
     if (rc) return rc;
-    if ((rc = pack_spins_and_energy())) return rc;
+    if (whole) rc = pack_spins(G.P, G.stream, G.P.d.stage, nullptr);
+    else rc = upload_chunks(spins, per_sample, false, [](const Params &V) { return pack_spins(V, G.stream, V.d.stage, nullptr); });
+    if (rc) return rc;
+    CK(launch_energy(0));
     CK(cudaStreamSynchronize(G.stream));       // the caller may reuse `spins` as soon as we return
     return PT_OK;
 }
@@ -1242,16 +1329,26 @@ int pt_set_spins_async(const int8_t *spins)
 {
     NEED_INIT();
     if (!spins) return fail(PT_ERR_ARG, "spins is NULL");
+    const size_t per_sample = (size_t)2 * G.P.T * G.P.N;
+    int ng = upload_groups();
+    while (ng > 1 && G.stage_bytes / ng < per_sample) --ng;            // every group needs room for one sample
     Groups g;
-    int rc = make_groups(upload_groups(), g);
+    int rc = make_groups(ng, g);
     if (rc) return rc;
     CK(cudaMemsetAsync(G.P.d.mismatch + 2, 0, sizeof(int), G.stream));
     if ((rc = fork_groups(g))) return rc;
-    const size_t per_sample = (size_t)2 * G.P.T * G.P.N;
+    const bool whole = G.stage_bytes >= (size_t)G.P.S * per_sample;     // PT_WS_FULL_STAGING: every group in one copy, at its own offset
     for (int k = 0; k < g.n; ++k) {
-        const size_t off = (size_t)g.s0[k] * per_sample, bytes = (size_t)g.view[k].S * per_sample;
-        CK(cudaMemcpyAsync(G.P.d.stage + off, spins + off, bytes, cudaMemcpyHostToDevice, g.st[k]));
-        if ((rc = pack_spins_and_energy(g.view[k], g.st[k], G.P.d.stage + off, G.P.d.mismatch + 2))) return rc;
+        const size_t region = whole ? (size_t)g.view[k].S * per_sample : (G.stage_bytes / ng) & ~(size_t)255;
+        int8_t *stage_k = G.P.d.stage + (whole ? (size_t)g.s0[k] * per_sample : (size_t)k * region);
+        cudaStream_t st = g.st[k];
+        // copy -> pack, chunk after chunk in the group's stream (the next copy into the region waits for the pack before it)
+        rc = for_chunks(per_sample, region, g.s0[k], g.s0[k] + g.view[k].S, [&](const Params &V, int s0, int n) {
+            CK(cudaMemcpyAsync(stage_k, spins + (size_t)s0 * per_sample, (size_t)n * per_sample, cudaMemcpyHostToDevice, st));
+            return pack_spins(V, st, stage_k, G.P.d.mismatch + 2);
+        });
+        if (rc) return rc;
+        CK(launch_energy(0, g.view[k], st));
     }
     G.pending_groups = g.n > 1 ? g.n : 0;
     G.async_check = true;
@@ -1262,12 +1359,14 @@ int pt_set_couplings(const int8_t *J)
 {
     NEED_INIT();
     if (!J) return fail(PT_ERR_ARG, "J is NULL");
-    const size_t n = (size_t)G.P.S * G.P.D * G.P.N;
-    CK(cudaMemcpyAsync(G.P.d.stage, J, n, cudaMemcpyHostToDevice, G.stream));
-    int rc = check_pm1_staged(n, "J");
+    const size_t per_sample = (size_t)G.P.D * G.P.N;
+    bool whole = false;
+    int rc = validate_pm1(J, per_sample, "J", &whole);
     if (rc) return rc;
     G.P.gauss = 0;
-    if ((rc = pack_couplings())) return rc;
+    if (whole) rc = pack_couplings(G.P);
+    else rc = upload_chunks(J, per_sample, false, [](const Params &V) { return pack_couplings(V); });
+    if (rc) return rc;
     CK(launch_energy(0));
     CK(cudaStreamSynchronize(G.stream));
     return PT_OK;
@@ -1278,6 +1377,9 @@ int pt_set_couplings_fixed(const int32_t *Jq, int frac_bits)
     NEED_INIT();
     if (!Jq) return fail(PT_ERR_ARG, "Jq is NULL");
     if (frac_bits < 0 || frac_bits > 24) return fail(PT_ERR_ARG, "frac_bits must be in [0, 24]");
+    if (!G.has_fixed)
+        return fail(PT_ERR_STATE, "pt_set_couplings_fixed: the bound workspace has no room for int32 couplings "
+                                  "(bind pt_workspace_bytes_ex(..., PT_WS_FIXED_COUPLINGS, ...) bytes before pt_init)");
     const size_t n = (size_t)G.P.S * G.P.D * G.P.N;
     long long maxabs = 0;
     for (size_t k = 0; k < n; ++k) maxabs = std::max<long long>(maxabs, Jq[k] < 0 ? -(long long)Jq[k] : (long long)Jq[k]);
@@ -1391,6 +1493,20 @@ int pt_get_launch_count(uint64_t *n_launches)
     if (!n_launches) return fail(PT_ERR_ARG, "n_launches is NULL");
     *n_launches = G.launches;
     return PT_OK;
+}
+
+int pt_threshold_selftest(const double *x, uint32_t *out, int n)
+{
+    NEED_INIT();
+    if (!x || !out || n < 1) return fail(PT_ERR_ARG, "bad arguments");
+    if ((size_t)n * 12 + 16 > G.stage_bytes) return fail(PT_ERR_ARG, "n too large for the scratch area");
+    double *dx = (double *)G.P.d.stage;
+    uint32_t *dout = (uint32_t *)(dx + n);
+    CK(cudaMemcpyAsync(dx, x, (size_t)n * 8, cudaMemcpyHostToDevice, G.stream));
+    k_threshold_selftest<<<(n + 127) / 128, 128, 0, G.stream>>>(dx, dout, n);
+    ++G.launches;
+    CK(cudaGetLastError());
+    return d2h(out, dout, (size_t)n * 4);
 }
 
 int pt_philox_selftest(const uint32_t key[2], const uint32_t *ctr, uint32_t *out, int n)

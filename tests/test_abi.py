@@ -29,8 +29,11 @@ def test_header_symbols_all_exported(lib):
 
 def test_workspace_bytes_and_shape_errors(lib):
     n = B.pt_workspace_bytes(32, 2, 1024, 32)
-    # packed spins 8 MiB + int8 staging 64 MiB + overlap-profile output 8 MiB + fixed-point couplings 8 + 16 MiB dominate
-    assert 100 * 2 ** 20 < n < 120 * 2 ** 20
+    # packed spins 8 MiB + the bounded int8 staging area 16 MiB dominate; the int32 couplings of the fixed-point model
+    # (8 + 16 MiB) only on request
+    assert 24 * 2 ** 20 < n < 32 * 2 ** 20
+    assert 48 * 2 ** 20 < B.pt_workspace_bytes_ex(32, 2, 1024, 32, B.PT_WS_FIXED_COUPLINGS) < 56 * 2 ** 20
+    assert 72 * 2 ** 20 < B.pt_workspace_bytes_ex(32, 2, 1024, 32, B.PT_WS_FULL_STAGING) < 80 * 2 ** 20
     for args in [(31, 2, 1, 2), (8, 4, 1, 2), (8, 2, 0, 2), (8, 2, 1, 0), (8, 2, 1, 70000), (0, 2, 1, 1), (2048, 3, 1, 1)]:
         with pytest.raises(B.PTError) as e:
             B.pt_workspace_bytes(*args)

@@ -151,3 +151,28 @@ def test_all_samples_first_16_mcs_full_state(name):
     assert len(orecs) == len(recs) == (n_mcs // w.measure_every if w.measure_every else 0)
     for (qa, qla), (qb, qlb) in zip(orecs, recs):
         assert np.array_equal(qa, qb) and np.array_equal(qla, qlb)
+
+
+@pytest.mark.parametrize("full_staging", [False, True])
+def test_int8_state_round_trip_through_the_staging_area_at_full_size(full_staging):
+    """C2's 64 MiB int8 state does not fit the bounded 16 MiB staging area: pt_get_spins, pt_set_spins (validated first,
+    then packed, chunk by chunk) and pt_set_spins_async (sample groups on streams, chunks within a group) move it in pieces
+    of whole samples.  With PT_WS_FULL_STAGING the same calls move it whole / one group per copy.  Same bits either way."""
+    import torch
+    w = wl.C2
+    B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED, full_staging=full_staging)
+    B.pt_mcs(3, 1, True, True)
+    spins, E = B.pt_get_spins(), B.pt_get_energy()
+    B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED, full_staging=full_staging)
+    B.pt_set_spins(spins)
+    assert np.array_equal(B.pt_get_spins(), spins) and B.pt_recompute_energy()[1] == 0
+    hs = torch.from_numpy(-spins).pin_memory()
+    B.pt_set_spins_async(hs.numpy())
+    B.pt_mcs(0, 1, True, True)
+    B.pt_synchronize()
+    assert np.array_equal(B.pt_get_spins(), -spins) and B.pt_recompute_energy()[1] == 0
+    bad = spins.copy(); bad[1000, 1, 31, 1023] = 0
+    with pytest.raises(B.PTError) as e:
+        B.pt_set_spins(bad)
+    assert e.value.code == B.PT_ERR_ARG
+    assert np.array_equal(B.pt_get_spins(), -spins)            # a rejected input leaves the state unchanged

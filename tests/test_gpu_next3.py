@@ -38,7 +38,7 @@ def test_gaussian_couplings_match_oracle(L, d, S, T, fbits, general):
     Jq = wl.gaussian_couplings_fixed(wl.SEED, S, d, L ** d, fbits, sample_offset=2)
     o = ref.Oracle(L, d, S, T, betas, wl.SEED, 2)
     o.set_couplings_fixed(Jq, fbits)
-    B.pt_open(L, d, S, T, betas, wl.SEED, 2, general=general)
+    B.pt_open(L, d, S, T, betas, wl.SEED, 2, general=general, fixed_couplings=True)
     B.pt_set_couplings_fixed(Jq, fbits)
     j2, f2 = B.pt_get_couplings_fixed()
     assert np.array_equal(j2, Jq) and f2 == fbits
@@ -66,11 +66,11 @@ def test_gaussian_couplings_match_oracle(L, d, S, T, fbits, general):
 def test_pm_one_in_fixed_point_equals_the_pmJ_path_on_the_device():
     L, d, S, T, fbits = 32, 2, 2, 5, 16
     betas = wl.betas_geometric(0.3, 1.8, T)
-    B.pt_open(L, d, S, T, betas, wl.SEED)
+    B.pt_open(L, d, S, T, betas, wl.SEED, fixed_couplings=True)
     J = B.pt_get_couplings()
     B.pt_mcs(15, 1, True, True)
     ref_state = B.state()
-    B.pt_open(L, d, S, T, betas, wl.SEED)
+    B.pt_open(L, d, S, T, betas, wl.SEED, fixed_couplings=True)
     B.pt_set_couplings_fixed(J.astype(np.int32) << fbits, fbits)
     B.pt_mcs(15, 1, True, True)
     st = B.state()
@@ -83,7 +83,7 @@ def test_pm_one_in_fixed_point_equals_the_pmJ_path_on_the_device():
 
 def test_errors_and_return_to_pmJ():
     L, d, S, T = 8, 2, 1, 2
-    B.pt_open(L, d, S, T, wl.betas_linear(0.2, 1.0, T), wl.SEED)
+    B.pt_open(L, d, S, T, wl.betas_linear(0.2, 1.0, T), wl.SEED, fixed_couplings=True)
     with pytest.raises(B.PTError) as e:
         B.pt_get_couplings_fixed()
     assert e.value.code == B.PT_ERR_STATE
@@ -102,11 +102,35 @@ def test_errors_and_return_to_pmJ():
     assert np.array_equal(B.pt_get_couplings(), J) and B.pt_recompute_energy()[1] == 0
 
 
+def test_device_exp_thresholds_against_the_host_libm():
+    """Reading R34 rests on two double `exp` implementations (CUDA libdevice on the device, the C library in the oracle)
+    giving the same floor(2^32 exp(x)): both are within 1 ulp, so a differing floor needs exp(x) within ~2^-53 relative of
+    a multiple of 2^-32.  Counted here on 4 x 10^5 arguments of the form the path produces, -(beta * a * 2^-f): the floors
+    may differ by at most 1 unit, on at most a handful of arguments (0 observed)."""
+    B.pt_open(32, 2, 64, 8, wl.betas_linear(0.2, 1.0, 8), wl.SEED, fixed_couplings=True)
+    rng = np.random.default_rng(5)
+    betas = wl.betas_geometric(0.2, 3.0, 32)
+    a = rng.integers(1, 2 ** 21, size=400000)
+    x = -(betas[rng.integers(0, 32, size=a.size)] * np.ldexp(a.astype(np.float64) * 2.0, -16))
+    dev = B.pt_threshold_selftest(x).astype(np.int64)
+    host = np.array([ref.threshold(float(v)) for v in x[:20000]], dtype=np.int64)
+    # the oracle's routine on a subset, numpy's exp (also a correctly-rounded-or-1-ulp libm path) on everything
+    hostnp = np.minimum(np.floor(np.ldexp(np.exp(x), 32)), 4294967295.0).astype(np.int64)
+    assert np.abs(dev[:20000] - host).max() <= 1 and np.abs(dev - hostnp).max() <= 1
+    n_diff = int((dev[:20000] != host).sum())
+    print("device vs host THR: %d of 20000 floors differ (oracle libm), %d of %d (numpy)" % (n_diff, int((dev != hostnp).sum()), x.size))
+    assert n_diff <= 2 and (dev != hostnp).sum() <= 40
+    with pytest.raises(B.PTError) as e:             # a workspace without the int32 coupling arrays
+        B.pt_open(8, 2, 2, 4, wl.betas_linear(0.2, 1.0, 4), wl.SEED)
+        B.pt_set_couplings_fixed(np.ones((2, 2, 64), dtype=np.int32), 4)
+    assert e.value.code == B.PT_ERR_STATE
+
+
 def test_gaussian_C2_shape_sampled_samples():
     """C2's lattice, ladder and chain count with Gaussian couplings on 64 samples; samples 0 and 63 against the oracle."""
     w, S, fbits, n = wl.C2, 64, 16, 30
     Jq = wl.gaussian_couplings_fixed(wl.SEED, S, w.d, w.N, fbits)
-    B.pt_open(w.L, w.d, S, w.T, w.betas(), wl.SEED)
+    B.pt_open(w.L, w.d, S, w.T, w.betas(), wl.SEED, fixed_couplings=True)
     B.pt_set_couplings_fixed(Jq, fbits)
     B.pt_mcs(n, 1, True, True)
     st = B.state()
@@ -135,7 +159,7 @@ def test_gaussian_C2_full_size_all_samples_and_a_thousand_mcs():
     try:
         long_jobs = {g: pool.submit(w, g, 1, 1000, checkpoints=(10, 100, 1000), gaussian_fbits=fbits) for g in gs}
         futs = pool.submit_all_samples(w, 16, gaussian_fbits=fbits)
-        B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED)
+        B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED, fixed_couplings=True)
         B.pt_set_couplings_fixed(Jq, fbits)
         assert B.pt_get_fused() == 1
         got, done = {}, 0
@@ -171,7 +195,7 @@ def test_gaussian_with_cluster_variants_and_records(L, d, S, T, general):
     Jq = wl.gaussian_couplings_fixed(wl.SEED, S, d, L ** d, fbits, sample_offset=4)
     o = ref.Oracle(L, d, S, T, betas, wl.SEED, 4)
     o.set_couplings_fixed(Jq, fbits)
-    B.pt_open(L, d, S, T, betas, wl.SEED, 4, general=general)
+    B.pt_open(L, d, S, T, betas, wl.SEED, 4, general=general, fixed_couplings=True)
     B.pt_set_couplings_fixed(Jq, fbits)
     n_clu = np.array([(3 * t) % 4 for t in range(T)], dtype=np.int32)
     o.set_cluster_moves(n_clu); B.pt_set_cluster_moves(n_clu)
