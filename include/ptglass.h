@@ -204,6 +204,13 @@ int pt_set_spins(const int8_t *spins);      /* values must be +1/-1 (PT_ERR_ARG 
  * validated up front: a byte that is neither +1 nor -1 is taken by its sign and counted, and the next pt_synchronize()
  * then returns PT_ERR_ARG. */
 int pt_set_spins_async(const int8_t *spins);
+/* The same state through a BIT-PACKED boundary, one eighth of the bytes: HOST uint32 [S][2][T(slot)][ceil(N/32)], bit
+ * (i & 31) of word (i >> 5) of a replica = site i in natural order, 1 <=> spin -1 (bits beyond site N-1 are ignored on
+ * input and zero on output).  This is a boundary format; the device-internal layout is different.
+ * pt_set_spins_packed queues copy + conversion + energies on the bound stream and returns without waiting (keep the buffer
+ * unchanged until the next synchronising call; use pinned memory); pt_get_spins_packed synchronises. */
+int pt_set_spins_packed(const uint32_t *bits);
+int pt_get_spins_packed(uint32_t *bits);
 /* Checkpoint / resume.  The RNG is counter-based, so the complete state of a run is: the couplings (or the
  * seed), the spins, the slot_of_temp maps and the three step counters; energies follow from the spins.  A run resumed with
  * pt_init (same arguments) + pt_set_spins + pt_set_perm + pt_set_counters continues bit-identically (the observables that

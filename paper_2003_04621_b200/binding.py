@@ -56,6 +56,8 @@ SYMBOLS = {
     "pt_get_counters": (_i, [_vp, _vp, _vp]),
     "pt_set_spins": (_i, [_vp]),
     "pt_set_spins_async": (_i, [_vp]),
+    "pt_set_spins_packed": (_i, [_vp]),
+    "pt_get_spins_packed": (_i, [_vp]),
     "pt_set_couplings": (_i, [_vp]),
     "pt_recompute_energy": (_i, [_vp, _vp]),
     "pt_set_couplings_fixed": (_i, [_vp, _i]),
@@ -355,6 +357,21 @@ def pt_set_spins_async(spins):
     unchanged until the next synchronising call."""
     assert spins.dtype == np.int8 and spins.flags["C_CONTIGUOUS"]
     _ck(lib().pt_set_spins_async(spins.ctypes.data))
+
+
+def pt_set_spins_packed(bits):
+    """bits: C-contiguous uint32 [S][2][T][ceil(N/32)] (pinned for an asynchronous copy; keep alive until the next sync)."""
+    assert bits.dtype == np.uint32 and bits.flags["C_CONTIGUOUS"]
+    assert bits.shape == (_shape["S"], 2, _shape["T"], (_shape["N"] + 31) // 32)
+    _ck(lib().pt_set_spins_packed(bits.ctypes.data))
+
+
+def pt_get_spins_packed(out=None):
+    shape = (_shape["S"], 2, _shape["T"], (_shape["N"] + 31) // 32)
+    b = np.zeros(shape, dtype=np.uint32) if out is None else out
+    assert b.dtype == np.uint32 and b.shape == shape and b.flags["C_CONTIGUOUS"]
+    _ck(lib().pt_get_spins_packed(b.ctypes.data))
+    return b
 
 
 def pt_set_couplings(J):

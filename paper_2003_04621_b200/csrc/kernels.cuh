@@ -231,6 +231,81 @@ __global__ void k_unpack_spins_fast(Params P, int8_t *dst)
     }
 }
 
+// ---- bit-packed boundary (pt_set_spins_packed / pt_get_spins_packed): natural-order bit maps [rep][ceil(N/32)] <-> the two
+// colour arrays.  Word-parallel lattices: one thread = the two natural words 2w, 2w+1 = word w of each colour.
+template <class LAT>
+__global__ void k_nat_to_colour_fast(Params P, const uint32_t *nat)
+{
+    using NL = NatLat<LAT::D, LAT::kLog2L>;
+    constexpr int W = NL::W;
+    const long total = (long)P.S * 2 * P.T * W;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        const int w = (int)(id % W);
+        const long rep = id / W;
+        const uint2 v = *(const uint2 *)(nat + (size_t)rep * 2 * W + 2 * w);
+        uint32_t a0, a1, b0, b1;
+        NL::deinterleave(2 * w, v.x, a0, a1);
+        NL::deinterleave(2 * w + 1, v.y, b0, b1);
+        uint32_t *dst = P.d.spin + (size_t)rep * 2 * W;
+        dst[w] = a0 | (b0 << 16);
+        dst[W + w] = a1 | (b1 << 16);
+    }
+}
+
+template <class LAT>
+__global__ void k_colour_to_nat_fast(Params P, uint32_t *nat)
+{
+    using NL = NatLat<LAT::D, LAT::kLog2L>;
+    constexpr int W = NL::W;
+    const long total = (long)P.S * 2 * P.T * W;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        const int w = (int)(id % W);
+        const long rep = id / W;
+        const uint32_t *sw = P.d.spin + (size_t)rep * 2 * W;
+        const uint32_t c0 = sw[w], c1 = sw[W + w];
+        *(uint2 *)(nat + (size_t)rep * 2 * W + 2 * w) =
+            make_uint2(NL::interleave(2 * w, c0, c1), NL::interleave(2 * w + 1, c0 >> 16, c1 >> 16));
+    }
+}
+
+// general L: one thread per natural word, bit by bit (the colour arrays must be zero before k_nat_to_colour_gen)
+__global__ void k_nat_to_colour_gen(Params P, const uint32_t *nat)
+{
+    const int NWn = (P.N + 31) / 32;
+    const long total = (long)P.S * 2 * P.T * NWn;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        const int n = (int)(id % NWn);
+        const long rep = id / NWn;
+        const uint32_t x = nat[id];
+        for (int b = 0; b < 32; ++b) {
+            const int i = 32 * n + b;
+            if (i >= P.N) break;
+            if ((x >> b) & 1u) {
+                const int p = colour_of_site(i, P.L, P.D), h = i >> 1;
+                atomicOr(P.d.spin + ((size_t)rep * 2 + p) * P.W + (h >> 5), 1u << (h & 31));
+            }
+        }
+    }
+}
+
+__global__ void k_colour_to_nat_gen(Params P, uint32_t *nat)
+{
+    const int NWn = (P.N + 31) / 32;
+    const long total = (long)P.S * 2 * P.T * NWn;
+    for (long id = blockIdx.x * (long)blockDim.x + threadIdx.x; id < total; id += (long)gridDim.x * blockDim.x) {
+        const int n = (int)(id % NWn);
+        const long rep = id / NWn;
+        uint32_t x = 0;
+        for (int b = 0; b < 32; ++b) {
+            const int i = 32 * n + b;
+            if (i >= P.N) break;
+            const int p = colour_of_site(i, P.L, P.D), h = i >> 1;
+            x |= ((P.d.spin[((size_t)rep * 2 + p) * P.W + (h >> 5)] >> (h & 31)) & 1u) << b;
+        }
+        nat[id] = x;
+    }
+}
+
 // counts staged bytes that are not +1/-1 (input validation of pt_set_spins / pt_set_couplings)
 __global__ void k_check_pm1(const int8_t *a, size_t n, int *bad)
 {

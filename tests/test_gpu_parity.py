@@ -389,6 +389,32 @@ def test_async_chunked_upload_then_mcs_matches_the_oracle(L, d, general, fused):
         B.pt_set_sample_groups(-1)
 
 
+@pytest.mark.parametrize("L,d,general", [(32, 2, False), (8, 2, False), (128, 2, False), (16, 3, False), (6, 2, True), (4, 3, True), (10, 2, True)])
+def test_bit_packed_boundary_round_trip_and_dynamics(L, d, general):
+    """pt_set_spins_packed / pt_get_spins_packed carry the state as natural-order bit maps (bit i = site i, 1 <=> -1): same
+    state as the int8 calls, and the dynamics that follow match the oracle fed with the int8 array."""
+    S, T, N = 5, 4, L ** d
+    betas = wl.betas_geometric(0.3, 1.7, T)
+    rng = np.random.default_rng(L + d)
+    spins = (rng.integers(0, 2, size=(S, 2, T, N), dtype=np.int8) * 2 - 1).astype(np.int8)
+    NWn = (N + 31) // 32
+    padded = np.zeros((S, 2, T, NWn * 32), dtype=np.uint8)
+    padded[..., :N] = spins < 0
+    bits = np.ascontiguousarray(np.packbits(padded, axis=-1, bitorder="little")).view("<u4").reshape(S, 2, T, NWn)
+    o = open_both(L, d, S, T, betas, offset=1, general=general)
+    o.set_spins(spins)
+    B.pt_set_spins_packed(bits)
+    assert np.array_equal(B.pt_get_spins(), spins)
+    assert np.array_equal(B.pt_get_spins_packed(), bits)
+    assert_same_state(o, "packed upload")
+    o.mcs(6, 1, True, True); B.pt_mcs(6, 1, True, True)
+    assert_same_state(o, "packed upload + mcs")
+    got = B.pt_get_spins_packed()
+    back = np.unpackbits(got.view(np.uint8).reshape(S, 2, T, NWn * 4), axis=-1, bitorder="little")[..., :N]
+    assert np.array_equal(np.where(back == 1, -1, 1).astype(np.int8), o.get_spins())
+    o.close()
+
+
 def test_counter_overflow_is_refused_and_leaves_the_state_alone():
     L, d, S, T = 8, 2, 2, 4
     betas = wl.betas_geometric(0.3, 1.6, T)
