@@ -9,6 +9,7 @@
 #pragma once
 #include "kernels.cuh"
 #include "houdayer_lanes.cuh"
+#include "houdayer_quad.cuh"
 #include "gauss.cuh"
 
 namespace ptg {
@@ -181,8 +182,10 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
     if (clk) phase_stamp(sPh, 3);
     for (int m = 0; m < a.n_mcs; ++m) {
         // ---- a1-a3: n_metro checkerboard sweeps
+#pragma unroll 1
         for (int it = 0; it < a.n_metro; ++it) {
             const uint32_t step = a.sweep0 + (uint32_t)m * (uint32_t)a.n_metro + (uint32_t)it;
+#pragma unroll 1
             for (int p = 0; p < 2; ++p) {
 #pragma unroll 1
                 for (int item = tid; item < R * W; item += NT) {
@@ -213,7 +216,34 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                 for (int t = tid; t < T; t += NT) sPair[t] = sE[sSot[t]] + sE[T + sSot[T + t]];
                 __syncthreads();
             }
-            if constexpr (LANES) {
+            if constexpr (QuadHoudayer<LAT>::kEligible && NT == 128) {
+                // FOUR lanes per temperature, all warps of the CTA at work: 32 temperatures at a time (houdayer_quad.cuh)
+                uint32_t *cc = msm + L.oScr + (tid >> 2) * QuadHoudayer<LAT>::kPairStride;
+                for (int t0 = 0; t0 < T; t0 += 32) {
+                    const int t = t0 + (tid >> 2);
+                    const int moves = (t < T) ? P.d.nclu[t] : 0;                // R36; 1 everywhere in a default run
+                    if (t < T && moves == 0 && (tid & 3) == 0) sLast[t] = 0u;
+                    for (int mv = 0; mv < a.max_clu; ++mv) {
+                        const bool active = mv < moves;
+                        int ra = 0, rb = T;
+                        uint32_t u = 0, o1, o2, o3;
+                        if (active) {
+                            ra = sSot[t];
+                            rb = T + sSot[T + t];
+                            philox4x32_10((uint32_t)mv, step, g, make_tag(DOM_HOUD, 0, 0, t), P.rk, u, o1, o2, o3);
+                        }
+                        int delta;
+                        const int size = houdayer_quad(lat, sS + ra * RS, sS + ra * RS + W, sS + rb * RS, sS + rb * RS + W, sJ, cc, u,
+                                                       active, lane, delta);
+                        if (active && (tid & 3) == 0) {
+                            sE[ra] += delta;
+                            sE[rb] -= delta;
+                            sLast[t] = (uint32_t)size;
+                            sCum[t] += (unsigned long long)size;
+                        }
+                    }
+                }
+            } else if constexpr (LANES) {
                 // one LANE per temperature: warp k takes temperatures [32k, 32k+32), then strides by the warps in use
                 const int groups = (T + 31) / 32, hw = groups < NWARPS ? groups : NWARPS;
                 if (wid < hw) {
