@@ -25,7 +25,7 @@ def _dev_flags():
     if not v:
         return []
     d, lg = (int(x) for x in v.split(","))
-    return ["-DPTG_DEV_D=%d" % d, "-DPTG_DEV_LG=%d" % lg]
+    return ["-DPTG_DEV_D=%d" % d, "-DPTG_DEV_LG=%d" % lg] + os.environ.get("PTG_DEV_EXTRA", "").split()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

@@ -318,6 +318,11 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
         if (clk) phase_stamp(sPh, 1);
         // ---- a4: PT pass (R9: sequential walk, each step seeing the previous).  Warp 0: all lanes draw the Philox
         // words, then one lane per chain walks its ladder; only the two index maps change.
+        // Measured and rejected on B200 (profiles/r2_fused_phases.md): a decision table over all (carried, rung) pairs built
+        // by the whole CTA (2.6 K instructions per sample and MCS against 1.6 K for this walk; C2 929 against 961 flips/ns),
+        // the rungs' own-resident decisions evaluated side by side with a warp per chain (939), and a banded table with a
+        // speculative accept-bit walk and a parallel rebuild of the map (PT phase 12.4 -> 9.5 us of CTA time, but C2 952,
+        // C3 977 against 1011): the walk costs ~500 cycles per rung whatever its instruction count.
         if (a.do_exchange && T > 1) {
             const uint32_t step = a.exch0 + (uint32_t)m;
             if (wid == 0) {
