@@ -49,8 +49,9 @@ KERNEL_CLASSES = ["k_sweep", "k_houdayer", "k_exchange", "k_measure", "k_mcs"]
 # (never measured in this run: a number taken under a profiler is not a bench value).  (workload, kernel) -> (bytes, file)
 NCU_TRAFFIC = {}
 try:
-    with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as _f:
-        NCU_TRAFFIC = {tuple(k.split("/")): (v["dram_bytes_per_launch"], v["source"]) for k, v in json.load(_f).items()}
+    import csv as _csv
+    with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as _f:
+        NCU_TRAFFIC = {(r["workload"], r["kernel"]): (float(r["dram_bytes_per_launch"]), r["source"]) for r in _csv.DictReader(_f)}
 except Exception:
     pass
 
