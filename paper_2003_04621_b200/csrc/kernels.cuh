@@ -1078,6 +1078,38 @@ __global__ void __launch_bounds__(128) k_profile_fast(LAT lat, Params P, int32_t
     const size_t repB = rep_index(P, s, 1, P.d.sot[rep_index(P, s, 1, t)]);
     const uint32_t *A0 = spin_words(P, repA, 0), *A1 = A0 + W, *B0 = spin_words(P, repB, 0), *B1 = B0 + W;
     (void)lat;
+    if constexpr (!SMALL && NL::WR >= 2) {
+        // L >= 64: a colour word holds 32 same-colour sites of one row, x = 64 jc + 2 k + x0 with x0 = (colour + y) & 1, so the
+        // words of one class (jc, x0) -- colour 0 on rows y = x0 (mod 2), colour 1 on the others -- share their x positions and
+        // are transposed as they are: no colour -> natural interleave at all.
+        constexpr int WRC = NL::WR / 2;                 // colour words per row
+        constexpr int ROWS = NW / NL::WR;               // lattice rows
+#pragma unroll 1
+        for (int cls = 0; cls < 2 * WRC; ++cls) {
+            const int jc = cls >> 1, x0 = cls & 1;
+            int acc = 0;                                // lane b: q = -1 sites with x = 64 jc + 2 b + x0
+#pragma unroll 1
+            for (int base = 0; base < ROWS; base += 32) {               // ROWS words of the class: one per row
+                const int y = base + lane;
+                uint32_t x = 0;
+                if (y < ROWS) {
+                    const int p = (x0 + y) & 1;                         // the colour whose sites of row y start at x0
+                    const int w = y * WRC + jc;
+                    x = (p ? A1[w] ^ B1[w] : A0[w] ^ B0[w]);
+                    const int c = __popc(x);
+                    if (c) atomicAdd(cnt + L + (y & (L - 1)), c);
+                }
+#pragma unroll
+                for (int k = 16; k >= 1; k >>= 1) {
+                    const uint32_t m = (k == 16) ? 0x0000FFFFu : (k == 8) ? 0x00FF00FFu : (k == 4) ? 0x0F0F0F0Fu : (k == 2) ? 0x33333333u : 0x55555555u;
+                    const uint32_t o = __shfl_xor_sync(FULL, x, k);
+                    x = (lane & k) ? ((x & ~m) | ((o >> k) & m)) : ((x & m) | ((o << k) & ~m));
+                }
+                acc += __popc(x);
+            }
+            cnt[64 * jc + 2 * lane + x0] = acc;
+        }
+    } else
 #pragma unroll 1
     for (int j = 0; j < CLS; ++j) {
         int acc = 0;                                   // lane b: number of q = -1 sites on bit b of the words of class j

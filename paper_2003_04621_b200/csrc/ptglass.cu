@@ -726,10 +726,19 @@ int pt_workspace_bytes_ex(int L, int d, int n_samples, int n_temps, int flags, s
     return PT_OK;
 }
 
+// nothing of an earlier problem may still run on the side streams when the workspace changes hands
+static void drain_side_streams()
+{
+    for (int k = 1; k < kMaxGroups; ++k)
+        if (g_side[k]) cudaStreamSynchronize(g_side[k]);
+}
+
 int pt_bind(void *device_workspace, size_t bytes, void *cuda_stream)
 {
     if (!device_workspace) return fail(PT_ERR_ARG, "device_workspace is NULL");
     if (((uintptr_t)device_workspace & 255) != 0) return fail(PT_ERR_ARG, "device_workspace must be 256-byte aligned");
+    if (G.bound && G.stream) cudaStreamSynchronize(G.stream);
+    drain_side_streams();
     G = Context{};
     G.ws = device_workspace;
     G.ws_bytes = bytes;
@@ -757,6 +766,9 @@ int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas,
 {
     if (!G.bound) return fail(PT_ERR_STATE, "pt_init: no workspace bound (call pt_bind first)");
     G.inited = false;
+    drain_side_streams();
+    G.pending_groups = 0;
+    G.async_check = false;
     int rc = check_shape(L, d, n_samples, n_temps);
     if (rc) return rc;
     if (!betas) return fail(PT_ERR_ARG, "betas is NULL");
@@ -856,6 +868,8 @@ int pt_init(int L, int d, int n_samples, int n_temps, const double *betas, uint6
 int pt_free(void)
 {
     if (G.bound && G.stream) cudaStreamSynchronize(G.stream);
+    drain_side_streams();
+    G.pending_groups = 0;
     G.inited = false;
     return PT_OK;
 }

@@ -18,7 +18,8 @@ def _built():
     B.pt_free()
 
 
-@pytest.mark.parametrize("L,d,S,T", [(8, 2, 3, 5), (32, 2, 2, 6), (128, 2, 1, 3), (8, 3, 2, 4), (16, 3, 2, 3),
+@pytest.mark.parametrize("L,d,S,T", [(8, 2, 3, 5), (16, 2, 2, 3), (32, 2, 2, 6), (64, 2, 2, 3), (128, 2, 1, 3), (256, 2, 1, 2),
+                                     (8, 3, 2, 4), (16, 3, 2, 3), (32, 3, 1, 2),
                                      (2, 2, 2, 3), (6, 2, 2, 4), (10, 3, 1, 2), (4, 3, 2, 3)])
 def test_profile_matches_oracle(L, d, S, T):
     betas = wl.betas_geometric(0.3, 1.5, T)
