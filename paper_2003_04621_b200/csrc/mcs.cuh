@@ -322,7 +322,10 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
         // by the whole CTA (2.6 K instructions per sample and MCS against 1.6 K for this walk; C2 929 against 961 flips/ns),
         // the rungs' own-resident decisions evaluated side by side with a warp per chain (939), and a banded table with a
         // speculative accept-bit walk and a parallel rebuild of the map (PT phase 12.4 -> 9.5 us of CTA time, but C2 952,
-        // C3 977 against 1011): the walk costs ~500 cycles per rung whatever its instruction count.
+        // C3 977 against 1011): the walk costs ~500 cycles per rung whatever its instruction count.  Last, the pass as a SCAN
+        // (a rung = a map on the number of rungs the arriving replica was carried, composed over the ladder in 5 shuffle
+        // steps, the map rebuilt in parallel from the accept mask): PT phase 12.4 -> 7.8 us of CTA time, bit-exact, and C2 969,
+        // C3 1005, C4 1153 against 959 / 1011 / 1152 -- the phase is no longer what limits the kernel, so the walk stays.
         if (a.do_exchange && T > 1) {
             const uint32_t step = a.exch0 + (uint32_t)m;
             if (wid == 0) {
