@@ -145,13 +145,12 @@ struct FastLat {
             const int row = w / WR, j = w - row * WR;
             const int y = row & (L - 1), z = row >> LOG2L;
             const uint32_t same = ld(w);
-            if ((p + y + z) & 1) {
-                nb[1] = same;
-                nb[0] = __funnelshift_r(same, ld(row * WR + ((j + 1) & (WR - 1))), 1);
-            } else {
-                nb[0] = same;
-                nb[1] = __funnelshift_l(ld(row * WR + ((j - 1) & (WR - 1))), same, 1);
-            }
+            // sites with odd x (row parity p + y + z odd) have their +x neighbour one bit up, the others their -x neighbour one
+            // bit down; the other neighbour has the same half-index.  Branch-free: threads of a warp differ in row parity.
+            const bool oddx = (p + y + z) & 1;
+            const uint32_t side = ld(row * WR + ((oddx ? j + 1 : j - 1) & (WR - 1)));
+            nb[0] = oddx ? __funnelshift_r(same, side, 1) : same;
+            nb[1] = oddx ? same : __funnelshift_l(side, same, 1);
             const int base = z * PW, jj = w - base;
             nb[2] = ld(base + ((jj + WR) & (PW - 1)));
             nb[3] = ld(base + ((jj - WR) & (PW - 1)));
