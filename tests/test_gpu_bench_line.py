@@ -1,0 +1,46 @@
+"""bench.py prints ONE JSON line with the keys the driver reads (metric, value, roofline, cpu_baseline, e2e, clocks,
+gpu_launches, per_config ...): checked here on the smallest workload so that a broken bench shows up in the test run."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def run_bench(*args):
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), *args], capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, out.stdout[-2000:]
+    return json.loads(lines[0])
+
+
+def test_bench_line_has_the_contracted_keys():
+    d = run_bench("--workload", "C1", "--steps", "4", "--warmup", "3", "--config-steps", "3", "--e2e-steps", "2")
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline",
+              "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline", "per_config"):
+        assert k in d, k
+    assert d["value"] > 0 and d["gpu_launches"] > 0 and d["vs_baseline"] is None and "workload" in d["config"]
+    r = d["roofline"]
+    for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic", "traffic_source", "phases", "sweep_only", "kernel_ms"):
+        assert k in r, k
+    assert r["bound"] == "alu" and 0 < r["frac"] < 1
+    assert set(r["phases"]["ns_per_spin"]) == {"metropolis", "houdayer", "exchange", "rest"}
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["one_core"]["cores"] == 1
+    e = d["e2e"]
+    assert e["value"] > 0 and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0 and e["packed_boundary"]["value"] > 0
+    assert set(d["per_config"]) == {"C1", "C2", "C3", "C4", "C5"}
+    for name in ("C2", "C3", "C4", "C5"):
+        pc = d["per_config"][name]
+        assert pc["value"] > 100 and 0 < pc["roofline"]["frac"] < 1 and pc["clocks"] is not None
+
+
+def test_reference_arm_prints_the_oracle_line():
+    d = run_bench("--impl", "reference", "--workload", "C1", "--steps", "3", "--warmup", "1")
+    assert d["impl"] == "reference" and d["value"] > 0 and d["gpu_launches"] == 0
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
