@@ -122,7 +122,9 @@ __device__ __forceinline__ void phase_stamp(unsigned long long *sPh, int k)
 // recomputed from scratch after the cluster moves (field_sum_word_q; the cluster itself depends on q only) and the PT walk
 // evaluates its thresholds in double (swap_threshold).
 // MEAS: overlap records after every a.measure_every-th MCS from the resident state (pt_mcs_measure_device).
-template <class LAT, int NT, int MINB, int GAUSS, bool MEAS>
+// MULTI: the cluster phase is the multi-cluster exchange (R37; a.do_houdayer == 2) on the four-lane strips -- a separate
+// instantiation (2D L = 32 only), so that the kernel of the paper's MCS keeps its code.
+template <class LAT, int NT, int MINB, int GAUSS, bool MEAS, bool MULTI = false>
 __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
 {
     constexpr int D = LAT::D, W = LAT::W, NWARPS = NT / 32;
@@ -216,7 +218,24 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
                 for (int t = tid; t < T; t += NT) sPair[t] = sE[sSot[t]] + sE[T + sSot[T + t]];
                 __syncthreads();
             }
-            if constexpr (QuadHoudayer<LAT>::kEligible && NT == 128) {
+            if constexpr (MULTI && QuadHoudayer<LAT>::kEligible && NT == 128) {
+                // multi-cluster exchange, four lanes per temperature (houdayer_multi_quad); R36's move counts do not apply
+                uint32_t *cc = msm + L.oScr + (tid >> 2) * QuadHoudayer<LAT>::kPairStride;
+                for (int t0 = 0; t0 < T; t0 += 32) {
+                    const int t = t0 + (tid >> 2);
+                    const bool active = t < T;
+                    const int ra = active ? sSot[t] : 0, rb = active ? T + sSot[T + t] : T;
+                    int delta;
+                    const int size = houdayer_multi_quad(lat, sS + ra * RS, sS + ra * RS + W, sS + rb * RS, sS + rb * RS + W, sJ, cc,
+                                                         step, g, active ? t : 0, P.rk, active, lane, delta);
+                    if (active && (tid & 3) == 0) {
+                        sE[ra] += delta;
+                        sE[rb] -= delta;
+                        sLast[t] = (uint32_t)size;
+                        sCum[t] += (unsigned long long)size;
+                    }
+                }
+            } else if constexpr (QuadHoudayer<LAT>::kEligible && NT == 128) {
                 // FOUR lanes per temperature, all warps of the CTA at work: 32 temperatures at a time (houdayer_quad.cuh)
                 uint32_t *cc = msm + L.oScr + (tid >> 2) * QuadHoudayer<LAT>::kPairStride;
                 for (int t0 = 0; t0 < T; t0 += 32) {

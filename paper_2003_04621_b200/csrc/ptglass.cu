@@ -577,6 +577,9 @@ bool mcs_fused_eligible(size_t *smem_out, int do_houdayer = 1, bool measure = fa
     return (smem + 1024) * 4 <= 227 * 1024;
 }
 
+// the multi-cluster exchange inside the fused kernel: 2D L = 32, +-J couplings (houdayer_multi_quad)
+bool mcs_multi_fused() { return G.fast && G.P.D == 2 && G.P.L == 32 && !G.P.gauss; }
+
 cudaError_t launch_mcs(const McsArgs &a, const Params &P = G.P, cudaStream_t st = nullptr)
 {
     if (!st) st = G.stream;
@@ -591,6 +594,9 @@ cudaError_t launch_mcs(const McsArgs &a, const Params &P = G.P, cudaStream_t st 
             // the fused measurement is instantiated for the +-J model only (pt_mcs_measure_device falls back otherwise)
             auto kern = !G.P.gauss ? (meas ? k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 0, true> : k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 0, false>)
                         : G.q_small ? k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 1, false> : k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 2, false>;
+            if constexpr (QuadHoudayer<LAT>::kEligible) {
+                if (a.do_houdayer == 2) kern = k_mcs<LAT, kMcsThreads, kMcsMinBlocks, 0, false, true>;
+            }
             err = allow_smem(kern, smem);
             if (err != cudaSuccess) return;
             const unsigned grid = (unsigned)P.S * (a.split_chains ? 2u : 1u);
@@ -949,8 +955,8 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
         (do_houdayer && (uint64_t)G.n_houdayer + M > 4294967295ull))
         return fail(PT_ERR_OVERFLOW, "a step counter would overflow");
     if (n_mcs == 0 || (n_metro == 0 && !do_houdayer && !do_exchange)) return PT_OK;
-    if (do_houdayer != 2 && mcs_fused_eligible(nullptr, do_houdayer)) {
-        const McsArgs a{n_mcs, n_metro, do_houdayer ? 1 : 0, do_exchange ? 1 : 0, mcs_split_chains(do_houdayer) ? 1 : 0,
+    if ((do_houdayer != 2 || mcs_multi_fused()) && mcs_fused_eligible(nullptr, do_houdayer)) {
+        const McsArgs a{n_mcs, n_metro, do_houdayer, do_exchange ? 1 : 0, mcs_split_chains(do_houdayer) ? 1 : 0,
                         G.max_clu, G.n_sweep, G.n_houdayer, G.n_exchange, 0, nullptr, nullptr, G.phase_clocks, 0, 0};
         const int rcf = run_fused(a);
         if (rcf) return rcf;

@@ -117,6 +117,36 @@ def test_multi_cluster_matches_oracle(L, d, S, T, general):
     same_state(o, "mixed")
 
 
+@pytest.mark.parametrize("T", [32, 40, 5])
+def test_fused_multi_cluster_on_register_strips(T):
+    """2D L = 32: pt_mcs(..., 2, ...) is ONE launch (houdayer_multi_quad: roots by a tournament over the index bits, one Philox
+    coin per root, one growth from the chosen roots) -- against the oracle's component labelling and against the separate
+    label-equivalence kernel, for one and two groups of 32 temperatures."""
+    L, d, S = 32, 2, 3
+    betas = wl.betas_geometric(0.2, 3.0, T)
+    o = ref.Oracle(L, d, S, T, betas, wl.SEED, 7)
+    B.pt_open(L, d, S, T, betas, wl.SEED, 7)
+    assert B.pt_get_fused() == 1
+    n0 = B.pt_get_launch_count()
+    o.mcs(12, 1, 2, True); B.pt_mcs(12, 1, 2, True)
+    assert B.pt_get_launch_count() - n0 == 1
+    same_state(o, "fused multi, T = %d" % T)
+    o.mcs(3, 2, 1, True); B.pt_mcs(3, 2, 1, True)              # the single-cluster move in between: one Houdayer counter
+    o.mcs(5, 1, 2, False); B.pt_mcs(5, 1, 2, False)
+    same_state(o, "fused multi after mixing, T = %d" % T)
+    fused = B.state()
+    try:
+        B.pt_open(L, d, S, T, betas, wl.SEED, 7)
+        B.pt_set_fused(0)
+        B.pt_mcs(12, 1, 2, True); B.pt_mcs(3, 2, 1, True); B.pt_mcs(5, 1, 2, False)
+        sep = B.state()
+    finally:
+        B.pt_set_fused(-1)
+    for k in fused:
+        assert np.array_equal(fused[k], sep[k]), k
+    o.close()
+
+
 def test_multi_cluster_special_cases_on_device():
     L, d, S, T = 16, 2, 3, 4
     N = L * L
