@@ -235,6 +235,47 @@ int pt_get_couplings_fixed(int32_t *Jq /* [S][d][N] or NULL */, int *frac_bits /
 /* Recompute every E from scratch and count slots whose tracked E differs (invariant check; must be 0). */
 int pt_recompute_energy(int32_t *E_slot_order /* [S][2][T] or NULL */, int *mismatch_count /* or NULL */);
 
+/* ---- one PT pass for callers that must not allocate device memory ------------------------------------------ */
+
+/* Everything above works inside a workspace the caller allocates and hands to pt_bind().  Some callers cannot do that:
+ * an analysis hook that runs inside somebody else's GPU job after that job's memory pool (a framework's caching
+ * allocator, a simulation sized to fill the card) has taken the device memory, so a fresh cudaMalloc fails or is against
+ * the host program's rules; a latency-critical loop that cannot afford the device-wide synchronisation that
+ * cudaMalloc / cudaFree imply while other streams are busy.  For them this ONE call needs no workspace, no pt_bind
+ * and no pt_init, and allocates no device memory, neither itself nor through a library routine: its scratch is a fixed
+ * area of PT_NOALLOC_SCRATCH_BYTES (4 MiB) that is part of libptglass.so's device image (every GPU on which the
+ * library's code is loaded holds that area until the process exits).
+ *
+ * pt_exchange_noalloc makes the decisions of pt_exchange() (Eq. (5); R9, R10) -- pass number `step`
+ * of a +-J problem of n_samples samples of an L^d lattice on the ladder betas, keyed by (seed, sample_offset) exactly as
+ * after pt_init_shard -- on arrays the CALLER holds:
+ *   E_dev             DEVICE const int32 [n_samples][2][n_temps], energy of every slot (slot order), read only;
+ *   slot_of_temp_dev  DEVICE int32, same shape, every row a permutation of 0..n_temps-1 (NOT checked: an entry out of
+ *                     range makes the kernel read outside E_dev), updated in place;
+ *   temp_of_slot_dev  DEVICE int32, same shape, overwritten with the inverse of the new slot_of_temp;
+ *   accepts_dev       DEVICE uint64 [n_samples][2][n_temps-1] or NULL: += 1 for every accepted pair;
+ *   betas             HOST double [n_temps], as for pt_init;  step = the value pt_get_counters() reports as n_exchange
+ *                     for the pass to reproduce;  cuda_stream: a cudaStream_t of the CURRENT device (NULL = default).
+ * With these, maps and counts come out bit-identical to pt_exchange() on the same state.  The call returns once the work
+ * is queued on cuda_stream; it does not synchronise.  The bound context (if any) is neither needed nor touched.
+ * What the scratch holds: the swap-threshold table of the ladder and the sign of every beta step, computed on the host
+ * in double and copied in on EVERY call (O(n_temps * table stride) exp() evaluations: meant for the occasional pass, not
+ * for the inner loop), and the energies in temperature order on which the walk runs.
+ * PT_ERR_ARG, nothing queued: an argument pt_init would reject (the shared-memory limit on L does not apply here), a
+ * NULL array other than accepts_dev, or a problem whose tables and energies need more than PT_NOALLOC_SCRATCH_BYTES (the
+ * message states both numbers; such problems need pt_bind + pt_exchange).  PT_ERR_CUDA: a CUDA call failed.
+ * SET-UP: the first call on each device asks the CUDA runtime where that device keeps the scratch area (no allocation,
+ * but a runtime query that may load the library's device code); make that first call before any stream capture begins
+ * on the device.  Later calls on the device skip it.
+ * SHARING: there is one scratch area per device and every call writes it, leaving its contents behind.  Each call
+ * rewrites all it will read, so nothing has to be cleared and the order of earlier calls does not matter -- but two calls
+ * whose work can overlap on the GPU (different streams without an event between them, or two host threads) race on it and
+ * give garbage.  Put them on one stream or order them with events.  Like the rest of the library, not thread-safe. */
+#define PT_NOALLOC_SCRATCH_BYTES (4u << 20)
+int pt_exchange_noalloc(int L, int d, int n_samples, int n_temps, const double *betas, uint64_t seed,
+                        uint32_t sample_offset, uint32_t step, const int32_t *E_dev, int32_t *slot_of_temp_dev,
+                        int32_t *temp_of_slot_dev, uint64_t *accepts_dev, void *cuda_stream);
+
 /* ---- diagnostics ---------------------------------------------------------------------------------------- */
 
 int pt_synchronize(void);                          /* cudaStreamSynchronize on the bound stream */

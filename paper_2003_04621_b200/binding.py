@@ -71,6 +71,7 @@ SYMBOLS = {
     "pt_get_phase_clocks": (_i, [_vp]),
     "pt_get_path": (_i, [_vp]),
     "pt_force_general_path": (_i, [_i]),
+    "pt_exchange_noalloc": (_i, [_i, _i, _i, _i, _vp, C.c_uint64, C.c_uint32, C.c_uint32, _vp, _vp, _vp, _vp, _vp]),
     "pt_philox_selftest": (_i, [_vp, _vp, _vp, _i]),
     "pt_threshold_selftest": (_i, [_vp, _vp, _i]),
     "pt_microbench": (_i, [_i, _i, _i, _vp, _vp, _vp, _vp]),
@@ -448,6 +449,36 @@ def pt_get_path() -> int:
 
 def pt_force_general_path(force):
     _ck(lib().pt_force_general_path(force))
+
+
+PT_NOALLOC_SCRATCH_BYTES = 4 << 20
+
+
+def pt_exchange_noalloc(L, d, betas, seed, sample_offset, step, E_dev, slot_of_temp_dev, temp_of_slot_dev,
+                        accepts_dev=None, stream=None):
+    """One PT pass on the caller's own device arrays, for callers that must not allocate device memory (a hook inside a
+    job whose memory pool already owns the card, a loop that cannot take cudaMalloc's device-wide synchronisation): needs
+    no workspace, no pt_bind, no pt_init; its scratch is a fixed 4 MiB area inside the library (see include/ptglass.h).
+    E_dev [S][2][T] int32 (slot order, read only), slot_of_temp_dev (updated in place) and temp_of_slot_dev (overwritten)
+    are torch CUDA int32 tensors of one shape; accepts_dev an int64 / uint64 CUDA tensor [S][2][T-1] or None.  S and T are
+    taken from E_dev's shape.  Queued on `stream` (default: torch's current stream of E_dev's device); does not
+    synchronise.  Calls whose GPU work may overlap race on the shared scratch: keep them on one stream."""
+    import torch
+
+    b = np.ascontiguousarray(betas, dtype=np.float64)
+    S, two, T = E_dev.shape
+    if two != 2 or b.shape != (T,):
+        raise PTError(PT_ERR_ARG, "E_dev must have shape [S][2][T] and betas shape (T,)")
+    for a in (E_dev, slot_of_temp_dev, temp_of_slot_dev):
+        assert a.is_cuda and a.dtype == torch.int32 and a.is_contiguous() and a.shape == E_dev.shape
+    if accepts_dev is not None:
+        assert accepts_dev.is_cuda and accepts_dev.element_size() == 8 and accepts_dev.is_contiguous()
+        assert tuple(accepts_dev.shape) == (S, 2, max(T - 1, 0))
+    with torch.cuda.device(E_dev.device):
+        st = torch.cuda.current_stream() if stream is None else stream
+        _ck(lib().pt_exchange_noalloc(int(L), int(d), int(S), int(T), _p(b), int(seed), int(sample_offset), int(step),
+                                      E_dev.data_ptr(), slot_of_temp_dev.data_ptr(), temp_of_slot_dev.data_ptr(),
+                                      None if accepts_dev is None else accepts_dev.data_ptr(), st.cuda_stream))
 
 
 def pt_philox_selftest(key, ctr):

@@ -1609,3 +1609,141 @@ int pt_philox_selftest(const uint32_t key[2], const uint32_t *ctr, uint32_t *out
 }
 
 }  // extern "C"
+
+// =========================================================================================================
+// pt_exchange_noalloc: one PT pass for callers that must not allocate device memory (include/ptglass.h).
+// A variant of k_exchange<GLOBAL_SCRATCH = true>: that kernel walks the ladder on scratch in global memory (the energies
+// in temperature order) and reads the threshold table and the signs of the beta steps from the caller's workspace.  Here
+// all three live in ONE fixed area that is part of this library's device image, so that a caller who cannot (or may not)
+// call cudaMalloc -- a hook inside a job whose memory pool already owns the card, a loop that cannot take cudaMalloc's
+// device-wide synchronisation -- can still run a pass.  Nothing below allocates or frees device memory.
+// =========================================================================================================
+
+// The scratch area.  In HOST code this name is only a handle for the runtime's symbol calls, not a device address: a
+// kernel that is handed `g_noalloc_scratch` itself would fault (or, on a system where the GPU can reach host memory,
+// quietly use the wrong bytes).  The host gets the real address from cudaGetSymbolAddress, once per device.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[PT_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kNoAllocMaxDevices = 64;
+void *g_noalloc_addr[kNoAllocMaxDevices] = {};      // device address of the area, per device ordinal; nullptr = not asked yet
+
+// One warp per (sample, chain).  Et = this chain's energies in temperature order (scratch), so = its slot_of_temp row
+// (walked in place).  The lanes draw 32 Philox words at a time, lane 0 walks the rungs in order (each rung sees the one
+// before, R9); same counters, same table, same comparisons as k_exchange, so the same decisions.
+__global__ void k_exchange_noalloc(int n_chains, int T, uint32_t g0, uint32_t step, uint32_t strideX, RoundKeys rk,
+                                   const uint32_t *__restrict__ thrX, const int32_t *__restrict__ sgn, int32_t *EtAll,
+                                   const int32_t *__restrict__ E, int32_t *sot, int32_t *tos, unsigned long long *accepts)
+{
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+    const long chain = (long)blockIdx.x * wpb + wib;
+    if (chain >= n_chains) return;
+    const uint32_t c = (uint32_t)(chain & 1), g = g0 + (uint32_t)(chain >> 1);
+    const size_t base = (size_t)chain * T;
+    int32_t *Et = EtAll + base, *so = sot + base;
+    for (int t = lane; t < T; t += 32) Et[t] = E[base + so[t]];
+    __syncwarp();
+    int32_t ea = 0, ra = 0;
+    if (lane == 0) { ea = Et[0]; ra = so[0]; }
+    for (int tb = 0; tb < T - 1; tb += 32) {
+        const int tl = tb + lane;
+        uint32_t u_l = 0, o1, o2, o3;
+        if (tl < T - 1) philox4x32_10((uint32_t)tl, step, g, make_tag(DOM_SWAP, 0, c, 0), rk, u_l, o1, o2, o3);
+        const int nstep = min(32, T - 1 - tb);
+        for (int j = 0; j < nstep; ++j) {
+            const uint32_t u = __shfl_sync(0xFFFFFFFFu, u_l, j);
+            if (lane == 0) {
+                const int t = tb + j;
+                const int32_t eb = Et[t + 1], rb = so[t + 1];
+                const int32_t dE = ea - eb;
+                const uint32_t m = (uint32_t)(dE < 0 ? -dE : dE) >> 2;
+                const uint32_t thr = (m < strideX) ? thrX[(size_t)t * strideX + m] : 0u;
+                const bool acc = ((long long)sgn[t] * dE <= 0) || (u < thr);
+                if (acc) {
+                    Et[t] = eb; so[t] = rb;                 // position t is final; (ea, ra) is carried up to t + 1
+                    if (accepts) accepts[(size_t)chain * (T - 1) + t] += 1ull;
+                } else {
+                    Et[t] = ea; so[t] = ra;
+                    ea = eb; ra = rb;
+                }
+            }
+        }
+    }
+    if (lane == 0) { Et[T - 1] = ea; so[T - 1] = ra; }
+    __syncwarp();
+    for (int t = lane; t < T; t += 32) tos[base + so[t]] = t;
+}
+
+}  // namespace
+
+extern "C" int pt_exchange_noalloc(int L, int d, int n_samples, int n_temps, const double *betas, uint64_t seed,
+                                   uint32_t sample_offset, uint32_t step, const int32_t *E_dev, int32_t *slot_of_temp_dev,
+                                   int32_t *temp_of_slot_dev, uint64_t *accepts_dev, void *cuda_stream)
+{
+    if (d != 2 && d != 3) return fail(PT_ERR_ARG, "pt_exchange_noalloc: d must be 2 or 3 (got %d)", d);
+    if (L < 2 || (L & 1)) return fail(PT_ERR_ARG, "pt_exchange_noalloc: L must be even and >= 2 (got %d)", L);
+    if (n_samples < 1 || n_samples > 65535) return fail(PT_ERR_ARG, "pt_exchange_noalloc: n_samples must be in [1, 65535] (got %d)", n_samples);
+    if (n_temps < 1 || n_temps > 65535) return fail(PT_ERR_ARG, "pt_exchange_noalloc: n_temps must be in [1, 65535] (got %d)", n_temps);
+    const double Nd = std::pow((double)L, d) * d;
+    if (Nd > 2147483647.0) return fail(PT_ERR_ARG, "pt_exchange_noalloc: N*d overflows int32");
+    if (!betas) return fail(PT_ERR_ARG, "pt_exchange_noalloc: betas is NULL");
+    for (int t = 0; t < n_temps; ++t)
+        if (!std::isfinite(betas[t]) || betas[t] < 0.0)
+            return fail(PT_ERR_ARG, "pt_exchange_noalloc: betas[%d] is negative or not finite", t);
+    if ((uint64_t)sample_offset + (uint64_t)n_samples > 4294967296ull)
+        return fail(PT_ERR_ARG, "pt_exchange_noalloc: sample_offset + n_samples overflows 2^32");
+    if (!E_dev || !slot_of_temp_dev || !temp_of_slot_dev)
+        return fail(PT_ERR_ARG, "pt_exchange_noalloc: E_dev, slot_of_temp_dev and temp_of_slot_dev must not be NULL");
+
+    // layout of the scratch area: threshold table | signs | energies by temperature, each 256-byte aligned
+    const long N = (d == 2) ? (long)L * L : (long)L * L * L;
+    const std::vector<double> b(betas, betas + n_temps);
+    const uint32_t strideX = swap_stride(b, d, N);
+    const size_t n_chains = (size_t)n_samples * 2;
+    const size_t table_bytes = align_up((size_t)(n_temps - 1) * strideX * 4);
+    const size_t sgn_bytes = align_up((size_t)n_temps * 4);
+    const size_t et_bytes = align_up(n_chains * (size_t)n_temps * 4);
+    const size_t need = table_bytes + sgn_bytes + et_bytes;
+    if (need > (size_t)PT_NOALLOC_SCRATCH_BYTES)
+        return fail(PT_ERR_ARG,
+                    "pt_exchange_noalloc: this problem needs %zu bytes of scratch (threshold table %zu + signs %zu + energies by "
+                    "temperature %zu) but the built-in area holds %zu: use pt_bind + pt_exchange with a caller-allocated workspace",
+                    need, table_bytes, sgn_bytes, et_bytes, (size_t)PT_NOALLOC_SCRATCH_BYTES);
+
+    // set-up, once per device, with that device current: where does this device keep the area?
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return fail(PT_ERR_CUDA, "pt_exchange_noalloc: device ordinal %d not supported", dev);
+    if (!g_noalloc_addr[dev]) {
+        void *addr = nullptr;
+        CK(cudaGetSymbolAddress(&addr, g_noalloc_scratch));
+        if (!addr) return fail(PT_ERR_CUDA, "pt_exchange_noalloc: the runtime returned no address for the scratch area");
+        g_noalloc_addr[dev] = addr;
+    }
+    char *area = (char *)g_noalloc_addr[dev];
+    uint32_t *thrX_d = (uint32_t *)area;
+    int32_t *sgn_d = (int32_t *)(area + table_bytes);
+    int32_t *Et_d = (int32_t *)(area + table_bytes + sgn_bytes);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    // tables on the host in double, as pt_init computes them (R5, R6); pageable source: the copies have left these
+    // vectors when cudaMemcpyAsync returns
+    std::vector<int32_t> sgn((size_t)n_temps, 0);
+    std::vector<uint32_t> thrX((size_t)(n_temps - 1) * strideX, 0u);
+    for (int t = 0; t + 1 < n_temps; ++t) {
+        sgn[t] = (b[t + 1] > b[t]) - (b[t + 1] < b[t]);
+        for (uint32_t m = 0; m < strideX; ++m) thrX[(size_t)t * strideX + m] = THR(thrX_arg(b, t, m));
+    }
+    if (!thrX.empty()) CK(cudaMemcpyAsync(thrX_d, thrX.data(), thrX.size() * 4, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(sgn_d, sgn.data(), sgn.size() * 4, cudaMemcpyHostToDevice, st));
+
+    const int wpb = 4;
+    k_exchange_noalloc<<<(unsigned)((n_chains + wpb - 1) / wpb), wpb * 32, 0, st>>>(
+        (int)n_chains, n_temps, sample_offset, step, strideX,
+        make_round_keys((uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32)), thrX_d, sgn_d, Et_d, E_dev, slot_of_temp_dev,
+        temp_of_slot_dev, (unsigned long long *)accepts_dev);
+    ++G.launches;
+    CK(cudaGetLastError());
+    return PT_OK;
+}
