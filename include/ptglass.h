@@ -21,7 +21,12 @@
  *    pt_init or after pt_free returns PT_ERR_STATE.
  *  - DEVICE MEMORY IS CALLER-OWNED: the caller (PyTorch) allocates one workspace of pt_workspace_bytes() bytes,
  *    256-byte aligned, and passes its raw device pointer and a cudaStream_t to pt_bind(); the library never
- *    allocates or frees device memory and launches everything on that stream.
+ *    allocates or frees device memory.  Work is queued on that stream, with one exception: where pt_mcs or
+ *    pt_set_spins_async cut the samples into groups (pt_set_sample_groups), groups 1.. run on up to 7 library-owned
+ *    non-blocking side streams, created on first use and kept until the process exits.  They start after everything queued
+ *    on the bound stream so far and the bound stream waits for them before the call returns (after pt_set_spins_async: at
+ *    the next call that touches the state), so to the caller every call is still ordered on the bound stream; pt_bind,
+ *    pt_init and pt_free synchronise them.
  *  - All `const T *` inputs are HOST pointers, caller-owned, copied during the call.  All output pointers are
  *    HOST buffers, caller-allocated with the documented shape (C order), filled after a stream synchronise.
  *    The *_device variants take DEVICE pointers instead and do not synchronise.
@@ -49,15 +54,21 @@ extern "C" {
  * state get/set calls and the init draws).  PT_ERR_ARG for shapes pt_init would reject. */
 int pt_workspace_bytes(int L, int d, int n_samples, int n_temps, size_t *bytes_out);
 /* The same with optional parts (flags OR-ed):
- *  PT_WS_FIXED_COUPLINGS  the int32 coupling arrays of the fixed-point (Gaussian) model, 24 bytes per bond (NEXT-3):
- *                         pt_init lays them out only where the bound workspace has room, and pt_set_couplings_fixed needs
- *                         them (PT_ERR_STATE otherwise);
+ *  PT_WS_FIXED_COUPLINGS  the int32 coupling arrays of the fixed-point (Gaussian) model, 24 bytes per bond (NEXT-3), which
+ *                         pt_set_couplings_fixed needs (PT_ERR_STATE without them);
  *  PT_WS_FULL_STAGING     a staging area of the whole int8 state (S*2*T*N bytes) instead of the bounded 16 MiB through
  *                         which the int8 get / set calls otherwise pass in chunks of samples: pt_set_spins_async can then
- *                         copy a whole sample group at a time.  (Any bytes bound beyond the minimum go to the staging area.) */
+ *                         copy a whole sample group at a time.
+ * pt_workspace_bytes_ex only SIZES the workspace; tell pt_init which parts it was sized for with pt_set_workspace_flags
+ * (same flags; after pt_bind, before pt_init; pt_bind resets them to 0).  pt_init never guesses from spare bytes: it lays
+ * out the int32 couplings iff PT_WS_FIXED_COUPLINGS is set, returns PT_ERR_STATE if the bound workspace is too small for
+ * the parts asked for, and gives every byte bound beyond the minimum to the staging area (up to one whole int8 state).
+ * pt_get_stage_bytes: the size the staging area ended up with (after pt_init). */
 #define PT_WS_FIXED_COUPLINGS 1
 #define PT_WS_FULL_STAGING    2
 int pt_workspace_bytes_ex(int L, int d, int n_samples, int n_temps, int flags, size_t *bytes_out);
+int pt_set_workspace_flags(int flags);
+int pt_get_stage_bytes(size_t *bytes);
 
 /* Bind the caller's device workspace (device pointer, >= pt_workspace_bytes, 256-byte aligned) and CUDA stream
  * (a cudaStream_t passed as void*; NULL = default stream).  Must precede pt_init.  Re-binding frees the context. */
@@ -73,7 +84,7 @@ int pt_bind(void *device_workspace, size_t bytes, void *cuda_stream);
  * PT_ERR_ARG: d not in {2,3}; L < 2 or odd (checkerboard needs a bipartite periodic lattice, R3); n_samples < 1 or
  * > 65535 per context (larger sets: several shards through pt_init_shard); n_temps < 1 or > 65535; betas NULL, negative
  * or non-finite; N*d > 2^31-1; a lattice whose coupling bits (4 d N / 8 bytes per sample) plus one replica exceed the
- * 227 KiB of shared memory of a CTA (2D: L > 608, 3D: L > 62); sample_offset+n_samples > 2^32.
+ * 227 KiB of shared memory of a CTA (2D: L > 608, 3D: L > 64); sample_offset+n_samples > 2^32.
  * PT_ERR_STATE: no workspace bound or workspace too small. */
 int pt_init(int L, int d, int n_samples, int n_temps, const double *betas, uint64_t seed);
 /* Same, for a shard holding global samples [sample_offset, sample_offset + n_samples) (multi-GPU). */
@@ -119,7 +130,8 @@ int houdayer_step(void);
  * the Philox block ctr = (i_min >> 2, step, g, tag(5, aux 1, 0, t)) is set.  E1 + E2 is conserved for any such union
  * (P:138).  last / cumulative count exchanged sites; the Houdayer step counter advances by one.  Components are found by
  * label propagation in shared memory, one CTA per (sample, temperature): PT_ERR_ARG if 6 N bytes of labels and site list do not
- * fit (N <= ~36000 sites: up to 2D L = 128, 3D L = 32).  In pt_mcs it is do_houdayer = 2 (separate kernels, not fused). */
+ * fit (N <= ~36000 sites: up to 2D L = 128, 3D L = 32).  In pt_mcs it is do_houdayer = 2: inside the fused launch on the 2D
+ * L = 32 lattice with +-J couplings (components by a tournament on bit maps), separate kernels on every other lattice. */
 int pt_set_cluster_moves(const int32_t *n_clu);
 int houdayer_multi_step(void);
 
@@ -289,8 +301,9 @@ int pt_get_kernel_times(double ms[5], uint64_t launches[5]);
  * the samples are cut into n groups, each issuing its sweep -> cluster -> exchange chain on its own stream (group 0 on the
  * bound stream, the others on library-owned side streams that fork from and join the bound stream inside the call), so
  * that the low-occupancy tail of one group's cluster kernel and its latency-bound exchange kernel overlap another group's
- * sweep.  Samples never interact (P:7), so results are bit-identical for every n.  n = -1: automatic (up to 3 groups while
- * each group still fills the GPU twice over); n = 1: one stream (used for per-kernel timing). */
+ * sweep.  Samples never interact (P:7), so results are bit-identical for every n.  n = -1: automatic (one group per wave
+ * of sweep CTAs -- SMs x resident CTAs per SM, both asked from the runtime -- at most 8 and at most S; BASELINE config 5
+ * runs 6); n in 1..8 (larger values are taken as 8): that many groups; n = 1: one stream (used for per-kernel timing). */
 int pt_set_sample_groups(int n);
 /* Phase split of the FUSED launch (pt_mcs where one CTA keeps a sample resident): CUDA events cannot separate the
  * Metropolis sweeps, the Houdayer moves and the PT pass inside one kernel, so when on, thread 0 of every CTA sums the SM
@@ -317,6 +330,9 @@ int pt_threshold_selftest(const double *x, uint32_t *out, int n);
  * DEVICE memory.  Returns sustained thread-operations per ns (best of 3 after a warm-up) and the kernel time. */
 int pt_microbench(int kind, int ctas_per_sm, int iters, void *device_scratch, void *cuda_stream,
                   double *thread_ops_per_ns, double *ms_out);
+/* 1 if this libptglass.so is a development build (PTG_DEV_LATTICE: kernels of one lattice dimension only; pt_init then
+ * refuses the other dimension with PT_ERR_ARG), 0 for the full library.  Benchmarks and tests assert 0. */
+int pt_is_dev_build(void);
 const char *pt_last_error(void);
 
 #ifdef __cplusplus

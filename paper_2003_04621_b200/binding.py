@@ -22,6 +22,9 @@ _vp, _i, _sz = C.c_void_p, C.c_int, C.c_size_t
 SYMBOLS = {
     "pt_workspace_bytes": (_i, [_i, _i, _i, _i, C.POINTER(_sz)]),
     "pt_workspace_bytes_ex": (_i, [_i, _i, _i, _i, _i, C.POINTER(_sz)]),
+    "pt_set_workspace_flags": (_i, [_i]),
+    "pt_get_stage_bytes": (_i, [C.POINTER(_sz)]),
+    "pt_is_dev_build": (_i, []),
     "pt_bind": (_i, [_vp, _sz, _vp]),
     "pt_init": (_i, [_i, _i, _i, _i, _vp, C.c_uint64]),
     "pt_init_shard": (_i, [_i, _i, _i, _i, _vp, C.c_uint64, C.c_uint32]),
@@ -135,6 +138,21 @@ def pt_workspace_bytes_ex(L, d, n_samples, n_temps, flags) -> int:
     return n.value
 
 
+def pt_set_workspace_flags(flags):
+    """Which optional parts (PT_WS_*) the bound workspace was sized for; after pt_bind, before pt_init."""
+    _ck(lib().pt_set_workspace_flags(int(flags)))
+
+
+def pt_get_stage_bytes() -> int:
+    n = _sz(0)
+    _ck(lib().pt_get_stage_bytes(C.byref(n)))
+    return n.value
+
+
+def pt_is_dev_build() -> int:
+    return int(lib().pt_is_dev_build())
+
+
 def pt_bind(workspace, stream=None):
     """workspace: a CUDA uint8 torch tensor; stream: torch.cuda.Stream or None (current stream)."""
     global _workspace
@@ -179,6 +197,7 @@ def pt_open(L, d, n_samples, n_temps, betas, seed, sample_offset=0, device="cuda
     ws = torch.empty(nbytes, dtype=torch.uint8, device=device)
     with torch.cuda.device(ws.device):
         pt_bind(ws, stream)
+        pt_set_workspace_flags(flags)
         if general:
             pt_force_general_path(0)
         if track_round_trips:

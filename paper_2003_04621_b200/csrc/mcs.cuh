@@ -337,7 +337,7 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
         if (clk) phase_stamp(sPh, 1);
         // ---- a4: PT pass (R9: sequential walk, each step seeing the previous).  Warp 0: all lanes draw the Philox
         // words, then one lane per chain walks its ladder; only the two index maps change.
-        // Measured and rejected on B200 (profiles/r2_fused_phases.md): a decision table over all (carried, rung) pairs built
+        // Measured and rejected on B200: a decision table over all (carried, rung) pairs built
         // by the whole CTA (2.6 K instructions per sample and MCS against 1.6 K for this walk; C2 929 against 961 flips/ns),
         // the rungs' own-resident decisions evaluated side by side with a warp per chain (939), and a banded table with a
         // speculative accept-bit walk and a parallel rebuild of the map (PT phase 12.4 -> 9.5 us of CTA time, but C2 952,
@@ -345,6 +345,10 @@ __global__ void __launch_bounds__(NT, MINB) k_mcs(LAT lat, Params P, McsArgs a)
         // (a rung = a map on the number of rungs the arriving replica was carried, composed over the ladder in 5 shuffle
         // steps, the map rebuilt in parallel from the accept mask): PT phase 12.4 -> 7.8 us of CTA time, bit-exact, and C2 969,
         // C3 1005, C4 1153 against 959 / 1011 / 1152 -- the phase is no longer what limits the kernel, so the walk stays.
+        // Round 3: the threshold of rung t + 1 fetched one rung ahead for both replicas that can arrive there (two independent
+        // loads in flight, selected by the decision at t): bit-exact, and SLOWER -- C2 943 / C3 918 / C4 1133 against 958 / 950 /
+        // 1151 flips/ns (same box, three alternating runs, plain pt_mcs): twice the loads and six more live registers on the
+        // one lane that walks cost more than the shorter dependency chain returns.
         if (a.do_exchange && T > 1) {
             const uint32_t step = a.exch0 + (uint32_t)m;
             if (wid == 0) {

@@ -41,7 +41,9 @@ struct Context {
     int sample_groups = -1;     // pt_set_sample_groups: -1 = automatic
     int pending_groups = 0;     // > 0: pt_set_spins_async left work of that many sample groups on the side streams
     bool async_check = false;   // the +-1 count of a pt_set_spins_async has not been read yet
-    bool has_fixed = false;     // the workspace holds the int32 coupling arrays (pt_workspace_bytes_fixed)
+    bool has_fixed = false;     // the workspace holds the int32 coupling arrays (PT_WS_FIXED_COUPLINGS)
+    int ws_flags = 0;           // pt_set_workspace_flags: the optional parts the caller sized the workspace for
+    int n_sm = 148, sweep_occ = 7;  // SMs of the device and resident k_sweep CTAs per SM, asked from the runtime in pt_init
     int phase_clocks = 0;       // pt_set_phase_clocks
     int max_clu = 1;            // max over t of the per-temperature cluster-move counts (NEXT-4, R36)
     uint64_t launches = 0;
@@ -483,13 +485,15 @@ cudaError_t ensure_side_streams(int n)
     return e;
 }
 
-// sample groups of a separate-kernel pt_mcs call.  Automatic: one group per wave of sweep CTAs (148 SMs x 7 CTAs), at most
-// kMaxGroups -- measured on C5 (5.9 waves): 1 group 733, 2: 811, 4: 852, 6: 862, 8: 862 flips/ns.
+// sample groups of a separate-kernel pt_mcs call.  Automatic: one group per wave of sweep CTAs (SMs x resident CTAs per SM,
+// both from the runtime: 148 x 7 on a B200), at most kMaxGroups -- measured on C5 (5.9 waves): 1 group 733, 2: 811, 4: 852,
+// 6: 862, 8: 862 flips/ns.
 int mcs_groups()
 {
     if (G.sample_groups > 0) return std::min(std::min(G.sample_groups, kMaxGroups), G.P.S);
     const long ctas = (long)G.P.S * (2 * G.P.T / sweep_group(G.P.T, G.P.W));     // sweep CTAs of the whole problem
-    const long waves = (ctas + 148L * 7 - 1) / (148L * 7);
+    const long wave = (long)G.n_sm * G.sweep_occ;
+    const long waves = (ctas + wave - 1) / wave;
     return (int)std::max(1L, std::min<long>(std::min<long>(waves, kMaxGroups), G.P.S));
 }
 
@@ -697,12 +701,16 @@ int run_fused(McsArgs a)
     int rc = make_groups(NG, g);
     if (rc) return rc;
     if ((rc = fork_groups(g))) return rc;
-    for (int k = 0; k < NG; ++k) {
-        a.rec_s0 = g.s0[k];
-        CK(launch_mcs(a, g.view[k], g.st[k]));
-    }
+    rc = [&]() -> int {
+        for (int k = 0; k < NG; ++k) {
+            a.rec_s0 = g.s0[k];
+            CK(launch_mcs(a, g.view[k], g.st[k]));
+        }
+        return PT_OK;
+    }();
     G.pending_groups = 0;
-    return join_groups(NG);
+    const int rcj = join_groups(NG);        // also after a failed launch: the side streams never stay forked
+    return rc ? rc : rcj;
 }
 
 }  // namespace
@@ -753,6 +761,32 @@ int pt_bind(void *device_workspace, size_t bytes, void *cuda_stream)
     return PT_OK;
 }
 
+int pt_set_workspace_flags(int flags)
+{
+    if (!G.bound) return fail(PT_ERR_STATE, "pt_set_workspace_flags: no workspace bound");
+    if (G.inited) return fail(PT_ERR_STATE, "pt_set_workspace_flags must precede pt_init (the workspace is laid out there)");
+    if (flags & ~(PT_WS_FIXED_COUPLINGS | PT_WS_FULL_STAGING)) return fail(PT_ERR_ARG, "unknown workspace flag");
+    G.ws_flags = flags;
+    return PT_OK;
+}
+
+int pt_get_stage_bytes(size_t *bytes)
+{
+    NEED_INIT_NOJOIN();
+    if (!bytes) return fail(PT_ERR_ARG, "bytes is NULL");
+    *bytes = G.stage_bytes;
+    return PT_OK;
+}
+
+int pt_is_dev_build(void)
+{
+#ifdef PTG_DEV_D
+    return 1;
+#else
+    return 0;
+#endif
+}
+
 int pt_force_general_path(int force)
 {
     if (force != -1 && force != 0) return fail(PT_ERR_ARG, "force must be -1 or 0");
@@ -777,6 +811,10 @@ int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas,
     G.async_check = false;
     int rc = check_shape(L, d, n_samples, n_temps);
     if (rc) return rc;
+#ifdef PTG_DEV_D
+    // development build (PTG_DEV_LATTICE): only lattices of this dimension were compiled; never run the other one on them
+    if (d != PTG_DEV_D) return fail(PT_ERR_ARG, "development build for d = %d only (got d = %d): rebuild without PTG_DEV_LATTICE", PTG_DEV_D, d);
+#endif
     if (!betas) return fail(PT_ERR_ARG, "betas is NULL");
     for (int t = 0; t < n_temps; ++t)
         if (!std::isfinite(betas[t]) || betas[t] < 0.0) return fail(PT_ERR_ARG, "betas[%d] is negative or not finite", t);
@@ -796,14 +834,34 @@ int pt_init_shard(int L, int d, int n_samples, int n_temps, const double *betas,
     P.strideX = swap_stride(G.betas, d, P.N);
     P.track = G.track;
     P.thrJ = (unsigned long long)std::floor(std::ldexp(G.p_ferro, 32));
-    // the int32 coupling arrays of the fixed-point model are laid out only where the bound workspace has room for them
-    G.has_fixed = carve(nullptr, L, d, n_samples, n_temps, P.strideX, nullptr, nullptr, true) <= G.ws_bytes;
+    // the int32 coupling arrays of the fixed-point model are laid out only where the caller asked for them
+    // (pt_set_workspace_flags); spare bytes never decide it
+    G.has_fixed = (G.ws_flags & PT_WS_FIXED_COUPLINGS) != 0;
     const size_t need = carve(nullptr, L, d, n_samples, n_temps, P.strideX, nullptr, nullptr, G.has_fixed);
     if (need > G.ws_bytes)
-        return fail(PT_ERR_STATE, "workspace too small: %zu bytes bound, %zu needed", G.ws_bytes, need);
+        return fail(PT_ERR_STATE, "workspace too small: %zu bytes bound, %zu needed%s", G.ws_bytes, need,
+                    G.has_fixed ? " (with PT_WS_FIXED_COUPLINGS)" : "");
     // whatever the caller bound beyond the minimum enlarges the staging area (PT_WS_FULL_STAGING: a whole int8 state)
     carve(G.ws, L, d, n_samples, n_temps, P.strideX, &P.d, &G.stage_bytes, G.has_fixed, (G.ws_bytes - need) & ~(size_t)255);
+    if ((G.ws_flags & PT_WS_FULL_STAGING) && G.stage_bytes < (size_t)n_samples * 2 * n_temps * (size_t)P.N)
+        return fail(PT_ERR_STATE, "workspace too small for PT_WS_FULL_STAGING: staging area %zu bytes, whole int8 state %zu",
+                    G.stage_bytes, (size_t)n_samples * 2 * n_temps * (size_t)P.N);
     G.fast = (G.force_general != 0) && fast_supported(L, d);
+    {   // what one wave of sweep CTAs is on THIS device (mcs_groups)
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+            G.n_sm = n;
+        with_lattice([&](auto lat) {
+            using LAT = decltype(lat);
+            const int R = sweep_group(P.T, P.W);
+            const size_t smem = ((size_t)2 * 2 * P.D * P.W + (size_t)R * 2 * P.W + (size_t)R * 4 + (size_t)R) * 4;
+            int nb = 0;
+            if (allow_smem(k_sweep<LAT>, smem) == cudaSuccess &&
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_sweep<LAT>, 128, smem) == cudaSuccess && nb > 0)
+                G.sweep_occ = nb;
+        });
+        cudaGetLastError();      // a failed query must not poison the calls that follow
+    }
     G.n_sweep = G.n_exchange = G.n_houdayer = 0;
     G.n_passes = 0;
     G.max_clu = 1;
@@ -976,14 +1034,19 @@ int pt_mcs(int n_mcs, int n_metro, int do_houdayer, int do_exchange)
     int rcg = make_groups(NG, g);
     if (rcg) return rcg;
     if ((rcg = fork_groups(g))) return rcg;
-    for (int m = 0; m < n_mcs; ++m)
-        for (int k = 0; k < NG; ++k) {
-            if (n_metro > 0) CK(launch_sweep(n_metro, G.n_sweep + (uint32_t)m * (uint32_t)n_metro, g.view[k], g.st[k]));
-            if (do_houdayer) CK(launch_houdayer_any(do_houdayer, G.n_houdayer + (uint32_t)m, g.view[k], g.st[k]));
-            if (do_exchange) CK(launch_exchange(G.n_exchange + (uint32_t)m, g.view[k], g.st[k]));
-        }
+    rcg = [&]() -> int {
+        for (int m = 0; m < n_mcs; ++m)
+            for (int k = 0; k < NG; ++k) {
+                if (n_metro > 0) CK(launch_sweep(n_metro, G.n_sweep + (uint32_t)m * (uint32_t)n_metro, g.view[k], g.st[k]));
+                if (do_houdayer) CK(launch_houdayer_any(do_houdayer, G.n_houdayer + (uint32_t)m, g.view[k], g.st[k]));
+                if (do_exchange) CK(launch_exchange(G.n_exchange + (uint32_t)m, g.view[k], g.st[k]));
+            }
+        return PT_OK;
+    }();
     G.pending_groups = 0;
-    if ((rcg = join_groups(NG))) return rcg;
+    const int rcj = join_groups(NG);        // also after a failed launch: the side streams never stay forked
+    if (rcg) return rcg;
+    if (rcj) return rcj;
     G.n_sweep += (uint32_t)(M * (uint64_t)n_metro);
     if (do_houdayer) G.n_houdayer += (uint32_t)M;
     if (do_exchange) { G.n_exchange += (uint32_t)M; G.n_passes += M; }
@@ -1353,24 +1416,34 @@ int pt_set_spins_async(const int8_t *spins)
     if (!spins) return fail(PT_ERR_ARG, "spins is NULL");
     const size_t per_sample = (size_t)2 * G.P.T * G.P.N;
     int ng = upload_groups();
-    while (ng > 1 && G.stage_bytes / ng < per_sample) --ng;            // every group needs room for one sample
+    // every group needs room for one sample in ITS region, which starts on a 256-byte boundary
+    const auto region_of = [&](int n) { return n == 1 ? G.stage_bytes : (G.stage_bytes / n) & ~(size_t)255; };
+    while (ng > 1 && region_of(ng) < per_sample) --ng;
     Groups g;
     int rc = make_groups(ng, g);
     if (rc) return rc;
     CK(cudaMemsetAsync(G.P.d.mismatch + 2, 0, sizeof(int), G.stream));
     if ((rc = fork_groups(g))) return rc;
     const bool whole = G.stage_bytes >= (size_t)G.P.S * per_sample;     // PT_WS_FULL_STAGING: every group in one copy, at its own offset
-    for (int k = 0; k < g.n; ++k) {
-        const size_t region = whole ? (size_t)g.view[k].S * per_sample : (G.stage_bytes / ng) & ~(size_t)255;
-        int8_t *stage_k = G.P.d.stage + (whole ? (size_t)g.s0[k] * per_sample : (size_t)k * region);
-        cudaStream_t st = g.st[k];
-        // copy -> pack, chunk after chunk in the group's stream (the next copy into the region waits for the pack before it)
-        rc = for_chunks(per_sample, region, g.s0[k], g.s0[k] + g.view[k].S, [&](const Params &V, int s0, int n) {
-            CK(cudaMemcpyAsync(stage_k, spins + (size_t)s0 * per_sample, (size_t)n * per_sample, cudaMemcpyHostToDevice, st));
-            return pack_spins(V, st, stage_k, G.P.d.mismatch + 2);
-        });
-        if (rc) return rc;
-        CK(launch_energy(0, g.view[k], st));
+    rc = [&]() -> int {
+        for (int k = 0; k < g.n; ++k) {
+            const size_t region = whole ? (size_t)g.view[k].S * per_sample : region_of(ng);
+            int8_t *stage_k = G.P.d.stage + (whole ? (size_t)g.s0[k] * per_sample : (size_t)k * region);
+            cudaStream_t st = g.st[k];
+            // copy -> pack, chunk after chunk in the group's stream (the next copy into the region waits for the pack before it)
+            const int rck = for_chunks(per_sample, region, g.s0[k], g.s0[k] + g.view[k].S, [&](const Params &V, int s0, int n) {
+                CK(cudaMemcpyAsync(stage_k, spins + (size_t)s0 * per_sample, (size_t)n * per_sample, cudaMemcpyHostToDevice, st));
+                return pack_spins(V, st, stage_k, G.P.d.mismatch + 2);
+            });
+            if (rck) return rck;
+            CK(launch_energy(0, g.view[k], st));
+        }
+        return PT_OK;
+    }();
+    if (rc) {                                // never return with the side streams forked
+        G.pending_groups = 0;
+        join_groups(g.n);
+        return rc;
     }
     G.pending_groups = g.n > 1 ? g.n : 0;
     G.async_check = true;
@@ -1461,8 +1534,9 @@ int pt_set_couplings_fixed(const int32_t *Jq, int frac_bits)
     if (!Jq) return fail(PT_ERR_ARG, "Jq is NULL");
     if (frac_bits < 0 || frac_bits > 24) return fail(PT_ERR_ARG, "frac_bits must be in [0, 24]");
     if (!G.has_fixed)
-        return fail(PT_ERR_STATE, "pt_set_couplings_fixed: the bound workspace has no room for int32 couplings "
-                                  "(bind pt_workspace_bytes_ex(..., PT_WS_FIXED_COUPLINGS, ...) bytes before pt_init)");
+        return fail(PT_ERR_STATE, "pt_set_couplings_fixed: the workspace was laid out without int32 couplings (bind "
+                                  "pt_workspace_bytes_ex(..., PT_WS_FIXED_COUPLINGS, ...) bytes and call "
+                                  "pt_set_workspace_flags(PT_WS_FIXED_COUPLINGS) before pt_init)");
     const size_t n = (size_t)G.P.S * G.P.D * G.P.N;
     long long maxabs = 0;
     for (size_t k = 0; k < n; ++k) maxabs = std::max<long long>(maxabs, Jq[k] < 0 ? -(long long)Jq[k] : (long long)Jq[k]);
@@ -1596,6 +1670,8 @@ int pt_philox_selftest(const uint32_t key[2], const uint32_t *ctr, uint32_t *out
 {
     if (!G.bound) return fail(PT_ERR_STATE, "pt_philox_selftest: no workspace bound");
     if (!key || !ctr || !out || n < 1) return fail(PT_ERR_ARG, "bad arguments");
+    // an asynchronous upload may still be copying into the staging area
+    if (G.inited && G.pending_groups) { const int rcj = join_pending(); if (rcj) return rcj; }
     // scratch: the staging area when initialised, else the start of the workspace
     char *scratch = G.inited ? (char *)G.P.d.stage : (char *)G.ws;
     const size_t avail = G.inited ? G.stage_bytes : G.ws_bytes;

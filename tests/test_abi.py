@@ -25,6 +25,7 @@ def test_header_symbols_all_exported(lib):
     assert names == set(B.SYMBOLS), names ^ set(B.SYMBOLS)
     for n in names:
         assert hasattr(lib, n)
+    assert B.pt_is_dev_build() == 0, "tests must run on the full library, not a PTG_DEV_LATTICE build"
 
 
 def test_workspace_bytes_and_shape_errors(lib):

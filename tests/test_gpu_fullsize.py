@@ -14,7 +14,7 @@ import pytest
 from oracle import ref
 from paper_2003_04621_b200 import binding as B
 from paper_2003_04621_b200 import build as build_mod
-from paper_2003_04621_b200 import workloads as wl
+import workloads as wl
 from oracle import pool as OP
 
 pytestmark = pytest.mark.gpu
@@ -161,6 +161,10 @@ def test_int8_state_round_trip_through_the_staging_area_at_full_size(full_stagin
     import torch
     w = wl.C2
     B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED, full_staging=full_staging)
+    # the flag delivers what the header promises: the whole int8 state, or the bounded 16 MiB
+    # (without it: 16 MiB plus the few bytes pt_workspace_bytes reserved for a swap table of the largest possible stride)
+    sb = B.pt_get_stage_bytes()
+    assert sb == w.S * 2 * w.T * w.N if full_staging else (16 << 20) <= sb < (17 << 20)
     B.pt_mcs(3, 1, True, True)
     spins, E = B.pt_get_spins(), B.pt_get_energy()
     B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED, full_staging=full_staging)
