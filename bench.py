@@ -37,7 +37,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2003_04621_b200 import workloads as wl  # noqa: E402
+import workloads as wl  # noqa: E402
 
 METRIC = "attempted_spin_flips_per_ns"
 UNIT = "flips/ns"
@@ -125,6 +125,17 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
+def shorten(x):
+    """Floats to 5 significant digits (the JSON line is read by people and kept by its tail)."""
+    if isinstance(x, float):
+        return float("%.5g" % x)
+    if isinstance(x, dict):
+        return {k: shorten(v) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [shorten(v) for v in x]
+    return x
+
+
 def cpu_model():
     try:
         with open("/proc/cpuinfo") as f:
@@ -134,6 +145,15 @@ def cpu_model():
     except Exception:
         pass
     return "unknown"
+
+
+def gauss_fbits(w):
+    """Fractional bits of the fixed-point Gaussian couplings (NEXT-3): 16 where the int32 energies allow it, else the most
+    that keep d * N * max|Jq| below 2^31 with |J| < 6 sigma (C5's 2D L=128: 12)."""
+    f = 16
+    while f > 0 and w.d * w.N * 6.0 * (1 << f) >= 2.0 ** 31:
+        f -= 1
+    return f
 
 
 def cluster_args(a, w):
@@ -154,7 +174,7 @@ def oracle_rate(a, w, procs, samples_per_proc, target_flips_per_proc):
     hd, n_clu = cluster_args(a, w)
     fixed = None
     if a.gaussian:
-        fixed = (wl.gaussian_couplings_fixed(wl.SEED, procs * samples_per_proc, w.d, w.N, 16), 16)
+        fixed = (wl.gaussian_couplings_fixed(wl.SEED, procs * samples_per_proc, w.d, w.N, gauss_fbits(w)), gauss_fbits(w))
     n_mcs = max(1, int(target_flips_per_proc / w.flips_per_sweep(samples_per_proc)))
     po = OP.PersistentOracles(w, procs, samples_per_proc, houdayer_mode=hd, fixed=fixed,
                               n_clu=None if n_clu is None else n_clu.tolist())
@@ -177,7 +197,7 @@ def run_reference(a, w, rank):
 
     P = OP.n_cores()
     hd, n_clu = cluster_args(a, w)
-    fixed = (wl.gaussian_couplings_fixed(wl.SEED, P, w.d, w.N, 16), 16) if a.gaussian else None
+    fixed = (wl.gaussian_couplings_fixed(wl.SEED, P, w.d, w.N, gauss_fbits(w)), gauss_fbits(w)) if a.gaussian else None
     ref_mcs = max(1, min(a.mcs_per_step, int(round(0.25 / (w.flips_per_sweep(1) * 30e-9)))))
     po = OP.PersistentOracles(w, P, 1, houdayer_mode=hd, fixed=fixed, n_clu=None if n_clu is None else n_clu.tolist())
     try:
@@ -209,7 +229,7 @@ def config_of(a, w, n_gpus, sample=None):
          "mcs_per_step": a.mcs_per_step, "mcs_order": "sweep" + (", houdayer" if w.houdayer else "") + ", exchange",
          "measure_every": w.measure_every, "seed": wl.SEED, "parallelism": "samples sharded x%d" % n_gpus,
          "l2": "flushed between steps (512 MiB write, untimed)", "round_trip_tracking": bool(a.track_round_trips),
-         "couplings": "gaussian, fixed point 2^-16 (NEXT-3)" if a.gaussian else "+-J, p = 1/2",
+         "couplings": "gaussian, fixed point 2^-%d (NEXT-3)" % gauss_fbits(w) if a.gaussian else "+-J, p = 1/2",
          "cluster_move": {"single": "one single-cluster move per temperature", "counts": "single-cluster moves, counts 4..1 hot to cold (NEXT-4)",
                           "multi": "multi-cluster exchange (NEXT-4)"}[a.cluster] if w.houdayer else "none"}
     if sample:
@@ -226,17 +246,39 @@ class GpuRun:
         from paper_2003_04621_b200 import binding as B
 
         self.a, self.w, self.rank, self.world, self.dev, self.flush, self.B, self.torch = a, w, rank, world, dev, flush, B, torch
-        B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED, sample_offset=rank * w.S, device=dev,
-                  track_round_trips=a.track_round_trips, fixed_couplings=a.gaussian, full_staging=True)
-        if a.gaussian:
-            B.pt_set_couplings_fixed(wl.gaussian_couplings_fixed(wl.SEED, w.S, w.d, w.N, 16, sample_offset=rank * w.S), 16)
-        self.hd, n_clu = cluster_args(a, w)
-        if n_clu is not None:
-            B.pt_set_cluster_moves(n_clu)
+        self.Jq = wl.gaussian_couplings_fixed(wl.SEED, w.S, w.d, w.N, gauss_fbits(w), sample_offset=rank * w.S) if a.gaussian else None
+        self.open()
         self.n_meas = (a.mcs_per_step // w.measure_every) if w.measure_every else 0
         self.Qrec = torch.empty((max(self.n_meas, 1), w.S, w.T), dtype=torch.int32, device=dev)
         self.QLrec = torch.empty_like(self.Qrec)
         self.flips_step = w.flips_per_sweep() * a.mcs_per_step
+
+    def open(self):
+        """pt_init of the workload (not timed): the state of MCS 0; same seed, same trajectory every time."""
+        a, w, B = self.a, self.w, self.B
+        B.pt_open(w.L, w.d, w.S, w.T, w.betas(), wl.SEED, sample_offset=self.rank * w.S, device=self.dev,
+                  track_round_trips=a.track_round_trips, fixed_couplings=a.gaussian, full_staging=True)
+        if self.Jq is not None:
+            B.pt_set_couplings_fixed(self.Jq, gauss_fbits(w))
+        self.hd, n_clu = cluster_args(a, w)
+        if n_clu is not None:
+            B.pt_set_cluster_moves(n_clu)
+
+    def from_mcs0(self, steps):
+        """SURVEY 8(d) timing protocol: the same run timed FROM MCS 0 (a fresh pt_init, the kernels already loaded by
+        the passes before it), next to the steady-state window (MCS >= 128) the warmed-up timed region covers."""
+        torch = self.torch
+        self.open()
+        self.barrier()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for k in range(steps):
+            self.flush.fill_(k & 0xFF)
+            evs[k][0].record()
+            self.step()
+            evs[k][1].record()
+        self.barrier()
+        ms = self.max_over_ranks(sum(e0.elapsed_time(e1) for e0, e1 in evs))
+        return {"value": self.world * self.flips_step * steps / (ms * 1e6), "mcs": [0, steps * self.a.mcs_per_step]}
 
     def step(self):
         if self.n_meas == 0:
@@ -277,11 +319,16 @@ class GpuRun:
             evs[k][1].record()
         self.barrier()
         t1 = time.time()
-        ms_total = self.max_over_ranks(sum(e0.elapsed_time(e1) for e0, e1 in evs))
+        ms_steps = [e0.elapsed_time(e1) for e0, e1 in evs]
+        ms_total = self.max_over_ranks(sum(ms_steps))
         launches = B.pt_get_launch_count() - launches0
         assert B.pt_recompute_energy()[1] == 0, "tracked energies diverged from recomputed energies"
+        # the steps are the repetitions (same work every step): median / min / max of this rank's per-step event times
+        stats = {"median": float(np.median(ms_steps)), "min": float(np.min(ms_steps)), "max": float(np.max(ms_steps))}
         return {"value": self.world * self.flips_step * steps / (ms_total * 1e6), "ms_per_step": ms_total / steps,
-                "ms_total": ms_total, "steps": steps, "gpu_launches": int(launches),
+                "ms_total": ms_total, "steps": steps, "gpu_launches": int(launches), "ms_step_stats": stats,
+                "value_median_step": self.world * self.flips_step / (stats["median"] * 1e6),
+                "mcs": [warmup * self.a.mcs_per_step, (warmup + steps) * self.a.mcs_per_step],
                 "clocks": sampler.window(t0, t1) if sampler else None}
 
     def instrumented(self, steps, t):
@@ -324,25 +371,23 @@ class GpuRun:
             per_mcs_us = t["ms_per_step"] / a.mcs_per_step * 1e3
             ph = {"metropolis": share[0] * per_mcs_us, "houdayer": share[1] * per_mcs_us, "exchange": share[2] * per_mcs_us,
                   "rest": share[3] * per_mcs_us}
-            how = "fused launch: un-instrumented time per MCS x the CTA clock64() share of each phase (pt_set_phase_clocks)"
+            how = "fused launch: time per MCS x clock64() share of each phase"
         else:
             ph = {"metropolis": kms[0] / n_mcs_pass * 1e3, "houdayer": kms[1] / n_mcs_pass * 1e3,
                   "exchange": kms[2] / n_mcs_pass * 1e3, "rest": max(pass_ms - kms[:4].sum(), 0.0) / n_mcs_pass * 1e3}
-            how = ("separate launches: CUDA events around every launch of the instrumented pass, which runs on ONE stream "
-                   "(pt_set_sample_groups(1)); rest = gaps between launches; the timed region overlaps sample groups on streams")
+            how = "separate launches: CUDA events per launch, instrumented pass on ONE stream; rest = gaps"
         phases = {"us_per_mcs": ph, "ns_per_spin": {k: v * 1e3 / spins_mcs for k, v in ph.items()},
                   "houdayer_over_metropolis": (ph["houdayer"] / ph["metropolis"]) if ph["metropolis"] > 0 else None,
                   "exchange_over_metropolis": (ph["exchange"] / ph["metropolis"]) if ph["metropolis"] > 0 else None,
-                  "how": how, "paper": "cluster update 2-5x the Metropolis time per spin (P:197); PT small (P:231)"}
+                  "how": how}
         traffic = NCU_TRAFFIC.get((w.name, KERNEL_CLASSES[dom])) if not a.gaussian and a.cluster == "single" else None
         roofline = {
             "bound": "alu", "kernel": KERNEL_CLASSES[dom], "achieved": A * dom_flips_ns, "peak": peak_ops,
             "unit": "Gop/s (INT32 thread-ops)", "frac": A * dom_flips_ns / peak_ops,
             "traffic": traffic[0] if traffic else None,
-            "traffic_source": traffic[1] if traffic else None,
-            "peak_how": "derived: 148 SMs x 128 INT32 lanes/clk (fma+alu pipes) x %.3f GHz max SM clock; achieved = A x attempted flips "
-                        "per launch / launch time with A = %d ALGORITHMIC ops/flip (Philox 10 + field 2d + decide 6), not an ncu counter; "
-                        "a %s launch = %d MCS = %d attempted flips" % (f_max, A, KERNEL_CLASSES[dom], mcs_per_launch, flips_per_launch),
+            "traffic_source": traffic[1].split(":")[0] if traffic else None,        # the file; profiles/ncu_traffic.csv has the details
+            "peak_how": "148 SMs x 128 INT32 lanes/clk x %.3f GHz; achieved = %d algorithmic ops/flip (SURVEY 8(d)) x flips per launch / "
+                        "launch time; a %s launch = %d MCS = %d flips" % (f_max, A, KERNEL_CLASSES[dom], mcs_per_launch, flips_per_launch),
             "flips_per_ns": dom_flips_ns, "ms_per_launch": dom_ms,
             "whole_mcs_frac": A * t["value"] / self.world / peak_ops,
             "hbm": {"algorithmic_bytes_per_flip": 0.25 / mcs_per_launch, "achieved_gbs": 0.25 / mcs_per_launch * dom_flips_ns,
@@ -387,6 +432,7 @@ class GpuRun:
     def e2e(self, steps):
         """End to end through the C ABI with HOST buffers: H2D of the int8 spins, the step, D2H of the energies."""
         torch, B, w = self.torch, self.B, self.w
+        assert B.pt_get_stage_bytes() == w.S * 2 * w.T * w.N, "PT_WS_FULL_STAGING not delivered"
         host_spins = torch.empty((w.S, 2, w.T, w.N), dtype=torch.int8).pin_memory()
         host_E = torch.empty((w.S, 2, w.T), dtype=torch.int32).pin_memory()
         hs, hE = host_spins.numpy(), host_E.numpy()
@@ -444,6 +490,7 @@ def main():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
     if rank == 0:
         build_mod.build()
+    assert B.pt_is_dev_build() == 0, "libptglass.so is a development build (PTG_DEV_LATTICE): rebuild the full library"
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
         dist.barrier()
@@ -471,11 +518,23 @@ def main():
     roofline["measurement_us_per_call"] = run.measurement_kernels()
     fast_path = bool(B.pt_get_path())
 
-    # ---- the other configs, same run, same protocol with fewer steps (N = 1 only: they are not part of the scaling line)
-    per_config = None
+    mcs0 = run.from_mcs0(max(a.warmup, 1))
+
+    # ---- the other configs, same run, same protocol with fewer steps (N = 1 only: they are not part of the scaling line).
+    # Numbers only (the prose that explains them is in the headline's roofline block and in DESIGN.md 9): the driver keeps
+    # the TAIL of the line, so it is kept short and ends with `summary`.
+    def compact(tc, rf, m0):
+        ph = rf["phases"]["us_per_mcs"]
+        return {"value": tc["value"], "ms_per_step": tc["ms_per_step"], "ms_step_stats": tc["ms_step_stats"], "steps": tc["steps"],
+                "gpu_launches": tc["gpu_launches"], "sm_mhz": (tc["clocks"] or {}).get("sm_mhz"),
+                "reasons": (tc["clocks"] or {}).get("reasons"), "kernel": rf["kernel"], "frac": rf["frac"],
+                "whole_mcs_frac": rf["whole_mcs_frac"], "kernel_flips_per_ns": rf["flips_per_ns"], "ms_per_launch": rf["ms_per_launch"],
+                "sweep_only_flips_per_ns": rf["sweep_only"]["flips_per_ns"], "from_mcs0": m0["value"],
+                "us_per_mcs": [ph["metropolis"], ph["houdayer"], ph["exchange"], ph["rest"]]}
+
+    per_config, summary = None, None
     if not a.no_per_config and world == 1:
-        per_config = {w.name: {"value": t["value"], "ms_per_step": t["ms_per_step"], "steps": t["steps"],
-                               "frac": roofline["frac"], "whole_mcs_frac": roofline["whole_mcs_frac"], "headline": True}}
+        per_config = {w.name: dict(compact(t, roofline, mcs0), headline=True)}
         for name in sorted(wl.CONFIGS):
             if name == w.name:
                 continue
@@ -483,13 +542,19 @@ def main():
             rc = GpuRun(a, wc, rank, world, dev, flush)
             tc = rc.timed(a.config_steps, a.warmup, sampler)
             rf = rc.instrumented(min(a.config_steps, 5), tc)
-            per_config[name] = {
-                "workload": config_of(a, wc, world)["workload"], "value": tc["value"], "unit": UNIT,
-                "ms_per_step": tc["ms_per_step"], "steps": tc["steps"], "mcs_per_step": a.mcs_per_step,
-                "gpu_launches": tc["gpu_launches"], "clocks": tc["clocks"],
-                "roofline": {k: rf[k] for k in ("kernel", "frac", "whole_mcs_frac", "flips_per_ns", "ms_per_launch", "sweep_only",
-                                                "kernel_ms", "kernel_launches", "kernel_ms_pass", "phases", "traffic", "traffic_source")},
-            }
+            per_config[name] = compact(tc, rf, rc.from_mcs0(max(a.warmup, 1)))
+        # [whole-MCS flips/ns, roofline frac of the dominant kernel, whole-MCS frac] per config; G2 / G5: the Gaussian
+        # (fixed-point, NEXT-3) model on the two Houdayer shapes C2 and C5, whole-MCS flips/ns against the same op-count peak
+        summary = {n: [per_config[n]["value"], per_config[n]["frac"], per_config[n]["whole_mcs_frac"]] for n in sorted(per_config)}
+        if not a.gaussian and a.cluster == "single":
+            import copy
+            ag = copy.copy(a)
+            ag.gaussian = True
+            for n, key in (("C2", "G2"), ("C5", "G5")):
+                rg = GpuRun(ag, wl.CONFIGS[n], rank, world, dev, flush)
+                tg = rg.timed(a.config_steps, a.warmup, sampler)
+                peak_ops = roofline["peak"]
+                summary[key] = [tg["value"], None, ALGO_OPS_PER_FLIP[wl.CONFIGS[n].d] * tg["value"] / peak_ops]
     if sampler:
         sampler.stop()
 
@@ -511,9 +576,11 @@ def main():
         "ms_per_step": t["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "int32", "data": "synthetic", "config": config_of(a, w, world),
         "clocks": t["clocks"], "e2e": e2e, "gpu_launches": t["gpu_launches"], "roofline": roofline, "cpu_baseline": cpu,
-        "per_config": per_config, "fast_path": fast_path,
+        "ms_step_stats": t["ms_step_stats"], "value_median_step": t["value_median_step"],
+        "timed_window_mcs": t["mcs"], "from_mcs0": mcs0, "fast_path": fast_path,
+        "per_config": per_config, "summary": summary,           # `summary` stays the LAST key (the driver keeps the tail)
     }
-    print(json.dumps(out))
+    print(json.dumps(shorten(out)))
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()

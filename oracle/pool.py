@@ -36,7 +36,7 @@ def run_chunk(job):
     (L, d, T, betas, seed, g0, n, n_mcs, houdayer, measure_every, checkpoints) = job[:11]
     o = ref.Oracle(L, d, n, T, np.asarray(betas, dtype=np.float64), seed, g0)
     if len(job) > 11 and job[11] is not None:       # fixed-point couplings (NEXT-3): an input of the run, drawn per global sample
-        from paper_2003_04621_b200 import workloads as wl
+        import workloads as wl
 
         fbits = int(job[11])
         o.set_couplings_fixed(wl.gaussian_couplings_fixed(seed, n, d, L ** d, fbits, sample_offset=g0), fbits)
@@ -65,7 +65,7 @@ class OraclePool:
         self.ex = ProcessPoolExecutor(max_workers=self.procs, mp_context=mp.get_context("spawn"))
 
     def submit(self, w, g0, n, n_mcs, checkpoints=(), seed=None, gaussian_fbits=None):
-        from paper_2003_04621_b200 import workloads as wl
+        import workloads as wl
 
         job = (w.L, w.d, w.T, w.betas().tolist(), wl.SEED if seed is None else seed, int(g0), int(n), int(n_mcs),
                bool(w.houdayer), int(w.measure_every), tuple(checkpoints), gaussian_fbits)
@@ -122,7 +122,7 @@ class PersistentOracles:
     """P oracle processes on disjoint sample ranges [g0 + k n, g0 + (k + 1) n), each alive across step() calls."""
 
     def __init__(self, w, procs, samples_per_proc, houdayer_mode=None, fixed=None, n_clu=None, seed=None, g0=0):
-        from paper_2003_04621_b200 import workloads as wl
+        import workloads as wl
 
         ctx = mp.get_context("spawn")
         self.procs, self.conns = [], []

@@ -1,7 +1,8 @@
 """ctypes front end of the CPU oracle (oracle/ref_ptglass.c).  TEST INFRASTRUCTURE ONLY.
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this.
-It imports nothing from the product package; the product never imports it.  Argument marshalling only --
+It imports nothing from the product package (oracle/pool.py takes shapes and beta ladders from the neutral top-level
+`workloads` module); the product never imports it.  Argument marshalling only --
 all arithmetic of the method is in ref_ptglass.c.
 """
 from __future__ import annotations

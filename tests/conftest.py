@@ -22,7 +22,7 @@ def full_length_jobs():
     early as possible (at collection, when a GPU is there and such a test is selected), so that they run on otherwise
     idle host cores while the other GPU tests execute; longest first."""
     if _full_length["jobs"] is None:
-        from paper_2003_04621_b200 import workloads as wl
+        import workloads as wl
         from oracle import pool as OP
         from oracle import ref
 

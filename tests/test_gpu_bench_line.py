@@ -16,7 +16,9 @@ def run_bench(*args):
     assert out.returncode == 0, out.stderr[-2000:]
     lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
     assert len(lines) == 1, out.stdout[-2000:]
-    return json.loads(lines[0])
+    d = json.loads(lines[0])
+    d["_line_bytes"] = len(lines[0])
+    return d
 
 
 def test_bench_line_has_the_contracted_keys():
@@ -37,7 +39,17 @@ def test_bench_line_has_the_contracted_keys():
     assert set(d["per_config"]) == {"C1", "C2", "C3", "C4", "C5"}
     for name in ("C2", "C3", "C4", "C5"):
         pc = d["per_config"][name]
-        assert pc["value"] > 100 and 0 < pc["roofline"]["frac"] < 1 and pc["clocks"] is not None
+        assert pc["value"] > 100 and 0 < pc["frac"] < 1 and pc["sm_mhz"] is not None and pc["from_mcs0"] > 0
+        st = pc["ms_step_stats"]
+        assert 0 < st["min"] <= st["median"] <= st["max"]
+    # SURVEY 8(d) timing protocol: per-step statistics, the steady-state window and the run from MCS 0
+    assert 0 < d["ms_step_stats"]["min"] <= d["ms_step_stats"]["median"] <= d["ms_step_stats"]["max"]
+    assert d["timed_window_mcs"][0] >= 128 and d["from_mcs0"]["mcs"][0] == 0 and d["from_mcs0"]["value"] > 0
+    # the driver keeps the TAIL of the line: every config's figures sit in `summary`, the last key, and the line is short
+    assert list(d)[-2] == "summary" and d["_line_bytes"] < 6144, d["_line_bytes"]
+    assert set(d["summary"]) == {"C1", "C2", "C3", "C4", "C5", "G2", "G5"}
+    for name, (value, frac, whole) in d["summary"].items():
+        assert value > 0 and 0 < whole < 1 and (frac is None or 0 < frac < 1), name
 
 
 def test_reference_arm_prints_the_oracle_line():

@@ -6,7 +6,7 @@ import pytest
 from oracle import ref
 from paper_2003_04621_b200 import binding as B
 from paper_2003_04621_b200 import build as build_mod
-from paper_2003_04621_b200 import workloads as wl
+import workloads as wl
 
 pytestmark = pytest.mark.gpu
 

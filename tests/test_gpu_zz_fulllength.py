@@ -12,7 +12,7 @@ import pytest
 
 from paper_2003_04621_b200 import binding as B
 from paper_2003_04621_b200 import build as build_mod
-from paper_2003_04621_b200 import workloads as wl
+import workloads as wl
 from oracle import pool as OP
 from tests.conftest import FULL_LENGTH_SAMPLES, full_length_jobs
 

@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 from oracle import ref
-from paper_2003_04621_b200 import workloads as wl
+import workloads as wl
 from tests import helpers as H
 
 SEED = wl.SEED

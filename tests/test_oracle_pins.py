@@ -9,7 +9,7 @@ import numpy as np
 import pytest
 
 from oracle import ref
-from paper_2003_04621_b200 import workloads as wl
+import workloads as wl
 from tests import helpers as H
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")

@@ -3,7 +3,7 @@ is the concatenation of runs over disjoint `sample_offset` ranges (SURVEY 8(c).1
 import numpy as np
 
 from oracle import ref
-from paper_2003_04621_b200 import workloads as wl
+import workloads as wl
 from oracle import pool as OP
 
 

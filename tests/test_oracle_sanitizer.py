@@ -18,7 +18,7 @@ ref.build = lambda force=False: %(lib)r          # the sanitised build instead o
 from tests import test_oracle_pins as pins
 pins.test_survey_worked_examples()
 import numpy as np
-from paper_2003_04621_b200 import workloads as wl
+import workloads as wl
 o = ref.Oracle(4, 3, 2, 5, wl.betas_geometric(0.3, 1.5, 5), wl.SEED, 1)
 o.mcs(6, 1, True, True)
 o.houdayer_multi_step()

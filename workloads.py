@@ -2,7 +2,8 @@
 
 This module holds NO arithmetic of the method: it only names shapes and builds the `betas` arrays that the
 harness passes, unchanged, to both the CUDA library and the CPU oracle.  It is the only
-module the tests' two sides share.  No public dataset is involved: the paper's workloads are random +-J samples
+module the tests' two sides share, and it belongs to neither: it sits at the repo root, outside the product package and
+outside oracle/.  No public dataset is involved: the paper's workloads are random +-J samples
 generated in-program; couplings and spins are drawn from `SEED` by each side's own Philox.
 """
 from __future__ import annotations
