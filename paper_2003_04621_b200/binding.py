@@ -1,4 +1,4 @@
-"""Thin Python binding of the C ABI in include/ptglass.h: same names, argument marshalling only.
+"""Thin Python binding of the C ABI in include/ptglass.h (and the probes of include/ptglass_diag.h): same names, argument marshalling only.
 
 Every step of the path runs in the CUDA kernels of libptglass.so.  PyTorch is used for exactly two things: the
 device workspace (one uint8 tensor) and the CUDA stream.  There is no CPU fallback: if the shared library is
@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libptglass.so")
 
 PT_OK, PT_ERR_ARG, PT_ERR_STATE, PT_ERR_OVERFLOW, PT_ERR_CUDA = 0, -1, -2, -3, -4
 
-# every symbol include/ptglass.h declares: name -> (restype, argtypes)
+# every symbol include/ptglass.h and include/ptglass_diag.h (probes) declare: name -> (restype, argtypes)
 _vp, _i, _sz = C.c_void_p, C.c_int, C.c_size_t
 SYMBOLS = {
     "pt_workspace_bytes": (_i, [_i, _i, _i, _i, C.POINTER(_sz)]),

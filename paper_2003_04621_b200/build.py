@@ -9,7 +9,7 @@ CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libptglass.so")
 SOURCES = [os.path.join(CSRC, "ptglass.cu"), os.path.join(CSRC, "microbench.cu")]
 DEPS = SOURCES + sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cuh")) + [
-    os.path.join(os.path.dirname(_HERE), "include", "ptglass.h")]
+    os.path.join(os.path.dirname(_HERE), "include", "ptglass.h"), os.path.join(os.path.dirname(_HERE), "include", "ptglass_diag.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
 

@@ -2,6 +2,7 @@
 // Measures, on the bound stream with CUDA events, how many 32-bit integer thread-operations per second the
 // GPU sustains for the instruction kinds the Metropolis sweep is made of.
 #include "../../include/ptglass.h"
+#include "../../include/ptglass_diag.h"
 
 #include <cuda_runtime.h>
 #include <stdint.h>

@@ -2,6 +2,7 @@
 // workspace carving, kernel dispatch.  No device memory is allocated here (the caller owns the workspace) and
 // there is no CPU fallback: every step of the path runs in the kernels of kernels.cuh.
 #include "../../include/ptglass.h"
+#include "../../include/ptglass_diag.h"
 
 #include <cuda_runtime.h>
 

@@ -1,4 +1,4 @@
-"""The C-ABI shared library loads and exports every symbol include/ptglass.h declares; argument and state errors
+"""The C-ABI shared library loads and exports every symbol include/ptglass.h and include/ptglass_diag.h declare; argument and state errors
 are reported without a GPU.  No compute calls here."""
 import os
 import re
@@ -20,6 +20,12 @@ def lib():
 
 def test_header_symbols_all_exported(lib):
     hdr = open(os.path.join(ROOT, "include", "ptglass.h")).read()
+    diag = open(os.path.join(ROOT, "include", "ptglass_diag.h")).read()
+    # the probes live in their own header: the method's header declares none of them
+    for probe in ("pt_microbench", "pt_philox_selftest", "pt_threshold_selftest", "pt_force_general_path", "pt_is_dev_build"):
+        assert re.search(r"\b%s\s*\(" % probe, re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)) is None, probe
+        assert re.search(r"\b%s\s*\(" % probe, diag), probe
+    hdr = hdr + diag
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
     names = set(re.findall(r"\b(pt_[a-z_]+|houdayer_step|houdayer_multi_step)\s*\(", hdr))
     assert names == set(B.SYMBOLS), names ^ set(B.SYMBOLS)
