@@ -215,3 +215,33 @@ def test_gaussian_with_cluster_variants_and_records(L, d, S, T, general):
         assert np.array_equal(Qo, Qr.cpu().numpy()[r]) and np.array_equal(QLo, QLr.cpu().numpy()[r])
     o.mcs(1, 1, 1, True)
     same_state(o, "records")
+
+
+def test_int32_couplings_are_laid_out_by_flag_never_by_spare_bytes():
+    """pt_init lays the int32 coupling arrays out iff pt_set_workspace_flags(PT_WS_FIXED_COUPLINGS) asked for them: a
+    workspace with room to spare does not get them unasked, and a workspace too small for what was asked is refused."""
+    import torch
+    L, d, S, T = 8, 2, 2, 4
+    betas = wl.betas_linear(0.2, 1.0, T)
+    Jq = wl.gaussian_couplings_fixed(wl.SEED, S, d, L * L, 16)
+    big = torch.empty(B.pt_workspace_bytes_ex(L, d, S, T, B.PT_WS_FIXED_COUPLINGS), dtype=torch.uint8, device="cuda:0")
+    B.pt_bind(big)
+    B.pt_init(L, d, S, T, betas, wl.SEED)                      # room for the arrays, but nobody asked
+    assert B.pt_get_stage_bytes() > 0
+    with pytest.raises(B.PTError) as e:
+        B.pt_set_couplings_fixed(Jq, 16)
+    assert e.value.code == B.PT_ERR_STATE and "pt_set_workspace_flags" in str(e.value)
+    B.pt_bind(big)                                             # re-binding resets the flags
+    B.pt_set_workspace_flags(B.PT_WS_FIXED_COUPLINGS)
+    B.pt_init(L, d, S, T, betas, wl.SEED)
+    B.pt_set_couplings_fixed(Jq, 16)
+    assert np.array_equal(B.pt_get_couplings_fixed()[0], Jq)
+    small = torch.empty(B.pt_workspace_bytes(L, d, S, T), dtype=torch.uint8, device="cuda:0")
+    B.pt_bind(small)
+    B.pt_set_workspace_flags(B.PT_WS_FIXED_COUPLINGS)
+    with pytest.raises(B.PTError) as e:
+        B.pt_init(L, d, S, T, betas, wl.SEED)
+    assert e.value.code == B.PT_ERR_STATE
+    with pytest.raises(B.PTError) as e:
+        B.pt_set_workspace_flags(64)
+    assert e.value.code == B.PT_ERR_ARG
